@@ -1,0 +1,242 @@
+"""CPU ORACLE (test infrastructure, NOT the product) -- ctypes front end of tgs_oracle.c.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` /
+``--impl reference`` legs may import this package.  It never imports the CUDA package
+``paper_2606_15924_b200`` and shares no code with it; cameras are duck-typed (any object
+with ``width height fx fy cx cy R t znear bg``), scenes come from ``workloads``.
+
+Two builds of the same C source: ``Oracle("f32")`` (the parity referee, discrete decisions in
+the kernel's precision) and ``Oracle("f64")`` (finite differences, cross-checks).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from types import SimpleNamespace
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tgs_oracle.c")
+
+
+def _lib_path(prec: str) -> str:
+    return os.path.join(_HERE, f"liboracle_{prec}.so")
+
+
+def build(force: bool = False) -> None:
+    """Compile both precisions with gcc.  -ffp-contract=off: no implicit FMA contraction;
+    -mfma only lets the explicit fma()/fmaf() calls inline (the result is the same either way,
+    fma is exactly specified)."""
+    has_fma = False
+    try:
+        with open("/proc/cpuinfo") as f:
+            has_fma = " fma " in f.read().replace("\n", " ")
+    except OSError:
+        pass
+    for prec, define in (("f32", []), ("f64", ["-DORC_F64"])):
+        out = _lib_path(prec)
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(_SRC):
+            continue
+        cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
+               "-Wall", "-Wno-unused-function"] + (["-mfma"] if has_fma else []) + define + \
+              [_SRC, "-o", out + ".tmp", "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(out + ".tmp", out)
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(C.c_void_p)
+
+
+class Oracle:
+    def __init__(self, precision: str = "f32"):
+        assert precision in ("f32", "f64")
+        build()
+        self.precision = precision
+        self.real = np.float32 if precision == "f32" else np.float64
+        self._creal = C.c_float if precision == "f32" else C.c_double
+        self.lib = C.CDLL(_lib_path(precision))
+        assert self.lib.orc_real_bytes() == np.dtype(self.real).itemsize
+        self.lib.orc_bin_sort.restype = C.c_int64
+        self.lib.orc_mix64.restype = C.c_uint64
+        self.lib.orc_mix64.argtypes = [C.c_uint64, C.c_uint64]
+
+        class Cam(C.Structure):
+            _fields_ = [("W", C.c_int32), ("H", C.c_int32), ("fx", self._creal), ("fy", self._creal),
+                        ("cx", self._creal), ("cy", self._creal), ("Rcw", self._creal * 9),
+                        ("tau", self._creal * 3), ("znear", self._creal), ("bg", self._creal * 3)]
+        self._Cam = Cam
+
+    # ---- helpers -------------------------------------------------------------------------
+    def r(self, a):
+        return np.ascontiguousarray(np.asarray(a), dtype=self.real)
+
+    def cam(self, cam):
+        c = self._Cam()
+        c.W, c.H = int(cam.width), int(cam.height)
+        # every camera scalar is first rounded to fp32 (the boundary type of the CUDA library)
+        f = lambda v: float(np.float32(v))
+        c.fx, c.fy, c.cx, c.cy, c.znear = f(cam.fx), f(cam.fy), f(cam.cx), f(cam.cy), f(cam.znear)
+        R = np.asarray(cam.R, dtype=np.float32).reshape(9)
+        t = np.asarray(cam.t, dtype=np.float32).reshape(3)
+        bg = np.asarray(cam.bg, dtype=np.float32).reshape(3)
+        for i in range(9):
+            c.Rcw[i] = float(R[i])
+        for i in range(3):
+            c.tau[i] = float(t[i])
+            c.bg[i] = float(bg[i])
+        return c
+
+    @staticmethod
+    def grid(cam):
+        return ((cam.width + 15) // 16, (cam.height + 15) // 16)
+
+    # ---- O1 ------------------------------------------------------------------------------
+    def preprocess(self, cam, sh_degree, means3D, scales, quats, opacities, sh):
+        N = int(np.asarray(means3D).shape[0])
+        K = (sh_degree + 1) ** 2
+        mu, sc, q, op = self.r(means3D), self.r(scales), self.r(quats), self.r(opacities)
+        shc = self.r(sh).reshape(N, K, 3)
+        o = SimpleNamespace(
+            means2D=np.zeros((N, 2), self.real), depths=np.zeros(N, self.real),
+            conic_opacity=np.zeros((N, 4), self.real), rgb=np.zeros((N, 3), self.real),
+            radii=np.zeros(N, np.int32), rect=np.zeros((N, 4), np.int32),
+            tiles_touched=np.zeros(N, np.uint32), clamped=np.zeros(N, np.uint8))
+        c = self.cam(cam)
+        self.lib.orc_preprocess(C.byref(c), N, sh_degree, _ptr(mu), _ptr(sc), _ptr(q), _ptr(op), _ptr(shc),
+                                _ptr(o.means2D), _ptr(o.depths), _ptr(o.conic_opacity), _ptr(o.rgb),
+                                _ptr(o.radii), _ptr(o.rect), _ptr(o.tiles_touched), _ptr(o.clamped))
+        return o
+
+    # ---- O2 ------------------------------------------------------------------------------
+    def bin_sort(self, cam, pre):
+        N = pre.depths.shape[0]
+        gx, gy = self.grid(cam)
+        P = int(pre.tiles_touched.astype(np.int64).sum())
+        keys = np.zeros(max(P, 1), np.uint64)
+        gid = np.zeros(max(P, 1), np.uint32)
+        offs = np.zeros(gx * gy + 1, np.uint32)
+        c = self.cam(cam)
+        P2 = self.lib.orc_bin_sort(C.byref(c), N, _ptr(self.r(pre.depths)), _ptr(pre.rect),
+                                   _ptr(pre.tiles_touched), _ptr(keys), _ptr(gid), _ptr(offs))
+        assert P2 == P
+        return SimpleNamespace(P=P, keys_sorted=keys[:P], gid_sorted=gid[:P], tile_offsets=offs)
+
+    # ---- O3 ------------------------------------------------------------------------------
+    def sample(self, cam, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, err=None, render=None, target=None):
+        H, W = cam.height, cam.width
+        gx, gy = self.grid(cam)
+        T = gx * gy
+        qerr = np.zeros(H * W, np.uint32)
+        score = np.zeros(T, np.uint64)
+        tiles = np.zeros(T, np.uint32)
+        tpo = np.zeros(T + 1, np.uint32)
+        pix = np.zeros(H * W, np.uint32)
+        kn = np.zeros(2, np.int32)
+        e = None if err is None else self.r(err).reshape(H, W)
+        rd = None if render is None else self.r(render).reshape(H, W, 3)
+        tg = None if target is None else self.r(target).reshape(H, W, 3)
+        assert e is not None or (rd is not None and tg is not None)
+        c = self.cam(cam)
+        self.lib.orc_sample(C.byref(c), _ptr(e), _ptr(rd), _ptr(tg), int(tile_pct[0]), int(tile_pct[1]),
+                            int(pixel_mode), int(pix_rate[0]), int(pix_rate[1]), C.c_uint64(seed),
+                            _ptr(qerr), _ptr(score), _ptr(tiles), _ptr(tpo), _ptr(pix), _ptr(kn))
+        k, n = int(kn[0]), int(kn[1])
+        return SimpleNamespace(k=k, n=n, qerr=qerr.reshape(H, W), tile_score=score, tiles=tiles[:k].copy(),
+                               tile_pix_offsets=tpo[:k + 1].copy(), pix=pix[:n].copy())
+
+    # ---- O4 ------------------------------------------------------------------------------
+    def raster_fwd(self, cam, binned, pre, samp):
+        n = samp.n
+        o = SimpleNamespace(color=np.zeros((n, 3), self.real), T=np.zeros(n, self.real),
+                            n_contrib=np.zeros(n, np.uint32), n_walked=np.zeros(n, np.uint32),
+                            margin=np.ones((n, 2), self.real))
+        c = self.cam(cam)
+        self.lib.orc_raster_fwd(C.byref(c), _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
+                                _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.rgb)),
+                                samp.k, _ptr(samp.tiles), _ptr(samp.tile_pix_offsets), _ptr(samp.pix),
+                                _ptr(o.color), _ptr(o.T), _ptr(o.n_contrib), _ptr(o.n_walked), _ptr(o.margin))
+        return o
+
+    # ---- O5 ------------------------------------------------------------------------------
+    def raster_bwd(self, cam, binned, pre, samp, fwd, dL_dcolor):
+        N = pre.means2D.shape[0]
+        g = self.r(dL_dcolor).reshape(samp.n, 3)
+        o = SimpleNamespace(dL_dmeans2D=np.zeros((N, 2), self.real), dL_dconic=np.zeros((N, 3), self.real),
+                            dL_dopacity=np.zeros(N, self.real), dL_drgb=np.zeros((N, 3), self.real))
+        c = self.cam(cam)
+        self.lib.orc_raster_bwd(C.byref(c), N, _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
+                                _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.rgb)),
+                                samp.k, _ptr(samp.tiles), _ptr(samp.tile_pix_offsets), _ptr(samp.pix),
+                                _ptr(self.r(fwd.T)), _ptr(fwd.n_contrib), _ptr(g),
+                                _ptr(o.dL_dmeans2D), _ptr(o.dL_dconic), _ptr(o.dL_dopacity), _ptr(o.dL_drgb))
+        return o
+
+    # ---- O6 ------------------------------------------------------------------------------
+    def project_bwd(self, cam, sh_degree, means3D, scales, quats, sh, radii, clamped,
+                    dL_dmeans2D, dL_dconic, dL_drgb):
+        N = int(np.asarray(means3D).shape[0])
+        K = (sh_degree + 1) ** 2
+        o = SimpleNamespace(dL_dmeans3D=np.zeros((N, 3), self.real), dL_dscales=np.zeros((N, 3), self.real),
+                            dL_dquats=np.zeros((N, 4), self.real), dL_dsh=np.zeros((N, K, 3), self.real))
+        c = self.cam(cam)
+        self.lib.orc_project_bwd(C.byref(c), N, sh_degree, _ptr(self.r(means3D)), _ptr(self.r(scales)),
+                                 _ptr(self.r(quats)), _ptr(self.r(sh).reshape(N, K, 3)),
+                                 _ptr(np.ascontiguousarray(radii, np.int32)),
+                                 _ptr(np.ascontiguousarray(clamped, np.uint8)),
+                                 _ptr(self.r(dL_dmeans2D)), _ptr(self.r(dL_dconic)), _ptr(self.r(dL_drgb)),
+                                 _ptr(o.dL_dmeans3D), _ptr(o.dL_dscales), _ptr(o.dL_dquats), _ptr(o.dL_dsh))
+        return o
+
+    def render_dense(self, cam, binned, pre):
+        img = np.zeros((cam.height, cam.width, 3), self.real)
+        c = self.cam(cam)
+        self.lib.orc_render_dense(C.byref(c), _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
+                                  _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.rgb)),
+                                  _ptr(img))
+        return img
+
+    # ---- small exported helpers (pinned individually) ---------------------------------------
+    def quat_to_R(self, q):
+        R = np.zeros(9, self.real)
+        self.lib.orc_quat_to_R(_ptr(self.r(q)), _ptr(R))
+        return R.reshape(3, 3)
+
+    def cov3d(self, s, q):
+        S = np.zeros(9, self.real)
+        self.lib.orc_cov3d(_ptr(self.r(s)), _ptr(self.r(q)), _ptr(S))
+        return S.reshape(3, 3)
+
+    def sh_basis(self, d):
+        B = np.zeros(16, self.real)
+        self.lib.orc_sh_basis(_ptr(self.r(d)), _ptr(B))
+        return B
+
+    def mix64(self, seed, idx):
+        return int(self.lib.orc_mix64(seed, idx))
+
+    # ---- whole path --------------------------------------------------------------------------
+    def pipeline(self, scene, dL_dcolor=None, backward=True):
+        """preprocess -> bin_sort -> sample -> fwd -> (bwd) on a ``workloads.Scene``."""
+        cam = scene.cam
+        pre = self.preprocess(cam, scene.sh_degree, scene.means3D, scene.scales, scene.quats,
+                              scene.opacities, scene.sh)
+        binned = self.bin_sort(cam, pre)
+        if scene.err is not None:
+            samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
+                               err=scene.err)
+        else:
+            render = self.render_dense(cam, binned, pre)
+            samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
+                               render=render, target=scene.target)
+        fwd = self.raster_fwd(cam, binned, pre, samp)
+        out = SimpleNamespace(pre=pre, binned=binned, samp=samp, fwd=fwd, rbwd=None, pbwd=None)
+        if backward:
+            g = dL_dcolor if dL_dcolor is not None else np.ones((samp.n, 3), np.float32)
+            out.rbwd = self.raster_bwd(cam, binned, pre, samp, fwd, g)
+            out.pbwd = self.project_bwd(cam, scene.sh_degree, scene.means3D, scene.scales, scene.quats, scene.sh,
+                                        pre.radii, pre.clamped, out.rbwd.dL_dmeans2D, out.rbwd.dL_dconic,
+                                        out.rbwd.dL_drgb)
+        return out
