@@ -1,0 +1,156 @@
+/*
+ * tgs.h -- C ABI of the B200-native TurboGS sparse-pixel rasterisation hot path.
+ *
+ * The five calls follow the paper's statement of one training iteration's rasterisation
+ * (PAPER.md = arxiv/paper_2606_15924 text; SURVEY.md section 8 is the scope table):
+ *
+ *   tgs_preprocess         EWA projection of 3D Gaussians to 2D splats      PAPER.md:62-64 (Sec. 3.1), 75
+ *   tgs_bin_sort           (tile, depth)-ordered Gaussian lists per tile    PAPER.md:64   ("K(p) ... sorted by depth")
+ *   tgs_sample             error-guided tile / pixel selection              PAPER.md:73, 93 (Eq. 2), 128-150 (Sec. 3.5), 156
+ *   tgs_raster_fwd_sparse  Eq. 1 alpha compositing on sampled pixels only   PAPER.md:66 (Eq. 1), 154-166 (Sec. 3.6, Fig. 6)
+ *   tgs_raster_bwd_sparse  its analytic backward + the projection chain     PAPER.md:69, 75, 166, 441 (Alg. 1 step 8)
+ *
+ * Conventions (all calls)
+ *   - Plain C, no C++/torch types.  Every pointer is a DEVICE pointer unless its name ends in
+ *     `_host` (then it is a HOST pointer, pinned or pageable) or it is `const tgs_camera*`
+ *     (host struct, copied by value into the launch).  The caller owns every buffer; nothing is
+ *     allocated per call and no pointer is retained after the call returns.
+ *   - `stream` is a cudaStream_t passed as void*.  Calls only enqueue work; they do not
+ *     synchronise, EXCEPT when a non-NULL `*_host` output is given (one cudaStreamSynchronize).
+ *     All calls are CUDA-graph capturable when the `_host` outputs are NULL.
+ *   - fp32 only, 16x16 tiles only, sh_degree in {0,1,2,3}.  Anything else returns
+ *     TGS_ERR_UNSUPPORTED.  There is no CPU fallback.
+ *   - Return value: TGS_OK or an error code; tgs_last_error(ctx) holds a message.
+ *   - Tile grid: gx = ceil(W/16), gy = ceil(H/16), T = gx*gy, tile_id = ty*gx + tx.
+ *   - Pixel (x, y) is sampled at the integer point (x, y); linear pixel index = y*W + x.
+ *   - Parameters are ACTIVATED: scales > 0, unit quaternions (w,x,y,z), opacities in (0,1);
+ *     gradients are w.r.t. those activated values (exp / sigmoid / normalise belong to the optimiser).
+ */
+#ifndef TGS_H_
+#define TGS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tgs_ctx tgs_ctx;
+
+/* One pinhole view.  R, t map world to camera: t_cam = R * x_world + t (R row-major). */
+typedef struct tgs_camera {
+    int32_t width, height;
+    float fx, fy, cx, cy;
+    float R[9];
+    float t[3];
+    float znear; /* Gaussians with camera-space z <= znear are culled (0.2 in the 3DGS kernels) */
+    float bg[3]; /* background colour added as T_final * bg */
+} tgs_camera;
+
+enum {
+    TGS_OK = 0,
+    TGS_ERR_INVALID_ARG = 1, /* NULL required pointer, non-positive size, bad fraction ...       */
+    TGS_ERR_CAPACITY = 2,    /* a caller buffer / workspace is too small (message says how much) */
+    TGS_ERR_CUDA = 3,        /* a CUDA runtime call or launch failed                             */
+    TGS_ERR_UNSUPPORTED = 4  /* sh_degree > 3, T > 2^20, P_capacity >= 2^32, ...                 */
+};
+
+enum { TGS_PIXELS_ALL = 0, TGS_PIXELS_BERNOULLI_ERR = 1 };
+
+/* Projected splat record, 12 x 32-bit words, 48 B, one per Gaussian (float4-aligned):
+ *   [0] mean2D.x  [1] mean2D.y  [2] conic A   [3] conic B
+ *   [4] conic C   [5] opacity   [6] red       [7] green
+ *   [8] blue      [9] depth t_z [10] rect_x = x0 | x1<<16 (uint32 bits)  [11] rect_y = y0 | y1<<16
+ * conic = inverse of the dilated 2D covariance [[A,B],[B,C]]; the Gaussian covers tiles
+ * x0 <= tx < x1, y0 <= ty < y1; a culled Gaussian has all 12 words zero. */
+#define TGS_SPLAT_WORDS 12
+/* Gradient record written by the raster half of tgs_raster_bwd_sparse, same stride:
+ *   [0..1] dL/dmean2D  [2..4] dL/d(A,B,C)  [5] dL/dopacity  [6..8] dL/drgb  [9..11] unused (0) */
+
+int tgs_create(tgs_ctx** ctx, int device);
+int tgs_destroy(tgs_ctx* ctx);
+const char* tgs_last_error(const tgs_ctx* ctx);
+const char* tgs_version(void);
+
+/* ---- a1: projection -------------------------------------------------------
+ * in : means3D[N,3] scales[N,3] quats[N,4] opacities[N] sh[N,K,3], K=(sh_degree+1)^2 (coefficient
+ *      major, channel minor; sh must be 16-byte aligned).
+ * out: splats[N,12] (layout above), radii[N] (int32, ceil(3 sigma_max), 0 = culled),
+ *      clamped[N] (bit c set <=> colour channel c was clamped at 0).
+ * The rect / depth / mean2D words are computed in a fixed, FMA-free fp32 expression order so that
+ * they are bit-reproducible. */
+int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree,
+                   const float* means3D, const float* scales, const float* quats,
+                   const float* opacities, const float* sh,
+                   float* splats, int32_t* radii, uint8_t* clamped, void* stream);
+
+/* ---- a2: binning + sort ------------------------------------------------------
+ * Produces the list of all (tile, Gaussian) pairs ordered by (tile_id, depth bits, Gaussian id):
+ *   gid_sorted[P], tile_offsets[T+1] (CSR: tile t owns [tile_offsets[t], tile_offsets[t+1])),
+ *   keys_sorted[P] = tile_id<<32 | float_bits(depth)   (optional, may be NULL).
+ * P = sum of tiles touched is data dependent: P_dev[0] = P, P_dev[1] = 1 if P > P_capacity (then
+ * the lists are invalid and, if P_host != NULL, the call returns TGS_ERR_CAPACITY).  P_host (host,
+ * nullable) receives P and forces one stream synchronisation.
+ * The sort is a hand-written stable LSD radix sort; because the low 32 key bits (depth) depend on
+ * the Gaussian only, those digit passes run on the N Gaussians BEFORE duplication and only the
+ * tile-id digits run on the P pairs (same result as sorting the 64-bit keys). */
+int tgs_bin_sort_workspace_bytes(int N, int64_t P_capacity, int num_tiles, size_t* bytes);
+int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                 int64_t P_capacity, uint64_t* keys_sorted, uint32_t* gid_sorted,
+                 uint32_t* tile_offsets, int64_t* P_dev, int64_t* P_host,
+                 void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a3: error-guided sampling (BASELINE.json configs) --------------
+ * Per-pixel error e(p) = err[y*W+x] if err != NULL, else sum_c |render - target| (Eq. 2).
+ * Fixed point q = trunc(clamp(e,0,15.999) * 2^20); tile score = (sum q << 8) / #pixels-in-image.
+ * Selects k = max(1, floor(pct_num*T/pct_den)) tiles by (score desc, tile_id asc), outputs them
+ * ascending in tiles[k]; per selected tile the pixel list (ALL in-image pixels, or
+ * BERNOULLI_ERR: keep iff u16(p)*S*den < num*cnt*q16(p)*2^16, at least one pixel per tile), in
+ * ascending local index, concatenated in pix[n]; tile_pix_offsets[k+1] is its CSR.
+ * Capacities: tile_score[T], tiles[T], tile_pix_offsets[T+1], pix[W*H].  kn_dev[0]=k, kn_dev[1]=n. */
+int tgs_sample_num_tiles(const tgs_camera* cam, int tile_pct_num, int tile_pct_den);
+int tgs_sample_workspace_bytes(const tgs_camera* cam, size_t* bytes);
+int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam,
+               const float* err, const float* render, const float* target,
+               int tile_pct_num, int tile_pct_den, int pixel_mode,
+               int pix_rate_num, int pix_rate_den, uint64_t seed,
+               uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+               int32_t* kn_dev, int32_t* kn_host,
+               void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- a4: sparse forward (Eq. 1, 154-166) ---------------------------------------
+ * For each sampled pixel p of sampled tile tiles[i]: front-to-back over the tile's range,
+ *   alpha = min(0.99, o * exp(-1/2 d^T conic d)), skipped if alpha < 1/255, stop before the
+ *   Gaussian that would take T below 1e-4;  color = sum c alpha T + T_final * bg.
+ * out_color[n,3], out_T[n] (T_final), n_contrib[n] (1-based position in the tile range of the last
+ * Gaussian composited, 0 = none), n_walked[n] (optional, NULL ok: range entries visited).
+ * k is the host-known tile count (tgs_sample_num_tiles); n is read from tile_pix_offsets[k]. */
+int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                          const uint32_t* tile_offsets, const uint32_t* gid_sorted,
+                          int k, const uint32_t* tiles, const uint32_t* tile_pix_offsets,
+                          const uint32_t* pix,
+                          float* out_color, float* out_T, uint32_t* n_contrib, uint32_t* n_walked,
+                          void* stream);
+
+/* ---- a5 + a6: sparse backward ----------------------------------
+ * Raster half: back-to-front replay from n_contrib, accumulating into dL_dsplats[N,12] (zeroed
+ * inside the call).  Projection half: chains dL_dsplats through tgs_preprocess to
+ * dL_dmeans3D[N,3] dL_dscales[N,3] dL_dquats[N,4] dL_dopacities[N] dL_dsh[N,K,3]; it is skipped when
+ * dL_dmeans3D == NULL (then only dL_dsplats is produced).  Derivatives are those of the forward as
+ * defined: zero through an active 0.99 alpha clamp, an active colour clamp and for culled Gaussians. */
+int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree,
+                          const float* splats, const uint32_t* tile_offsets, const uint32_t* gid_sorted,
+                          int k, const uint32_t* tiles, const uint32_t* tile_pix_offsets,
+                          const uint32_t* pix,
+                          const float* out_T, const uint32_t* n_contrib, const float* dL_dcolor,
+                          const float* means3D, const float* scales, const float* quats,
+                          const float* sh, const int32_t* radii, const uint8_t* clamped,
+                          float* dL_dsplats,
+                          float* dL_dmeans3D, float* dL_dscales, float* dL_dquats,
+                          float* dL_dopacities, float* dL_dsh, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TGS_H_ */

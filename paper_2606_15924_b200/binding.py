@@ -1,0 +1,247 @@
+"""Thin ctypes binding of libtgs.so (include/tgs.h).  Argument marshalling only: every step of
+the hot path runs in the CUDA kernels; torch is used for device memory and streams.
+
+There is no fallback: importing this module without the built library, or creating a context
+without a CUDA device, raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from types import SimpleNamespace
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtgs.so")
+
+SPLAT_WORDS = 12
+PIXELS_ALL = 0
+PIXELS_BERNOULLI_ERR = 1
+
+ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "TGS_ERR_CUDA",
+             4: "TGS_ERR_UNSUPPORTED"}
+
+# every symbol include/tgs.h declares (tests check the library exports them all)
+SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_preprocess",
+           "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
+           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse"]
+
+
+class TgsError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{ERR_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+class Camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("cx", C.c_float), ("cy", C.c_float), ("R", C.c_float * 9), ("t", C.c_float * 3),
+                ("znear", C.c_float), ("bg", C.c_float * 3)]
+
+    @staticmethod
+    def of(cam) -> "Camera":
+        """From any object with width height fx fy cx cy R t znear bg (e.g. workloads.Camera)."""
+        if isinstance(cam, Camera):
+            return cam
+        c = Camera()
+        c.width, c.height = int(cam.width), int(cam.height)
+        c.fx, c.fy, c.cx, c.cy, c.znear = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy), float(cam.znear)
+        R = [float(v) for v in list(getattr(cam.R, "reshape", lambda *_: cam.R)(-1))]
+        for i in range(9):
+            c.R[i] = R[i]
+        for i in range(3):
+            c.t[i] = float(cam.t[i])
+            c.bg[i] = float(cam.bg[i])
+        return c
+
+    @property
+    def grid(self):
+        return ((self.width + 15) // 16, (self.height + 15) // 16)
+
+    @property
+    def num_tiles(self):
+        gx, gy = self.grid
+        return gx * gy
+
+
+def load_library() -> C.CDLL:
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_15924_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, u64 = C.c_void_p, C.c_int, C.c_int64, C.c_uint64
+    lib.tgs_create.argtypes = [C.POINTER(vp), i32]
+    lib.tgs_destroy.argtypes = [vp]
+    lib.tgs_last_error.argtypes = [vp]
+    lib.tgs_last_error.restype = C.c_char_p
+    lib.tgs_version.restype = C.c_char_p
+    cam = C.POINTER(Camera)
+    lib.tgs_preprocess.argtypes = [vp, cam, i32, i32] + [vp] * 5 + [vp] * 3 + [vp]
+    lib.tgs_bin_sort_workspace_bytes.argtypes = [i32, i64, i32, C.POINTER(C.c_size_t)]
+    lib.tgs_bin_sort.argtypes = [vp, cam, i32, vp, i64, vp, vp, vp, vp, C.POINTER(i64), vp, C.c_size_t, vp]
+    lib.tgs_sample_num_tiles.argtypes = [cam, i32, i32]
+    lib.tgs_sample_workspace_bytes.argtypes = [cam, C.POINTER(C.c_size_t)]
+    lib.tgs_sample.argtypes = [vp, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp,
+                               C.POINTER(C.c_int32), vp, C.c_size_t, vp]
+    lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
+                                         [vp] + [vp] * 5 + [vp]
+    return lib
+
+
+def _p(t):
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device, contiguous tensors only"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class TGS:
+    """One library context on one CUDA device.  Method names are the C-ABI names without `tgs_`."""
+
+    def __init__(self, device: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2606_15924_b200 needs a CUDA device (no CPU fallback)")
+        self.lib = load_library()
+        self.device = torch.device("cuda", device)
+        torch.cuda.set_device(self.device)
+        torch.cuda.current_stream()  # make sure the primary context exists
+        h = C.c_void_p()
+        rc = self.lib.tgs_create(C.byref(h), device)
+        if rc != 0:
+            raise TgsError(rc, "tgs_create failed")
+        self._h = h
+
+    def __del__(self):
+        h = getattr(self, "_h", None)
+        if h:
+            self.lib.tgs_destroy(h)
+            self._h = None
+
+    def _check(self, rc):
+        if rc != 0:
+            raise TgsError(rc, self.lib.tgs_last_error(self._h).decode())
+
+    # ---- a1 ----
+    def preprocess(self, cam, sh_degree, means3D, scales, quats, opacities, sh, out=None, stream=None):
+        cam = Camera.of(cam)
+        N = means3D.shape[0]
+        if out is None:
+            out = SimpleNamespace(splats=torch.empty((N, SPLAT_WORDS), dtype=torch.float32, device=self.device),
+                                  radii=torch.empty(N, dtype=torch.int32, device=self.device),
+                                  clamped=torch.empty(N, dtype=torch.uint8, device=self.device))
+        self._check(self.lib.tgs_preprocess(self._h, C.byref(cam), N, sh_degree, _p(means3D), _p(scales), _p(quats),
+                                            _p(opacities), _p(sh), _p(out.splats), _p(out.radii), _p(out.clamped),
+                                            _stream(stream)))
+        return out
+
+    # ---- a2 ----
+    def bin_sort_workspace_bytes(self, N, P_capacity, num_tiles):
+        b = C.c_size_t()
+        rc = self.lib.tgs_bin_sort_workspace_bytes(N, P_capacity, num_tiles, C.byref(b))
+        if rc != 0:
+            raise TgsError(rc, "tgs_bin_sort_workspace_bytes")
+        return b.value
+
+    def bin_sort(self, cam, splats, P_capacity, want_keys=False, out=None, workspace=None, sync=True, stream=None):
+        cam = Camera.of(cam)
+        N = splats.shape[0]
+        T = cam.num_tiles
+        if out is None:
+            out = SimpleNamespace(
+                keys_sorted=torch.empty(max(P_capacity, 1), dtype=torch.int64, device=self.device) if want_keys else None,
+                gid_sorted=torch.empty(max(P_capacity, 1), dtype=torch.int32, device=self.device),
+                tile_offsets=torch.empty(T + 1, dtype=torch.int32, device=self.device),
+                P_dev=torch.zeros(2, dtype=torch.int64, device=self.device), P=None)
+        need = self.bin_sort_workspace_bytes(N, P_capacity, T)
+        if workspace is None:
+            workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
+        ph = C.c_int64(-1)
+        rc = self.lib.tgs_bin_sort(self._h, C.byref(cam), N, _p(splats), P_capacity, _p(out.keys_sorted),
+                                   _p(out.gid_sorted), _p(out.tile_offsets), _p(out.P_dev),
+                                   C.byref(ph) if sync else None, _p(workspace), workspace.numel(), _stream(stream))
+        if sync:
+            out.P = ph.value
+        self._check(rc)
+        return out
+
+    # ---- a3 ----
+    def sample_num_tiles(self, cam, num, den):
+        cam = Camera.of(cam)
+        return self.lib.tgs_sample_num_tiles(C.byref(cam), num, den)
+
+    def sample_workspace_bytes(self, cam):
+        cam = Camera.of(cam)
+        b = C.c_size_t()
+        rc = self.lib.tgs_sample_workspace_bytes(C.byref(cam), C.byref(b))
+        if rc != 0:
+            raise TgsError(rc, "tgs_sample_workspace_bytes")
+        return b.value
+
+    def sample(self, cam, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, err=None, render=None, target=None,
+               out=None, workspace=None, sync=True, stream=None):
+        cam = Camera.of(cam)
+        T = cam.num_tiles
+        if out is None:
+            out = SimpleNamespace(tile_score=torch.empty(T, dtype=torch.int64, device=self.device),
+                                  tiles=torch.empty(T, dtype=torch.int32, device=self.device),
+                                  tile_pix_offsets=torch.empty(T + 1, dtype=torch.int32, device=self.device),
+                                  pix=torch.empty(cam.width * cam.height, dtype=torch.int32, device=self.device),
+                                  kn_dev=torch.zeros(2, dtype=torch.int32, device=self.device), k=None, n=None)
+        if workspace is None:
+            workspace = torch.empty(self.sample_workspace_bytes(cam), dtype=torch.uint8, device=self.device)
+        kn = (C.c_int32 * 2)(-1, -1)
+        self._check(self.lib.tgs_sample(self._h, C.byref(cam), _p(err), _p(render), _p(target), int(tile_pct[0]),
+                                        int(tile_pct[1]), int(pixel_mode), int(pix_rate[0]), int(pix_rate[1]),
+                                        C.c_uint64(seed), _p(out.tile_score), _p(out.tiles), _p(out.tile_pix_offsets),
+                                        _p(out.pix), _p(out.kn_dev), kn if sync else None, _p(workspace),
+                                        workspace.numel(), _stream(stream)))
+        out.k = self.sample_num_tiles(cam, tile_pct[0], tile_pct[1])
+        if sync:
+            assert kn[0] == out.k
+            out.n = int(kn[1])
+        return out
+
+    # ---- a4 ----
+    def raster_fwd_sparse(self, cam, splats, binned, samp, n_capacity=None, want_walked=False, out=None, stream=None):
+        cam = Camera.of(cam)
+        n = n_capacity if n_capacity is not None else samp.n
+        if out is None:
+            out = SimpleNamespace(color=torch.empty((n, 3), dtype=torch.float32, device=self.device),
+                                  T=torch.empty(n, dtype=torch.float32, device=self.device),
+                                  n_contrib=torch.empty(n, dtype=torch.int32, device=self.device),
+                                  n_walked=torch.empty(n, dtype=torch.int32, device=self.device) if want_walked else None)
+        self._check(self.lib.tgs_raster_fwd_sparse(self._h, C.byref(cam), splats.shape[0], _p(splats),
+                                                   _p(binned.tile_offsets), _p(binned.gid_sorted), samp.k,
+                                                   _p(samp.tiles), _p(samp.tile_pix_offsets), _p(samp.pix),
+                                                   _p(out.color), _p(out.T), _p(out.n_contrib), _p(out.n_walked),
+                                                   _stream(stream)))
+        return out
+
+    # ---- a5 + a6 ----
+    def raster_bwd_sparse(self, cam, sh_degree, splats, binned, samp, fwd, dL_dcolor, means3D=None, scales=None,
+                          quats=None, sh=None, radii=None, clamped=None, project=True, out=None, stream=None):
+        cam = Camera.of(cam)
+        N = splats.shape[0]
+        if out is None:
+            out = SimpleNamespace(dL_dsplats=torch.empty((N, SPLAT_WORDS), dtype=torch.float32, device=self.device))
+            if project:
+                K = (sh_degree + 1) ** 2
+                out.dL_dmeans3D = torch.empty((N, 3), dtype=torch.float32, device=self.device)
+                out.dL_dscales = torch.empty((N, 3), dtype=torch.float32, device=self.device)
+                out.dL_dquats = torch.empty((N, 4), dtype=torch.float32, device=self.device)
+                out.dL_dopacities = torch.empty(N, dtype=torch.float32, device=self.device)
+                out.dL_dsh = torch.empty((N, K, 3), dtype=torch.float32, device=self.device)
+        g = lambda name: _p(getattr(out, name)) if project else None
+        self._check(self.lib.tgs_raster_bwd_sparse(
+            self._h, C.byref(cam), N, sh_degree, _p(splats), _p(binned.tile_offsets), _p(binned.gid_sorted), samp.k,
+            _p(samp.tiles), _p(samp.tile_pix_offsets), _p(samp.pix), _p(fwd.T), _p(fwd.n_contrib), _p(dL_dcolor),
+            _p(means3D), _p(scales), _p(quats), _p(sh), _p(radii), _p(clamped), _p(out.dL_dsplats),
+            g("dL_dmeans3D"), g("dL_dscales"), g("dL_dquats"), g("dL_dopacities"), g("dL_dsh"), _stream(stream)))
+        return out

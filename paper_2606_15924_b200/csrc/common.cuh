@@ -1,0 +1,84 @@
+// Internal declarations shared by the CUDA translation units of libtgs (never by the oracle).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "../../include/tgs.h"
+
+namespace tgs {
+
+constexpr int kTile = 16;
+constexpr int kTilePixels = 256;
+constexpr int kSplatWords = TGS_SPLAT_WORDS;
+
+// Readings of the paper (R2/R3): constants of the 3DGS kernels TurboGS modifies.
+constexpr float kLowpass = 0.3f;
+constexpr float kJClamp = 1.3f;
+constexpr float kAlphaMin = 0.00392156862745098f;  // 1/255
+constexpr float kAlphaMax = 0.99f;
+constexpr float kTMin = 0.0001f;
+
+struct ctx_impl {
+    int device;
+    int num_sms;
+    char err[512];
+};
+
+// Kernel-side copy of the camera (same fields as tgs_camera; passed by value).
+struct CamK {
+    int W, H, gx, gy;
+    float fx, fy, cx, cy;
+    float R[9];
+    float t[3];
+    float znear;
+    float bg[3];
+};
+
+inline CamK make_camk(const tgs_camera* c) {
+    CamK k;
+    k.W = c->width; k.H = c->height;
+    k.gx = (c->width + kTile - 1) / kTile; k.gy = (c->height + kTile - 1) / kTile;
+    k.fx = c->fx; k.fy = c->fy; k.cx = c->cx; k.cy = c->cy;
+    for (int i = 0; i < 9; ++i) k.R[i] = c->R[i];
+    for (int i = 0; i < 3; ++i) { k.t[i] = c->t[i]; k.bg[i] = c->bg[i]; }
+    k.znear = c->znear;
+    return k;
+}
+
+__device__ __forceinline__ void unpack_rect(uint32_t rx, uint32_t ry, int& x0, int& y0, int& x1, int& y1) {
+    x0 = (int)(rx & 0xffffu); x1 = (int)(rx >> 16);
+    y0 = (int)(ry & 0xffffu); y1 = (int)(ry >> 16);
+}
+
+// ---- launchers (one per translation unit) ---------------------------------------------------
+cudaError_t launch_preprocess(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
+                              const float* op, const float* sh, float* splats, int32_t* radii,
+                              uint8_t* clamped, cudaStream_t s);
+
+size_t binsort_workspace_bytes(int N, int64_t Pcap, int T);
+cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats, int64_t Pcap, uint64_t* keys_sorted,
+                            uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev, void* ws,
+                            size_t ws_bytes, int num_sms, cudaStream_t s);
+
+size_t sample_workspace_bytes(int T);
+cudaError_t launch_sample(const CamK& cam, const float* err, const float* render, const float* target, int k,
+                          int mode, int rnum, int rden, uint64_t seed, uint64_t* tile_score, uint32_t* tiles,
+                          uint32_t* tpo, uint32_t* pix, int32_t* kn_dev, void* ws, cudaStream_t s);
+
+cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
+                              const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                              const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
+                              uint32_t* n_walked, int num_sms, cudaStream_t s);
+
+cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
+                              const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                              const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
+                              const float* dL_dcolor, float* dL_dsplats, int num_sms, cudaStream_t s);
+
+cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
+                               const float* sh, const int32_t* radii, const uint8_t* clamped,
+                               const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
+                               float* dsh, cudaStream_t s);
+
+}  // namespace tgs

@@ -1,0 +1,247 @@
+// tgs_raster_bwd_sparse, projection half: chains dL/d(mean2D, conic, opacity, rgb) of every
+// Gaussian through the EWA projection and the SH colour to dL/d(mean3D, scale, quaternion,
+// opacity, SH) ("This pipeline is differentiable", 441).
+// One thread per Gaussian, no atomics; HBM-bound (reads 236 + 48 B, writes 236 B at degree 3).
+#include "common.cuh"
+
+namespace tgs {
+
+namespace {
+
+constexpr float SH_C0 = 0.28209479177387814f;
+constexpr float SH_C1 = 0.4886025119029199f;
+constexpr float SH_C2A = 1.0925484305920792f;
+constexpr float SH_C2B = 0.31539156525252005f;
+constexpr float SH_C2C = 0.5462742152960396f;
+constexpr float SH_C3A = 0.5900435899266435f;
+constexpr float SH_C3B = 2.890611442640554f;
+constexpr float SH_C3C = 0.4570457994644658f;
+constexpr float SH_C3D = 0.3731763325901154f;
+constexpr float SH_C3E = 1.445305721320277f;
+
+// basis values B[k] and their gradients dB[k][0..2] w.r.t. the direction components
+template <int D>
+__device__ __forceinline__ void sh_basis_and_grad(float x, float y, float z, float* B, float (*dB)[3]) {
+    constexpr int K = (D + 1) * (D + 1);
+#pragma unroll
+    for (int k = 0; k < K; ++k) { dB[k][0] = 0.f; dB[k][1] = 0.f; dB[k][2] = 0.f; }
+    B[0] = SH_C0;
+    if (D >= 1) {
+        B[1] = -SH_C1 * y; dB[1][1] = -SH_C1;
+        B[2] = SH_C1 * z;  dB[2][2] = SH_C1;
+        B[3] = -SH_C1 * x; dB[3][0] = -SH_C1;
+    }
+    if (D >= 2) {
+        const float xx = x * x, yy = y * y, zz = z * z;
+        B[4] = SH_C2A * x * y;  dB[4][0] = SH_C2A * y;  dB[4][1] = SH_C2A * x;
+        B[5] = -SH_C2A * y * z; dB[5][1] = -SH_C2A * z; dB[5][2] = -SH_C2A * y;
+        B[6] = SH_C2B * (2.f * zz - xx - yy);
+        dB[6][0] = -2.f * SH_C2B * x; dB[6][1] = -2.f * SH_C2B * y; dB[6][2] = 4.f * SH_C2B * z;
+        B[7] = -SH_C2A * x * z; dB[7][0] = -SH_C2A * z; dB[7][2] = -SH_C2A * x;
+        B[8] = SH_C2C * (xx - yy); dB[8][0] = 2.f * SH_C2C * x; dB[8][1] = -2.f * SH_C2C * y;
+        if (D >= 3) {
+            B[9] = -SH_C3A * y * (3.f * xx - yy);
+            dB[9][0] = -6.f * SH_C3A * x * y; dB[9][1] = -3.f * SH_C3A * (xx - yy);
+            B[10] = SH_C3B * x * y * z;
+            dB[10][0] = SH_C3B * y * z; dB[10][1] = SH_C3B * x * z; dB[10][2] = SH_C3B * x * y;
+            B[11] = -SH_C3C * y * (4.f * zz - xx - yy);
+            dB[11][0] = 2.f * SH_C3C * x * y; dB[11][1] = -SH_C3C * (4.f * zz - xx - 3.f * yy);
+            dB[11][2] = -8.f * SH_C3C * y * z;
+            B[12] = SH_C3D * z * (2.f * zz - 3.f * xx - 3.f * yy);
+            dB[12][0] = -6.f * SH_C3D * x * z; dB[12][1] = -6.f * SH_C3D * y * z;
+            dB[12][2] = 3.f * SH_C3D * (2.f * zz - xx - yy);
+            B[13] = -SH_C3C * x * (4.f * zz - xx - yy);
+            dB[13][0] = -SH_C3C * (4.f * zz - 3.f * xx - yy); dB[13][1] = 2.f * SH_C3C * x * y;
+            dB[13][2] = -8.f * SH_C3C * x * z;
+            B[14] = SH_C3E * z * (xx - yy);
+            dB[14][0] = 2.f * SH_C3E * x * z; dB[14][1] = -2.f * SH_C3E * y * z; dB[14][2] = SH_C3E * (xx - yy);
+            B[15] = -SH_C3A * x * (xx - 3.f * yy);
+            dB[15][0] = -3.f * SH_C3A * (xx - yy); dB[15][1] = 6.f * SH_C3A * x * y;
+        }
+    }
+}
+
+template <int D>
+__global__ void __launch_bounds__(128)
+project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const float* __restrict__ sc,
+                   const float* __restrict__ qt, const float* __restrict__ sh, const int32_t* __restrict__ radii,
+                   const uint8_t* __restrict__ clamped, const float4* __restrict__ dsp,
+                   float* __restrict__ dmu, float* __restrict__ dsc, float* __restrict__ dqt,
+                   float* __restrict__ dop, float* __restrict__ dsh) {
+    constexpr int K = (D + 1) * (D + 1);
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    float gmu[3] = {0.f, 0.f, 0.f}, gs[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gop = 0.f;
+    float* gsh = dsh + (size_t)i * (K * 3);
+    bool live = radii[i] > 0;
+    const float* W = cam.R;
+    float m0 = 0.f, m1 = 0.f, m2 = 0.f, t0 = 0.f, t1 = 0.f, tz = 1.f;
+    if (live) {
+        m0 = mu[3 * i]; m1 = mu[3 * i + 1]; m2 = mu[3 * i + 2];
+        t0 = W[0] * m0 + W[1] * m1 + W[2] * m2 + cam.t[0];
+        t1 = W[3] * m0 + W[4] * m1 + W[5] * m2 + cam.t[1];
+        tz = W[6] * m0 + W[7] * m1 + W[8] * m2 + cam.t[2];
+        live = tz > cam.znear;
+    }
+    if (!live) {
+#pragma unroll
+        for (int e = 0; e < K * 3; ++e) gsh[e] = 0.f;
+    } else {
+        const float4 d0 = dsp[3 * (size_t)i], d1 = dsp[3 * (size_t)i + 1], d2 = dsp[3 * (size_t)i + 2];
+        const float gmx = d0.x, gmy = d0.y, gA = d0.z, gB = d0.w, gC = d1.x;
+        gop = d1.y;
+        const float grgb[3] = {d1.z, d1.w, d2.x};
+        // ---- forward intermediates ----
+        const float limx = kJClamp * ((0.5f * (float)cam.W) / cam.fx);
+        const float limy = kJClamp * ((0.5f * (float)cam.H) / cam.fy);
+        const float txtz = t0 / tz, tytz = t1 / tz;
+        float cxr = txtz, cyr = tytz;
+        int clx = 0, cly = 0;
+        if (cxr > limx) { cxr = limx; clx = 1; } else if (cxr < -limx) { cxr = -limx; clx = -1; }
+        if (cyr > limy) { cyr = limy; cly = 1; } else if (cyr < -limy) { cyr = -limy; cly = -1; }
+        const float tz2 = tz * tz, itz = 1.0f / tz, itz2 = 1.0f / tz2;
+        const float J00 = cam.fx * itz, J02 = -(cam.fx * cxr * tz) * itz2;
+        const float J11 = cam.fy * itz, J12 = -(cam.fy * cyr * tz) * itz2;
+        float Tm[6];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            Tm[c] = J00 * W[c] + J02 * W[6 + c];
+            Tm[3 + c] = J11 * W[3 + c] + J12 * W[6 + c];
+        }
+        const float4 q = reinterpret_cast<const float4*>(qt)[i];
+        const float w = q.x, x = q.y, y = q.z, z = q.w;
+        float Rq[9];
+        Rq[0] = 1.f - 2.f * (y * y + z * z); Rq[1] = 2.f * (x * y - w * z); Rq[2] = 2.f * (x * z + w * y);
+        Rq[3] = 2.f * (x * y + w * z); Rq[4] = 1.f - 2.f * (x * x + z * z); Rq[5] = 2.f * (y * z - w * x);
+        Rq[6] = 2.f * (x * z - w * y); Rq[7] = 2.f * (y * z + w * x); Rq[8] = 1.f - 2.f * (x * x + y * y);
+        const float s[3] = {sc[3 * i], sc[3 * i + 1], sc[3 * i + 2]};
+        float M[9], Sg[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c) M[3 * r + c] = Rq[3 * r + c] * s[c];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                Sg[3 * r + c] = M[3 * r] * M[3 * c] + M[3 * r + 1] * M[3 * c + 1] + M[3 * r + 2] * M[3 * c + 2];
+        float V[6];
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                V[3 * r + c] = Tm[3 * r] * Sg[c] + Tm[3 * r + 1] * Sg[3 + c] + Tm[3 * r + 2] * Sg[6 + c];
+        const float a = V[0] * Tm[0] + V[1] * Tm[1] + V[2] * Tm[2] + kLowpass;
+        const float b = V[0] * Tm[3] + V[1] * Tm[4] + V[2] * Tm[5];
+        const float c = V[3] * Tm[3] + V[4] * Tm[4] + V[5] * Tm[5] + kLowpass;
+        const float det = a * c - b * b;
+        const float idet = 1.0f / det;
+        const float A = c * idet, B = -b * idet, C = a * idet;
+        // ---- conic -> cov2D: H = -M Ghat M ----
+        const float hB = 0.5f * gB;
+        const float X00 = gA * A + hB * B, X01 = gA * B + hB * C, X10 = hB * A + gC * B, X11 = hB * B + gC * C;
+        const float H00 = -(A * X00 + B * X10), H01 = -(A * X01 + B * X11), H11 = -(B * X01 + C * X11);
+        float HT[6];
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            HT[cc] = H00 * Tm[cc] + H01 * Tm[3 + cc];
+            HT[3 + cc] = H01 * Tm[cc] + H11 * Tm[3 + cc];
+        }
+        float dSg[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) dSg[3 * r + cc] = Tm[r] * HT[cc] + Tm[3 + r] * HT[3 + cc];
+        float dTm[6];
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc)
+                dTm[3 * r + cc] = 2.f * (HT[3 * r] * Sg[cc] + HT[3 * r + 1] * Sg[3 + cc] + HT[3 * r + 2] * Sg[6 + cc]);
+        const float dJ00 = dTm[0] * W[0] + dTm[1] * W[1] + dTm[2] * W[2];
+        const float dJ02 = dTm[0] * W[6] + dTm[1] * W[7] + dTm[2] * W[8];
+        const float dJ11 = dTm[3] * W[3] + dTm[4] * W[4] + dTm[5] * W[5];
+        const float dJ12 = dTm[3] * W[6] + dTm[4] * W[7] + dTm[5] * W[8];
+        float dt0 = 0.f, dt1 = 0.f, dt2 = 0.f;
+        dt2 += -(cam.fx * itz2) * dJ00 - (cam.fy * itz2) * dJ11;
+        if (clx == 0) { dt0 += -(cam.fx * itz2) * dJ02; dt2 += (2.f * cam.fx * t0 * itz2 * itz) * dJ02; }
+        else dt2 += ((float)clx * cam.fx * limx * itz2) * dJ02;
+        if (cly == 0) { dt1 += -(cam.fy * itz2) * dJ12; dt2 += (2.f * cam.fy * t1 * itz2 * itz) * dJ12; }
+        else dt2 += ((float)cly * cam.fy * limy * itz2) * dJ12;
+        dt0 += gmx * cam.fx * itz;
+        dt1 += gmy * cam.fy * itz;
+        dt2 += -gmx * cam.fx * t0 * itz2 - gmy * cam.fy * t1 * itz2;
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) gmu[cc] = W[cc] * dt0 + W[3 + cc] * dt1 + W[6 + cc] * dt2;
+        // ---- Sigma = M M^T ----
+        float dM[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc)
+                dM[3 * r + cc] = 2.f * (dSg[3 * r] * M[cc] + dSg[3 * r + 1] * M[3 + cc] + dSg[3 * r + 2] * M[6 + cc]);
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) gs[cc] = Rq[cc] * dM[cc] + Rq[3 + cc] * dM[3 + cc] + Rq[6 + cc] * dM[6 + cc];
+        float dR[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int cc = 0; cc < 3; ++cc) dR[3 * r + cc] = dM[3 * r + cc] * s[cc];
+        gq[0] = 2.f * (z * (dR[3] - dR[1]) + y * (dR[2] - dR[6]) + x * (dR[7] - dR[5]));
+        gq[1] = 2.f * (y * (dR[1] + dR[3]) + z * (dR[2] + dR[6]) + w * (dR[7] - dR[5])) - 4.f * x * (dR[4] + dR[8]);
+        gq[2] = 2.f * (x * (dR[1] + dR[3]) + w * (dR[2] - dR[6]) + z * (dR[5] + dR[7])) - 4.f * y * (dR[0] + dR[8]);
+        gq[3] = 2.f * (w * (dR[3] - dR[1]) + x * (dR[2] + dR[6]) + y * (dR[5] + dR[7])) - 4.f * z * (dR[0] + dR[4]);
+        // ---- colour ----
+        const float o0 = -(W[0] * cam.t[0] + W[3] * cam.t[1] + W[6] * cam.t[2]);
+        const float o1 = -(W[1] * cam.t[0] + W[4] * cam.t[1] + W[7] * cam.t[2]);
+        const float o2 = -(W[2] * cam.t[0] + W[5] * cam.t[1] + W[8] * cam.t[2]);
+        const float v0 = m0 - o0, v1 = m1 - o1, v2 = m2 - o2;
+        const float len = sqrtf(v0 * v0 + v1 * v1 + v2 * v2), ilen = 1.0f / len;
+        const float d[3] = {v0 * ilen, v1 * ilen, v2 * ilen};
+        float Bk[K], dB[K][3];
+        sh_basis_and_grad<D>(d[0], d[1], d[2], Bk, dB);
+        const uint8_t cl = clamped[i];
+        float gch[3];
+#pragma unroll
+        for (int ch = 0; ch < 3; ++ch) gch[ch] = (cl & (1u << ch)) ? 0.f : grgb[ch];
+        float dd[3] = {0.f, 0.f, 0.f};
+        const float* s_i = sh + (size_t)i * (K * 3);
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                const float sv = __ldg(s_i + 3 * k + ch) * gch[ch];
+                gsh[3 * k + ch] = Bk[k] * gch[ch];
+                dd[0] = fmaf(dB[k][0], sv, dd[0]); dd[1] = fmaf(dB[k][1], sv, dd[1]); dd[2] = fmaf(dB[k][2], sv, dd[2]);
+            }
+        }
+        const float dot = d[0] * dd[0] + d[1] * dd[1] + d[2] * dd[2];
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) gmu[cc] += (dd[cc] - d[cc] * dot) * ilen;
+    }
+    dmu[3 * i] = gmu[0]; dmu[3 * i + 1] = gmu[1]; dmu[3 * i + 2] = gmu[2];
+    dsc[3 * i] = gs[0]; dsc[3 * i + 1] = gs[1]; dsc[3 * i + 2] = gs[2];
+    reinterpret_cast<float4*>(dqt)[i] = make_float4(gq[0], gq[1], gq[2], gq[3]);
+    dop[i] = gop;
+}
+
+}  // namespace
+
+cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
+                               const float* sh, const int32_t* radii, const uint8_t* clamped,
+                               const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
+                               float* dsh, cudaStream_t s) {
+    const int threads = 128, blocks = (N + threads - 1) / threads;
+    const float4* dsp = reinterpret_cast<const float4*>(dL_dsplats);
+#define TGS_PB(DD) project_bwd_kernel<DD><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, sh, radii, clamped, dsp, dmu, dsc, dqt, dop, dsh)
+    switch (D) {
+        case 0: TGS_PB(0); break;
+        case 1: TGS_PB(1); break;
+        case 2: TGS_PB(2); break;
+        default: TGS_PB(3); break;
+    }
+#undef TGS_PB
+    return cudaGetLastError();
+}
+
+}  // namespace tgs

@@ -1,0 +1,224 @@
+// C-ABI entry points of libtgs (include/tgs.h): argument validation, error reporting and launch
+// order.  No arithmetic of the method lives here.
+#include <stdarg.h>
+#include <string.h>
+
+#include <new>
+
+#include "common.cuh"
+
+using namespace tgs;
+
+struct tgs_ctx : public ctx_impl {};
+
+namespace {
+
+int fail(tgs_ctx* ctx, int code, const char* fmt, ...) {
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+int cuda_fail(tgs_ctx* ctx, const char* where, cudaError_t e) {
+    return fail(ctx, TGS_ERR_CUDA, "%s: %s", where, cudaGetErrorString(e));
+}
+
+bool cam_ok(const tgs_camera* c) {
+    return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f;
+}
+
+int num_tiles(const tgs_camera* c) {
+    return ((c->width + kTile - 1) / kTile) * ((c->height + kTile - 1) / kTile);
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* tgs_version(void) { return "tgs 0.1 (sm_100a)"; }
+
+int tgs_create(tgs_ctx** out, int device) {
+    if (!out) return TGS_ERR_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || device < 0 || device >= count) return TGS_ERR_CUDA;  // no GPU, no fallback
+    tgs_ctx* c = new (std::nothrow) tgs_ctx();
+    if (!c) return TGS_ERR_INVALID_ARG;
+    c->device = device;
+    c->err[0] = 0;
+    cudaDeviceProp prop;
+    e = cudaGetDeviceProperties(&prop, device);
+    if (e != cudaSuccess) { delete c; return TGS_ERR_CUDA; }
+    c->num_sms = prop.multiProcessorCount;
+    e = cudaSetDevice(device);
+    if (e != cudaSuccess) { delete c; return TGS_ERR_CUDA; }
+    *out = c;
+    return TGS_OK;
+}
+
+int tgs_destroy(tgs_ctx* ctx) {
+    delete ctx;
+    return TGS_OK;
+}
+
+const char* tgs_last_error(const tgs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+
+int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree, const float* means3D,
+                   const float* scales, const float* quats, const float* opacities, const float* sh,
+                   float* splats, int32_t* radii, uint8_t* clamped, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: bad camera");
+    if (N < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: N < 0");
+    if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_preprocess: sh_degree %d not in 0..3", sh_degree);
+    if (num_tiles(cam) > (1 << 20) || cam->width > 65535 * kTile || cam->height > 65535 * kTile)
+        return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_preprocess: image too large (T > 2^20)");
+    if (N == 0) return TGS_OK;
+    if (!means3D || !scales || !quats || !opacities || !sh || !splats || !radii || !clamped)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: null pointer");
+    if (((uintptr_t)sh & 15) || ((uintptr_t)quats & 15) || ((uintptr_t)splats & 15))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: sh, quats and splats must be 16-byte aligned");
+    cudaError_t e = launch_preprocess(make_camk(cam), N, sh_degree, means3D, scales, quats, opacities, sh, splats,
+                                      radii, clamped, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_preprocess", e);
+    return TGS_OK;
+}
+
+int tgs_bin_sort_workspace_bytes(int N, int64_t P_capacity, int T, size_t* bytes) {
+    if (!bytes || N < 0 || P_capacity < 0 || T <= 0) return TGS_ERR_INVALID_ARG;
+    *bytes = binsort_workspace_bytes(N, P_capacity, T);
+    return TGS_OK;
+}
+
+int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats, int64_t P_capacity,
+                 uint64_t* keys_sorted, uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev,
+                 int64_t* P_host, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: bad camera");
+    if (N < 0 || P_capacity < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: negative size");
+    if (P_capacity >= (int64_t)0xffffffffll) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_bin_sort: P_capacity >= 2^32-1");
+    const int T = num_tiles(cam);
+    if (T > (1 << 20)) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_bin_sort: T > 2^20");
+    if (!gid_sorted || !tile_offsets || !P_dev || !workspace || (N > 0 && !splats))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: null pointer");
+    const size_t need = binsort_workspace_bytes(N, P_capacity, T);
+    if (workspace_bytes < need)
+        return fail(ctx, TGS_ERR_CAPACITY, "tgs_bin_sort: workspace %zu B < required %zu B", workspace_bytes, need);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = launch_bin_sort(make_camk(cam), N, splats, P_capacity, keys_sorted, gid_sorted, tile_offsets,
+                                    P_dev, workspace, workspace_bytes, ctx->num_sms, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_bin_sort", e);
+    if (P_host) {
+        int64_t h[2];
+        e = cudaMemcpyAsync(h, P_dev, sizeof(h), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return cuda_fail(ctx, "tgs_bin_sort (P readback)", e);
+        *P_host = h[0];
+        if (h[1]) return fail(ctx, TGS_ERR_CAPACITY, "tgs_bin_sort: P = %lld exceeds P_capacity = %lld",
+                              (long long)h[0], (long long)P_capacity);
+    }
+    return TGS_OK;
+}
+
+int tgs_sample_num_tiles(const tgs_camera* cam, int num, int den) {
+    if (!cam_ok(cam) || den <= 0 || num < 0) return -1;
+    const int T = num_tiles(cam);
+    int64_t k = ((int64_t)num * T) / den;
+    if (k < 1) k = 1;
+    if (k > T) k = T;
+    return (int)k;
+}
+
+int tgs_sample_workspace_bytes(const tgs_camera* cam, size_t* bytes) {
+    if (!cam_ok(cam) || !bytes) return TGS_ERR_INVALID_ARG;
+    *bytes = sample_workspace_bytes(num_tiles(cam));
+    return TGS_OK;
+}
+
+int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const float* render, const float* target,
+               int tile_pct_num, int tile_pct_den, int pixel_mode, int pix_rate_num, int pix_rate_den,
+               uint64_t seed, uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+               int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: bad camera");
+    if (tile_pct_den <= 0 || tile_pct_num < 0 || tile_pct_num > tile_pct_den)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: tile fraction %d/%d not in [0,1]", tile_pct_num, tile_pct_den);
+    if (pixel_mode != TGS_PIXELS_ALL && pixel_mode != TGS_PIXELS_BERNOULLI_ERR)
+        return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_sample: pixel_mode %d", pixel_mode);
+    if (pixel_mode == TGS_PIXELS_BERNOULLI_ERR &&
+        (pix_rate_den <= 0 || pix_rate_den > 255 || pix_rate_num < 0 || pix_rate_num > 255))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: pixel rate %d/%d outside 0..255", pix_rate_num, pix_rate_den);
+    if (!err && !(render && target)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: need err or render+target");
+    if (!tile_score || !tiles || !tile_pix_offsets || !pix || !kn_dev || !workspace)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: null pointer");
+    const int T = num_tiles(cam);
+    if (T > (1 << 20)) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_sample: T > 2^20");
+    const size_t need = sample_workspace_bytes(T);
+    if (workspace_bytes < need)
+        return fail(ctx, TGS_ERR_CAPACITY, "tgs_sample: workspace %zu B < required %zu B", workspace_bytes, need);
+    const int k = tgs_sample_num_tiles(cam, tile_pct_num, tile_pct_den);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = launch_sample(make_camk(cam), err, render, target, k, pixel_mode, pix_rate_num, pix_rate_den, seed,
+                                  tile_score, tiles, tile_pix_offsets, pix, kn_dev, workspace, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_sample", e);
+    if (kn_host) {
+        e = cudaMemcpyAsync(kn_host, kn_dev, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return cuda_fail(ctx, "tgs_sample (k,n readback)", e);
+    }
+    return TGS_OK;
+}
+
+int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                          const uint32_t* tile_offsets, const uint32_t* gid_sorted, int k, const uint32_t* tiles,
+                          const uint32_t* tile_pix_offsets, const uint32_t* pix, float* out_color, float* out_T,
+                          uint32_t* n_contrib, uint32_t* n_walked, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad camera");
+    if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad N or k");
+    if (k == 0) return TGS_OK;
+    if (!splats || !tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !out_color || !out_T || !n_contrib)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: null pointer");
+    cudaError_t e = launch_raster_fwd(make_camk(cam), splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix,
+                                      out_color, out_T, n_contrib, n_walked, ctx->num_sms, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_fwd_sparse", e);
+    return TGS_OK;
+}
+
+int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree, const float* splats,
+                          const uint32_t* tile_offsets, const uint32_t* gid_sorted, int k, const uint32_t* tiles,
+                          const uint32_t* tile_pix_offsets, const uint32_t* pix, const float* out_T,
+                          const uint32_t* n_contrib, const float* dL_dcolor, const float* means3D,
+                          const float* scales, const float* quats, const float* sh, const int32_t* radii,
+                          const uint8_t* clamped, float* dL_dsplats, float* dL_dmeans3D, float* dL_dscales,
+                          float* dL_dquats, float* dL_dopacities, float* dL_dsh, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: bad camera");
+    if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: bad N or k");
+    if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_raster_bwd_sparse: sh_degree %d", sh_degree);
+    if (N == 0) return TGS_OK;
+    if (!splats || !dL_dsplats) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: null pointer");
+    if (k > 0 && (!tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !out_T || !n_contrib || !dL_dcolor))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: null pointer");
+    cudaStream_t s = (cudaStream_t)stream;
+    const CamK ck = make_camk(cam);
+    cudaError_t e = launch_raster_bwd(ck, N, splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix, out_T,
+                                      n_contrib, dL_dcolor, dL_dsplats, ctx->num_sms, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (raster)", e);
+    if (dL_dmeans3D) {
+        if (!dL_dscales || !dL_dquats || !dL_dopacities || !dL_dsh || !means3D || !scales || !quats || !sh || !radii || !clamped)
+            return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: null pointer (projection half)");
+        if (((uintptr_t)quats & 15) || ((uintptr_t)dL_dquats & 15) || ((uintptr_t)dL_dsplats & 15))
+            return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: quats, dL_dquats, dL_dsplats must be 16-byte aligned");
+        e = launch_project_bwd(ck, N, sh_degree, means3D, scales, quats, sh, radii, clamped, dL_dsplats, dL_dmeans3D,
+                               dL_dscales, dL_dquats, dL_dopacities, dL_dsh, s);
+        if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (projection)", e);
+    }
+    return TGS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,288 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element, on the same seeded inputs.  Run on the B200 box with ``-m gpu``.
+
+Bit exact: splat rect / depth / mean2D words, radii, clamp masks, sort keys, sorted ids, per-tile
+ranges, tile scores, sampled tiles and pixel lists.  Tolerance: forward 1e-5 rel / 1e-6 abs,
+gradients 1e-3 rel / 1e-5 abs (BASELINE.json north_star).
+"""
+import numpy as np
+import pytest
+
+import workloads
+from helpers import (MARGIN, binned_dev, check_forward, check_grad, dev, pack_splats, samp_dev, scene_dev,
+                     tainted_gaussians, u32, unpack_splats)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def tgs(torch):
+    import paper_2606_15924_b200 as pk
+    return pk.TGS(0)
+
+
+def _scenes():
+    return {
+        "cfg1": lambda: workloads.make(1),
+        "small_rot": lambda: workloads.small_random_scene(7, 3000, 200, 136, sh_degree=3, bg=(0.1, 0.3, 0.2), spread=1.3,
+                                                          log_scale=(-2.8, 0.6)),
+        "small_d1": lambda: workloads.small_random_scene(8, 2000, 333, 77, sh_degree=1, spread=1.5, log_scale=(-3.0, 0.8)),
+        "small_d2": lambda: workloads.small_random_scene(9, 1500, 97, 211, sh_degree=2, bg=(1.0, 1.0, 1.0), spread=1.0,
+                                                         log_scale=(-2.5, 0.7)),
+        "cfg2": lambda: workloads.make(2),
+    }
+
+
+_cache = {}
+
+
+def oracle_run(name, orc32):
+    if name not in _cache:
+        sc = _scenes()[name]()
+        g = None
+        r = orc32.pipeline(sc, backward=False)
+        g = workloads.dl_dcolor(SCENES.index(name), r.samp.n)
+        r.rbwd = orc32.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, g)
+        r.pbwd = orc32.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii,
+                                   r.pre.clamped, r.rbwd.dL_dmeans2D, r.rbwd.dL_dconic, r.rbwd.dL_drgb)
+        r.g = g
+        r.sc = sc
+        _cache[name] = r
+    return _cache[name]
+
+
+SCENES = ["cfg1", "small_rot", "small_d1", "small_d2", "cfg2"]
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_preprocess_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    d = scene_dev(sc, torch)
+    out = tgs.preprocess(sc.cam, sc.sh_degree, d.means3D, d.scales, d.quats, d.opacities, d.sh)
+    torch.cuda.synchronize()
+    got = out.splats.cpu().numpy()
+    want = pack_splats(r.pre)
+    gu, wu = got.view(np.uint32), want.view(np.uint32)
+    assert np.array_equal(out.radii.cpu().numpy(), r.pre.radii)
+    assert np.array_equal(out.clamped.cpu().numpy(), r.pre.clamped)
+    for w in (0, 1, 9, 10, 11):  # mean2D, depth, rect: decide integers downstream -> bit exact
+        assert np.array_equal(gu[:, w], wu[:, w]), f"word {w}"
+    for w in (2, 3, 4, 5):       # conic, opacity: canonical arithmetic makes these bit exact too
+        assert np.array_equal(gu[:, w], wu[:, w]), f"word {w}"
+    assert np.abs(got[:, 6:9] - want[:, 6:9]).max() <= 1e-6  # rgb
+    assert (r.pre.radii > 0).sum() > 0.3 * sc.N
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_bin_sort_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    splats = dev(pack_splats(r.pre), torch)  # stage isolated: the oracle's upstream bits
+    P = r.binned.P
+    out = tgs.bin_sort(sc.cam, splats, P + 17, want_keys=True)
+    torch.cuda.synchronize()
+    assert out.P == P
+    assert np.array_equal(u32(out.tile_offsets), r.binned.tile_offsets)
+    assert np.array_equal(u32(out.gid_sorted)[:P], r.binned.gid_sorted)
+    assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:P], r.binned.keys_sorted)
+    # exact capacity works, one less reports TGS_ERR_CAPACITY with the required size
+    out2 = tgs.bin_sort(sc.cam, splats, P)
+    assert out2.P == P and np.array_equal(u32(out2.gid_sorted)[:P], r.binned.gid_sorted)
+    import paper_2606_15924_b200 as pk
+    with pytest.raises(pk.TgsError) as ei:
+        tgs.bin_sort(sc.cam, splats, P - 1)
+    assert ei.value.code == 2 and str(P) in str(ei.value)
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_sample_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    if sc.err is not None:
+        out = tgs.sample(sc.cam, sc.tile_pct, sc.pixel_mode, sc.pix_rate, sc.sample_seed, err=dev(sc.err, torch))
+    else:
+        render = orc32.render_dense(sc.cam, r.binned, r.pre)
+        out = tgs.sample(sc.cam, sc.tile_pct, sc.pixel_mode, sc.pix_rate, sc.sample_seed,
+                         render=dev(render, torch), target=dev(sc.target, torch))
+    torch.cuda.synchronize()
+    s = r.samp
+    assert (out.k, out.n) == (s.k, s.n)
+    assert np.array_equal(out.tile_score.cpu().numpy().view(np.uint64), s.tile_score)
+    assert np.array_equal(u32(out.tiles)[:s.k], s.tiles)
+    assert np.array_equal(u32(out.tile_pix_offsets)[:s.k + 1], s.tile_pix_offsets)
+    assert np.array_equal(u32(out.pix)[:s.n], s.pix)
+
+
+@pytest.mark.parametrize("mode,pct,rate", [(0, (100, 100), (1, 1)), (0, (5, 100), (1, 1)), (1, (100, 100), (1, 2)),
+                                           (1, (40, 100), (1, 7)), (1, (70, 100), (255, 255)), (0, (0, 100), (1, 1))])
+def test_sample_modes(mode, pct, rate, orc32, tgs, torch):
+    rng = np.random.default_rng(5)
+    for (W, H) in [(1297, 840), (33, 17), (16, 16), (1, 1), (250, 3)]:
+        cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+        err = workloads.blob_error_map(rng, W, H, 9)
+        err[rng.integers(0, H), rng.integers(0, W)] = np.nan
+        err[rng.integers(0, H), rng.integers(0, W)] = 1e20
+        if W * H > 1000:
+            err[:32, :48] = 0.0  # zero-error tiles: BERNOULLI keeps exactly one pixel each
+        s = orc32.sample(cam, pct, mode, rate, seed=99, err=err)
+        out = tgs.sample(cam, pct, mode, rate, 99, err=dev(err, torch))
+        assert (out.k, out.n) == (s.k, s.n)
+        assert np.array_equal(out.tile_score.cpu().numpy().view(np.uint64), s.tile_score)
+        assert np.array_equal(u32(out.tiles)[:s.k], s.tiles)
+        assert np.array_equal(u32(out.tile_pix_offsets)[:s.k + 1], s.tile_pix_offsets)
+        assert np.array_equal(u32(out.pix)[:s.n], s.pix)
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_raster_fwd_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    splats = dev(pack_splats(r.pre), torch)
+    b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
+    out = tgs.raster_fwd_sparse(sc.cam, splats, b, s, want_walked=True)
+    torch.cuda.synchronize()
+    rep = check_forward(out.color.cpu().numpy(), out.T.cpu().numpy(), u32(out.n_contrib), r.fwd)
+    ok = r.fwd.margin[:, 0] > MARGIN
+    assert np.array_equal(u32(out.n_walked)[ok], r.fwd.n_walked[ok])
+    print(name, rep)
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_raster_bwd_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    splats = dev(pack_splats(r.pre), torch)
+    b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
+    fwd = type("F", (), {})()
+    fwd.T = dev(r.fwd.T, torch)
+    fwd.n_contrib = dev(r.fwd.n_contrib.astype(np.int64), torch, torch.int32)
+    d = scene_dev(sc, torch)
+    out = tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, b, s, fwd, dev(r.g, torch), d.means3D, d.scales, d.quats,
+                                d.sh, dev(r.pre.radii, torch), dev(r.pre.clamped, torch))
+    torch.cuda.synchronize()
+    good = ~tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+    assert good.mean() > 0.9
+    ds = out.dL_dsplats.cpu().numpy()
+    worst = {}
+    worst["mean2D"] = check_grad("dL_dmean2D", ds[:, 0:2], r.rbwd.dL_dmeans2D, good)
+    worst["conic"] = check_grad("dL_dconic", ds[:, 2:5], r.rbwd.dL_dconic, good)
+    worst["opacity"] = check_grad("dL_dopacity", ds[:, 5], r.rbwd.dL_dopacity, good)
+    worst["rgb"] = check_grad("dL_drgb", ds[:, 6:9], r.rbwd.dL_drgb, good)
+    assert not ds[:, 9:].any()
+    worst["means3D"] = check_grad("dL_dmeans3D", out.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
+    worst["scales"] = check_grad("dL_dscales", out.dL_dscales.cpu().numpy(), r.pbwd.dL_dscales, good)
+    worst["quats"] = check_grad("dL_dquats", out.dL_dquats.cpu().numpy(), r.pbwd.dL_dquats, good)
+    worst["sh"] = check_grad("dL_dsh", out.dL_dsh.cpu().numpy(), r.pbwd.dL_dsh, good)
+    worst["opac"] = check_grad("dL_dopacities", out.dL_dopacities.cpu().numpy(), r.rbwd.dL_dopacity, good)
+    assert np.abs(r.pbwd.dL_dmeans3D).max() > 1e-3  # a real gradient, not zeros against zeros
+    print(name, {k: round(v, 3) for k, v in worst.items()})
+
+
+@pytest.mark.parametrize("name", SCENES)
+def test_end_to_end_all_gpu(name, orc32, tgs, torch):
+    """preprocess -> bin_sort -> sample -> fwd -> bwd entirely on the GPU, no oracle data in between."""
+    import paper_2606_15924_b200 as pk
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    d = scene_dev(sc, torch)
+    step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 1000, want_walked=True)
+    kw = dict(err=dev(sc.err, torch)) if sc.err is not None else None
+    if kw is None:
+        # config 1: the mask comes from a dense render (full mask) and its residual to the target
+        step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, (100, 100), 0,
+                     err=torch.ones((sc.cam.height, sc.cam.width), device="cuda"))
+        P, k, n = step.counts()
+        img = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
+        img[step.samp.pix[:n].long()] = step.fwd.color[:n]
+        kw = dict(render=img.reshape(sc.cam.height, sc.cam.width, 3).contiguous(), target=dev(sc.target, torch))
+    step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
+                 sc.sample_seed, **kw)
+    P, k, n = step.counts()
+    assert (P, k) == (r.binned.P, r.samp.k)
+    if sc.err is not None:
+        assert n == r.samp.n and np.array_equal(u32(step.samp.pix)[:n], r.samp.pix)
+        rep = check_forward(step.fwd.color[:n].cpu().numpy(), step.fwd.T[:n].cpu().numpy(),
+                            u32(step.fwd.n_contrib)[:n], r.fwd)
+        g = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
+        g[:n] = dev(r.g, torch)
+        bw = step.backward(g)
+        torch.cuda.synchronize()
+        good = ~tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+        check_grad("dL_dmeans3D", bw.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
+        check_grad("dL_dscales", bw.dL_dscales.cpu().numpy(), r.pbwd.dL_dscales, good)
+        check_grad("dL_dquats", bw.dL_dquats.cpu().numpy(), r.pbwd.dL_dquats, good)
+        check_grad("dL_dsh", bw.dL_dsh.cpu().numpy(), r.pbwd.dL_dsh, good)
+        check_grad("dL_dopacities", bw.dL_dopacities.cpu().numpy(), r.rbwd.dL_dopacity, good)
+
+
+def test_full_mask_equals_dense_and_empty_gradients(orc32, tgs, torch):
+    """north_star: a full mask reproduces dense rendering; zero upstream gradient gives zero gradients."""
+    sc = workloads.small_random_scene(21, 4000, 250, 130, sh_degree=3, bg=(0.2, 0.1, 0.4), spread=1.4)
+    pre = orc32.preprocess(sc.cam, 3, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+    b = orc32.bin_sort(sc.cam, pre)
+    dense = orc32.render_dense(sc.cam, b, pre).reshape(-1, 3)
+    full = orc32.sample(sc.cam, (100, 100), 0, err=np.ones((130, 250), np.float32))
+    of = orc32.raster_fwd(sc.cam, b, pre, full)
+    splats = dev(pack_splats(pre), torch)
+    out = tgs.raster_fwd_sparse(sc.cam, splats, binned_dev(b, torch, sc.cam.num_tiles), samp_dev(full, torch))
+    img = np.zeros_like(dense); img[full.pix] = out.color.cpu().numpy()
+    ok = np.zeros(len(dense), bool); ok[full.pix] = of.margin[:, 0] > MARGIN
+    assert np.abs(img - dense)[ok].max() <= 1e-6 + 1e-5 * np.abs(dense).max()
+    fwd = type("F", (), {})(); fwd.T = out.T; fwd.n_contrib = out.n_contrib
+    d = scene_dev(sc, torch)
+    bw = tgs.raster_bwd_sparse(sc.cam, 3, splats, binned_dev(b, torch, sc.cam.num_tiles), samp_dev(full, torch), fwd,
+                               torch.zeros((full.n, 3), device="cuda"), d.means3D, d.scales, d.quats, d.sh,
+                               dev(pre.radii, torch), dev(pre.clamped, torch))
+    for a in (bw.dL_dsplats, bw.dL_dmeans3D, bw.dL_dscales, bw.dL_dquats, bw.dL_dopacities, bw.dL_dsh):
+        assert not a.any().item()
+
+
+def test_degenerate_inputs(orc32, tgs, torch):
+    import paper_2606_15924_b200 as pk
+    cam = workloads.Camera(64, 48, 64.0, 64.0, 32.0, 24.0, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    # every Gaussian culled (behind the camera): P = 0, all ranges empty, forward = background
+    N = 100
+    rng = np.random.default_rng(0)
+    mu = rng.uniform(-1, 1, (N, 3)).astype(np.float32); mu[:, 2] -= 5
+    sc = np.full((N, 3), 0.1, np.float32); q = np.tile(np.array([1, 0, 0, 0], np.float32), (N, 1))
+    op = np.full(N, 0.5, np.float32); sh = np.zeros((N, 1, 3), np.float32)
+    cam.bg = (0.25, 0.5, 0.75)
+    step = pk.SparseRasterStep(tgs, cam, N, 0, 64)
+    err = torch.ones((48, 64), device="cuda")
+    fw = step.forward(dev(mu, torch), dev(sc, torch), dev(q, torch), dev(op, torch), dev(sh, torch), (100, 100), 0, err=err)
+    P, k, n = step.counts()
+    assert (P, k, n) == (0, 12, 64 * 48)
+    assert not step.pre.splats.any().item() and not step.binned.tile_offsets.any().item()
+    assert torch.equal(fw.color[:n], torch.tensor([0.25, 0.5, 0.75], device="cuda").expand(n, 3))
+    assert (fw.T[:n] == 1).all().item() and not fw.n_contrib[:n].any().item()
+    bw = step.backward(torch.ones((64 * 48, 3), device="cuda"))
+    assert not bw.dL_dmeans3D.any().item() and not bw.dL_dsh.any().item()
+    # unsupported / invalid arguments fail loudly
+    with pytest.raises(pk.TgsError) as ei:
+        tgs.preprocess(cam, 4, dev(mu, torch), dev(sc, torch), dev(q, torch), dev(op, torch), dev(sh, torch))
+    assert ei.value.code == 4
+    with pytest.raises(pk.TgsError):
+        tgs.sample(cam, (3, 2), 0, err=err)
+    with pytest.raises(pk.TgsError):
+        tgs.sample(cam, (1, 2), 0)
+
+
+def test_sort_stability_with_duplicate_depths(orc32, tgs, torch):
+    """Equal depths inside a tile must keep ascending Gaussian id (reading 6)."""
+    sc = workloads.small_random_scene(33, 5000, 160, 96, sh_degree=0, spread=1.2, log_scale=(-2.4, 0.5))
+    pre = orc32.preprocess(sc.cam, 0, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+    vis = np.nonzero(pre.radii > 0)[0]
+    pre.depths[vis] = np.float32(3.0) + (vis % 5).astype(np.float32)  # only 5 distinct depths
+    b = orc32.bin_sort(sc.cam, pre)
+    out = tgs.bin_sort(sc.cam, dev(pack_splats(pre), torch), b.P, want_keys=True)
+    assert np.array_equal(u32(out.gid_sorted)[:b.P], b.gid_sorted)
+    assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:b.P], b.keys_sorted)
+    assert np.array_equal(u32(out.tile_offsets), b.tile_offsets)
