@@ -1,0 +1,376 @@
+#!/usr/bin/env python
+"""bench.py -- one TurboGS sparse-raster step (all five C-ABI calls) on seeded synthetic scenes.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--pct P] [--impl tgs|reference]
+
+A "step" is one pass of the whole hot path over one view: tgs_preprocess -> tgs_bin_sort ->
+tgs_sample -> tgs_raster_fwd_sparse -> tgs_raster_bwd_sparse (raster + projection halves).
+Default workload = BASELINE.json configs[1] (100k Gaussians, 980x545, top 30% tiles).
+Prints ONE JSON line (rank 0).  Multi-GPU = independent replicas, one view per rank, no data-path
+collective (replicas only); the barrier / max-over-ranks timing uses NCCL.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "sampled px/s fwd+bwd raster and Gaussian-px evals/s; % of HBM/FP32 roofline"
+UNIT = "sampled_px/s"
+
+# Algorithmic FP32 flops per Gaussian-pixel evaluation, counted from the oracle's arithmetic
+# (DESIGN.md "Roofline accounting"): every visited (pixel, Gaussian) costs the power / exp / alpha
+# test; a composited one additionally the blend (forward) or the nine partial derivatives (backward).
+FWD_FLOPS_WALK, FWD_FLOPS_BLEND = 15, 10
+BWD_FLOPS_WALK, BWD_FLOPS_BLEND = 15, 64
+SM_COUNT, FP32_LANES, SM_MAX_GHZ = 148, 128, 1.965
+FP32_PEAK_TFLOPS = SM_COUNT * FP32_LANES * 2 * SM_MAX_GHZ / 1e3  # 74.4: FMA = 2 flop, nominal max clock
+
+
+def load_scene(cfg: int, pct: int):
+    import workloads
+    return workloads.make(cfg, pct=pct) if cfg == 5 else workloads.make(cfg)
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0}, "fallback"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.005):
+        super().__init__(daemon=True)
+        self.index, self.period, self.samples, self.reasons = index, period_s, [], set()
+        self.stop_flag = threading.Event()
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        while not self.stop_flag.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# --------------------------------------------------------------------------------------------
+def time_oracle(scene, steps, warmup):
+    """The CPU oracle as it stands, single thread: one full step per iteration."""
+    import oracle
+    import workloads
+    o = oracle.Oracle("f32")
+    times, n = [], None
+    g = None
+    for i in range(warmup + steps):
+        t0 = time.perf_counter()
+        r = o.pipeline(scene, dL_dcolor=g, backward=g is not None)
+        if g is None:  # first pass only sizes the upstream gradient (outside the timing)
+            g = workloads.dl_dcolor(0, r.samp.n)
+            t0 = time.perf_counter()
+            r = o.pipeline(scene, dL_dcolor=g, backward=True)
+        dt = time.perf_counter() - t0
+        n = r.samp.n
+        if i >= warmup:
+            times.append(dt)
+    return n, times, r
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores (this tier's reference arm)."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene = load_scene(args.config, args.pct)
+    n, times, r = time_oracle(scene, args.steps, args.warmup)
+    total = sum(times)
+    val = n * len(times) / total
+    cfg = workload_config(scene, args, r.binned.P, r.samp.k, n)
+    cfg["l2"] = "n/a (CPU)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": cfg,
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": f"{len(times)} full steps of the workload, single thread"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_config(scene, args, P, k, n):
+    return {"workload": f"BASELINE.json configs[{args.config - 1}] ({scene.name})", "gaussians": scene.N,
+            "sh_degree": scene.sh_degree, "image": [scene.cam.width, scene.cam.height],
+            "tiles": scene.cam.num_tiles, "tile_pct": list(scene.tile_pct),
+            "pixel_mode": "all" if scene.pixel_mode == 0 else "bernoulli_err", "pairs_P": int(P),
+            "sampled_tiles_k": int(k), "sampled_pixels_n": int(n), "parallelism": f"replicas x{args.gpus}"}
+
+
+def run_tgs(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2606_15924_b200 as pk
+    import workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    scene = load_scene(args.config, args.pct)
+    cam = scene.cam
+    tg = pk.TGS(local)
+    H = {k: torch.from_numpy(np.ascontiguousarray(getattr(scene, k))).pin_memory()
+         for k in ("means3D", "scales", "quats", "opacities", "sh")}
+    if scene.err is None:  # config 1: mask from the residual of a dense render; use a fixed seeded error map instead
+        err_np = workloads.blob_error_map(np.random.default_rng(0), cam.width, cam.height, 8)
+    else:
+        err_np = scene.err
+    H["err"] = torch.from_numpy(np.ascontiguousarray(err_np)).pin_memory()
+    D = {k: v.to(dev) for k, v in H.items()}
+
+    # size the pair buffers: one preprocess, then P = sum of tiles touched (plumbing, untimed)
+    pre = tg.preprocess(cam, scene.sh_degree, D["means3D"], D["scales"], D["quats"], D["opacities"], D["sh"])
+    rw = pre.splats[:, 10:12].contiguous().view(torch.int32)
+    P_est = int((((rw[:, 0] >> 16) - (rw[:, 0] & 0xffff)).long() * ((rw[:, 1] >> 16) - (rw[:, 1] & 0xffff)).long()).sum())
+    del pre, rw
+    step = pk.SparseRasterStep(tg, cam, scene.N, scene.sh_degree, P_est + 1024, want_walked=True)
+
+    def fwd():
+        step.forward(D["means3D"], D["scales"], D["quats"], D["opacities"], D["sh"], scene.tile_pct, scene.pixel_mode,
+                     scene.pix_rate, scene.sample_seed, err=D["err"])
+
+    fwd()
+    P, k, n = step.counts()
+    walked = int(step.fwd.n_walked[:n].long().sum())
+    blended = int(step.fwd.n_blended[:n].long().sum())
+    replayed = int(step.fwd.n_contrib[:n].long().sum())
+    g_host = torch.from_numpy(workloads.dl_dcolor(0, n) / np.float32(n)).pin_memory()
+    g_dev = torch.zeros((cam.width * cam.height, 3), device=dev)
+    g_dev[:n] = g_host.to(dev)
+    step.fwd.n_walked = None   # work counters are not part of the timed step
+    step.fwd.n_blended = None
+
+    def full_step():
+        fwd()
+        step.backward(g_dev)
+
+    flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 256 MiB > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        full_step()
+    barrier()
+
+    # ---- timed region: K steps, each bracketed by CUDA events, L2 flushed between steps ----
+    sampler = ClockSampler(local)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    l0 = tg.launch_count()
+    barrier()
+    for s, e in ev:
+        flush.fill_(1.0)
+        s.record()
+        full_step()
+        e.record()
+    barrier()
+    launches = tg.launch_count() - l0
+    sampler.stop_flag.set()
+    sampler.join()
+    step_ms = [s.elapsed_time(e) for s, e in ev]
+    total_ms = sum(step_ms)
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        nt = torch.tensor([n], device=dev, dtype=torch.float64)
+        dist.all_reduce(nt, op=dist.ReduceOp.SUM)
+        n_total = float(nt.item())
+    else:
+        n_total = float(n)
+    value = n_total * args.steps / (total_ms * 1e-3)
+
+    # ---- per-call breakdown (separate pass; events between the calls) ----
+    names = ["preprocess", "bin_sort", "sample", "raster_fwd", "raster_bwd", "project_bwd"]
+    acc = {k_: 0.0 for k_ in names}
+    tgs_, st = tg, step
+    for _ in range(args.steps):
+        flush.fill_(1.0)
+        e_ = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+        e_[0].record()
+        tgs_.preprocess(cam, scene.sh_degree, D["means3D"], D["scales"], D["quats"], D["opacities"], D["sh"], out=st.pre)
+        e_[1].record()
+        tgs_.bin_sort(cam, st.pre.splats, st.P_capacity, out=st.binned, workspace=st.ws_sort, sync=False)
+        e_[2].record()
+        tgs_.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed, err=D["err"], out=st.samp,
+                    workspace=st.ws_sample, sync=False)
+        e_[3].record()
+        tgs_.raster_fwd_sparse(cam, st.pre.splats, st.binned, st.samp, out=st.fwd)
+        e_[4].record()
+        tgs_.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, st.binned, st.samp, st.fwd, g_dev, project=False,
+                               out=st.bwd)
+        e_[5].record()
+        tgs_.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, st.binned, st.samp, st.fwd, g_dev, D["means3D"],
+                               D["scales"], D["quats"], D["sh"], st.pre.radii, st.pre.clamped, project=True, out=st.bwd)
+        e_[6].record()
+        torch.cuda.synchronize()
+        d = [e_[i].elapsed_time(e_[i + 1]) for i in range(6)]
+        for nm, v in zip(names[:5], d[:5]):
+            acc[nm] += v
+        acc["project_bwd"] += max(d[5] - d[4], 0.0)  # second call = raster + projection
+    per_call_ms = {k_: v / args.steps for k_, v in acc.items()}
+
+    # ---- roofline of the dominant kernel ----
+    peaks, peak_src = measured_peaks()
+    fwd_flops = FWD_FLOPS_WALK * walked + FWD_FLOPS_BLEND * blended
+    bwd_flops = BWD_FLOPS_WALK * replayed + BWD_FLOPS_BLEND * blended
+    K = (scene.sh_degree + 1) ** 2
+    hbm_bytes = {"preprocess": scene.N * (4 * (11 + 3 * K) + 48 + 5), "project_bwd": scene.N * (4 * (10 + 3 * K) + 48 + 5 + 4 * (11 + 3 * K)),
+                 "bin_sort": scene.N * (12 + 4 * 16 + 8 + 8 + 16) + P * (8 + 2 * 16 + 8)}
+    kernels = {
+        "raster_fwd": {"bound": "alu", "achieved": fwd_flops / (per_call_ms["raster_fwd"] * 1e-3) / 1e12,
+                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"},
+        "raster_bwd": {"bound": "alu", "achieved": bwd_flops / (per_call_ms["raster_bwd"] * 1e-3) / 1e12,
+                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"},
+    }
+    for nm in ("preprocess", "project_bwd", "bin_sort"):
+        kernels[nm] = {"bound": "hbm", "achieved": hbm_bytes[nm] / (per_call_ms[nm] * 1e-3) / 1e9,
+                       "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    for v in kernels.values():
+        v["frac"] = v["achieved"] / v["peak"]
+    dominant = max(("raster_fwd", "raster_bwd", "preprocess", "project_bwd", "bin_sort"), key=lambda k_: per_call_ms[k_])
+    roof = dict(kernels[dominant])
+    roof.update({"kernel": dominant, "traffic": None, "ms": per_call_ms[dominant],
+                 "peak_source": ("nominal fp32: 148 SM x 128 lanes x 2 flop x 1.965 GHz" if roof["bound"] == "alu"
+                                 else f"MEASURED_PEAKS.json hbm_gbs ({peak_src})")})
+
+    # ---- end to end: host buffers in, host gradients out, copies inside the timed region ----
+    Hout = {k_: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k_, v in
+            (("dL_dmeans3D", step.bwd.dL_dmeans3D), ("dL_dscales", step.bwd.dL_dscales), ("dL_dquats", step.bwd.dL_dquats),
+             ("dL_dopacities", step.bwd.dL_dopacities), ("dL_dsh", step.bwd.dL_dsh))}
+    g_pin = torch.zeros((cam.width * cam.height, 3)).pin_memory()
+    g_pin[:n] = g_host
+    h2d = sum(v.numel() * v.element_size() for v in H.values()) + n * 12
+    d2h = sum(v.numel() * v.element_size() for v in Hout.values())
+
+    def e2e_step():
+        for k_, v in H.items():
+            D[k_].copy_(v, non_blocking=True)
+        g_dev[:n].copy_(g_pin[:n], non_blocking=True)
+        full_step()
+        for k_, v in Hout.items():
+            v.copy_(getattr(step.bwd, k_), non_blocking=True)
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    es, ee = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    es.record()
+    for _ in range(args.steps):
+        e2e_step()
+    ee.record()
+    barrier()
+    e2e_ms = es.elapsed_time(ee)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    e2e_val = n_total * args.steps / (e2e_ms * 1e-3)
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": dict(workload_config(scene, args, P, k, n), l2="flushed between steps (256 MiB write)"),
+            "clocks": sampler.summary(),
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": e2e_ms / args.steps},
+            "gpu_launches": int(launches),
+            "roofline": roof,
+            "per_call_ms": per_call_ms,
+            "kernels": kernels,
+            "work": {"fwd_evals": walked, "bwd_evals": replayed, "blended": blended,
+                     "fwd_evals_per_s": walked / (per_call_ms["raster_fwd"] * 1e-3),
+                     "bwd_evals_per_s": replayed / (per_call_ms["raster_bwd"] * 1e-3),
+                     "raster_px_per_s": n / ((per_call_ms["raster_fwd"] + per_call_ms["raster_bwd"]) * 1e-3)}}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        reps = 3 if scene.N <= 200_000 else 1
+        n_o, times, _ = time_oracle(scene, reps, 0)
+        line["cpu_baseline"] = {"value": n_o * len(times) / sum(times), "unit": UNIT, "cores": 1, "kind": "oracle",
+                                "sample": f"{len(times)} full step(s) of the same workload, single thread, "
+                                          f"{sum(times):.1f} s", "host_cores_available": os.cpu_count()}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=2, help="1..5, 1-based index into BASELINE.json configs")
+    ap.add_argument("--pct", type=int, default=20, help="tile percentage for config 5")
+    ap.add_argument("--impl", default="tgs", choices=["tgs", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.config > 2:  # bigger configs: keep the whole run within a few minutes
+            args.steps, args.warmup = min(args.steps, 2), min(args.warmup, 1)
+        run_reference(args)
+    else:
+        run_tgs(args)
+
+
+if __name__ == "__main__":
+    main()

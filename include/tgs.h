@@ -72,6 +72,9 @@ int tgs_create(tgs_ctx** ctx, int device);
 int tgs_destroy(tgs_ctx* ctx);
 const char* tgs_last_error(const tgs_ctx* ctx);
 const char* tgs_version(void);
+/* Number of CUDA kernels this library has launched in this process (all contexts); bench.py
+ * reports the difference over its timed region as gpu_launches. */
+uint64_t tgs_launch_count(void);
 
 /* ---- a1: projection -------------------------------------------------------
  * in : means3D[N,3] scales[N,3] quats[N,4] opacities[N] sh[N,K,3], K=(sh_degree+1)^2 (coefficient
@@ -124,14 +127,15 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam,
  *   alpha = min(0.99, o * exp(-1/2 d^T conic d)), skipped if alpha < 1/255, stop before the
  *   Gaussian that would take T below 1e-4;  color = sum c alpha T + T_final * bg.
  * out_color[n,3], out_T[n] (T_final), n_contrib[n] (1-based position in the tile range of the last
- * Gaussian composited, 0 = none), n_walked[n] (optional, NULL ok: range entries visited).
+ * Gaussian composited, 0 = none); optional work counters (NULL ok): n_walked[n] = range entries
+ * visited, n_blended[n] = Gaussians actually composited (alpha >= 1/255 and not terminated).
  * k is the host-known tile count (tgs_sample_num_tiles); n is read from tile_pix_offsets[k]. */
 int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
                           const uint32_t* tile_offsets, const uint32_t* gid_sorted,
                           int k, const uint32_t* tiles, const uint32_t* tile_pix_offsets,
                           const uint32_t* pix,
                           float* out_color, float* out_T, uint32_t* n_contrib, uint32_t* n_walked,
-                          void* stream);
+                          uint32_t* n_blended, void* stream);
 
 /* ---- a5 + a6: sparse backward ----------------------------------
  * Raster half: back-to-front replay from n_contrib, accumulating into dL_dsplats[N,12] (zeroed

@@ -23,7 +23,7 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
              4: "TGS_ERR_UNSUPPORTED"}
 
 # every symbol include/tgs.h declares (tests check the library exports them all)
-SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_preprocess",
+SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
            "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse"]
 
@@ -76,6 +76,7 @@ def load_library() -> C.CDLL:
     lib.tgs_last_error.argtypes = [vp]
     lib.tgs_last_error.restype = C.c_char_p
     lib.tgs_version.restype = C.c_char_p
+    lib.tgs_launch_count.restype = C.c_uint64
     cam = C.POINTER(Camera)
     lib.tgs_preprocess.argtypes = [vp, cam, i32, i32] + [vp] * 5 + [vp] * 3 + [vp]
     lib.tgs_bin_sort_workspace_bytes.argtypes = [i32, i64, i32, C.POINTER(C.c_size_t)]
@@ -84,7 +85,7 @@ def load_library() -> C.CDLL:
     lib.tgs_sample_workspace_bytes.argtypes = [cam, C.POINTER(C.c_size_t)]
     lib.tgs_sample.argtypes = [vp, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp,
                                C.POINTER(C.c_int32), vp, C.c_size_t, vp]
-    lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp]
+    lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
                                          [vp] + [vp] * 5 + [vp]
     return lib
@@ -123,6 +124,9 @@ class TGS:
         if h:
             self.lib.tgs_destroy(h)
             self._h = None
+
+    def launch_count(self) -> int:
+        return int(self.lib.tgs_launch_count())
 
     def _check(self, rc):
         if rc != 0:
@@ -216,12 +220,13 @@ class TGS:
             out = SimpleNamespace(color=torch.empty((n, 3), dtype=torch.float32, device=self.device),
                                   T=torch.empty(n, dtype=torch.float32, device=self.device),
                                   n_contrib=torch.empty(n, dtype=torch.int32, device=self.device),
-                                  n_walked=torch.empty(n, dtype=torch.int32, device=self.device) if want_walked else None)
+                                  n_walked=torch.empty(n, dtype=torch.int32, device=self.device) if want_walked else None,
+                                  n_blended=torch.empty(n, dtype=torch.int32, device=self.device) if want_walked else None)
         self._check(self.lib.tgs_raster_fwd_sparse(self._h, C.byref(cam), splats.shape[0], _p(splats),
                                                    _p(binned.tile_offsets), _p(binned.gid_sorted), samp.k,
                                                    _p(samp.tiles), _p(samp.tile_pix_offsets), _p(samp.pix),
                                                    _p(out.color), _p(out.T), _p(out.n_contrib), _p(out.n_walked),
-                                                   _stream(stream)))
+                                                   _p(getattr(out, "n_blended", None)), _stream(stream)))
         return out
 
     # ---- a5 + a6 ----

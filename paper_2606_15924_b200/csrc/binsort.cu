@@ -307,6 +307,7 @@ void radix_pass(const uint32_t* kin, const uint32_t* vin, uint32_t* kout, uint32
     radix_scan_kernel<<<256, kScanThreads, 0, s>>>(w.hist, nb, n_dev, n_host_or_cap, w.dtot);
     radix_scatter_kernel<<<nb, kRadixThreads, 0, s>>>(kin, vin, kout, vout, n_dev, n_host_or_cap, shift, mask,
                                                       w.hist, w.dtot);
+    count_launches(3);
 }
 
 }  // namespace
@@ -357,6 +358,7 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, int64
     const int rb = num_sms * 8;
     ranges_kernel<<<rb, 256, 0, s>>>(w.tkA, P_dev, T, tile_offsets);
     if (keys_sorted) keys64_kernel<<<rb, 256, 0, s>>>(w.tkA, gid_sorted, splats, P_dev, keys_sorted);
+    count_launches(6 + (keys_sorted ? 1 : 0));  // depth_keys, counts, bsum_scan, offsets, duplicate, ranges
     return cudaGetLastError();
 }
 

@@ -51,6 +51,9 @@ __device__ __forceinline__ void unpack_rect(uint32_t rx, uint32_t ry, int& x0, i
     y0 = (int)(ry & 0xffffu); y1 = (int)(ry >> 16);
 }
 
+// Every kernel launch of the library is counted (tgs_launch_count).
+void count_launches(int n);
+
 // ---- launchers (one per translation unit) ---------------------------------------------------
 cudaError_t launch_preprocess(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                               const float* op, const float* sh, float* splats, int32_t* radii,
@@ -69,7 +72,7 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, int num_sms, cudaStream_t s);
+                              uint32_t* n_walked, uint32_t* n_blended, int num_sms, cudaStream_t s);
 
 cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,

@@ -205,6 +205,7 @@ cudaError_t launch_preprocess(const CamK& cam, int N, int D, const float* mu, co
         case 2: preprocess_kernel<2><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, op, sh, sp, radii, clamped); break;
         default: preprocess_kernel<3><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, op, sh, sp, radii, clamped); break;
     }
+    count_launches(1);
     return cudaGetLastError();
 }
 

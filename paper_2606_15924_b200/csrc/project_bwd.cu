@@ -241,6 +241,7 @@ cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, c
         default: TGS_PB(3); break;
     }
 #undef TGS_PB
+    count_launches(1);
     return cudaGetLastError();
 }
 

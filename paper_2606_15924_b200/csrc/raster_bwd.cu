@@ -134,6 +134,7 @@ cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const
     raster_bwd_kernel<<<k, kBwdThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                 gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
                                                 dL_dsplats);
+    count_launches(1);
     return cudaGetLastError();
 }
 

@@ -20,7 +20,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
                   float* __restrict__ out_color, float* __restrict__ out_T, uint32_t* __restrict__ n_contrib,
-                  uint32_t* __restrict__ n_walked) {
+                  uint32_t* __restrict__ n_walked, uint32_t* __restrict__ n_blended) {
     __shared__ float4 s_a[kBatch];  // mx, my, -A/2, -B
     __shared__ float4 s_b[kBatch];  // -C/2, opacity, r, g
     __shared__ float s_c[kBatch];   // b
@@ -37,7 +37,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
             py = (float)(id / (uint32_t)cam.W);
         }
         float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-        uint32_t last = 0, walked = 0;
+        uint32_t last = 0, walked = 0, blended = 0;
         bool done = !active;
 
         for (uint32_t b0 = start; b0 < end; b0 += kBatch) {
@@ -69,6 +69,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
                     const float w = alpha * T;
                     C0 = fmaf(bb.z, w, C0); C1 = fmaf(bb.w, w, C1); C2 = fmaf(s_c[jj], w, C2);
                     T = Tn;
+                    ++blended;
                     last = (b0 - start) + jj + 1;
                 }
             }
@@ -81,6 +82,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
             out_T[o] = T;
             n_contrib[o] = last;
             if (n_walked) n_walked[o] = walked;
+            if (n_blended) n_blended[o] = blended;
         }
         __syncthreads();  // shared batch buffers are reused by the next tile
     }
@@ -91,12 +93,13 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, int num_sms, cudaStream_t s) {
+                              uint32_t* n_walked, uint32_t* n_blended, int num_sms, cudaStream_t s) {
     (void)num_sms;
     if (k <= 0) return cudaSuccess;
     raster_fwd_kernel<<<k, kFwdThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                 gid_sorted, k, tiles, tpo, pix, out_color, out_T, n_contrib,
-                                                n_walked);
+                                                n_walked, n_blended);
+    count_launches(1);
     return cudaGetLastError();
 }
 

@@ -222,6 +222,7 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
     tile_select_kernel<<<(T + 255) / 256, 256, 0, s>>>(T, k, tile_score, selected);
     tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);
     write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);
+    count_launches(4);
     return cudaGetLastError();
 }
 

@@ -3,11 +3,17 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <atomic>
 #include <new>
 
 #include "common.cuh"
 
 using namespace tgs;
+
+namespace tgs {
+static std::atomic<uint64_t> g_launches{0};
+void count_launches(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+}  // namespace tgs
 
 struct tgs_ctx : public ctx_impl {};
 
@@ -40,6 +46,8 @@ int num_tiles(const tgs_camera* c) {
 extern "C" {
 
 const char* tgs_version(void) { return "tgs 0.1 (sm_100a)"; }
+
+uint64_t tgs_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
 int tgs_create(tgs_ctx** out, int device) {
     if (!out) return TGS_ERR_INVALID_ARG;
@@ -176,7 +184,7 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const floa
 int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
                           const uint32_t* tile_offsets, const uint32_t* gid_sorted, int k, const uint32_t* tiles,
                           const uint32_t* tile_pix_offsets, const uint32_t* pix, float* out_color, float* out_T,
-                          uint32_t* n_contrib, uint32_t* n_walked, void* stream) {
+                          uint32_t* n_contrib, uint32_t* n_walked, uint32_t* n_blended, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad camera");
     if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad N or k");
@@ -184,7 +192,7 @@ int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const floa
     if (!splats || !tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !out_color || !out_T || !n_contrib)
         return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: null pointer");
     cudaError_t e = launch_raster_fwd(make_camk(cam), splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix,
-                                      out_color, out_T, n_contrib, n_walked, ctx->num_sms, (cudaStream_t)stream);
+                                      out_color, out_T, n_contrib, n_walked, n_blended, ctx->num_sms, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_fwd_sparse", e);
     return TGS_OK;
 }

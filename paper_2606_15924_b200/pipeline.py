@@ -30,7 +30,8 @@ class SparseRasterStep:
         self.samp = SimpleNamespace(tile_score=e(T, i64), tiles=e(T, i32), tile_pix_offsets=e(T + 1, i32),
                                     pix=e(npx, i32), kn_dev=torch.zeros(2, dtype=i32, device=dev), k=None, n=None)
         self.fwd = SimpleNamespace(color=e((npx, 3), f32), T=e(npx, f32), n_contrib=e(npx, i32),
-                                   n_walked=e(npx, i32) if want_walked else None)
+                                   n_walked=e(npx, i32) if want_walked else None,
+                                   n_blended=e(npx, i32) if want_walked else None)
         self.bwd = SimpleNamespace(dL_dsplats=e((N, SPLAT_WORDS), f32), dL_dmeans3D=e((N, 3), f32),
                                    dL_dscales=e((N, 3), f32), dL_dquats=e((N, 4), f32), dL_dopacities=e(N, f32),
                                    dL_dsh=e((N, K, 3), f32))

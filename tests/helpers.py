@@ -107,21 +107,32 @@ def tainted_gaussians(N, binned, samp, ofwd, margin=MARGIN):
     return bad
 
 
-def check_grad(name, got, ref, good_rows=None, rtol=GRAD_RTOL, atol=GRAD_ATOL, scale_floor=None):
-    """|got - ref| <= atol + rtol * max(|ref|, scale_floor) elementwise on the rows in good_rows.
+def check_grad(name, got, ref, tainted=None, rtol=GRAD_RTOL, atol=GRAD_ATOL):
+    """Gradient comparison, rows = Gaussians, columns = the components of one parameter block.
 
-    scale_floor (optional, per row) is the magnitude of the terms that were summed to form the
-    element (sum of |terms|): when a gradient is a cancelling sum, fp32 accumulation-order noise is
-    relative to that magnitude, not to the (much smaller) result."""
-    got = np.asarray(got, np.float64).reshape(len(ref), -1)
+    1. Elementwise bar (north_star): |got - ref| <= atol + rtol * |ref|.
+    2. An element that misses (1) must be a cancelling sum: it has to pass the same bar measured
+       against the largest component of its own block, |got - ref| <= atol + rtol * max_row|ref|
+       (fp32 accumulation-order noise scales with the summed terms, not with a result that cancelled),
+       and such elements must be rare (<= 2 + 1e-4 of all elements).  Their count is returned.
+    3. Rows in `tainted` (a pixel that reaches the Gaussian sits on a decision threshold, so the
+       GPU may legitimately have replayed one Gaussian more or less) are held to the loose bound
+       atol + rtol * max|ref| over the whole array instead.
+    """
     ref2 = np.asarray(ref, np.float64).reshape(len(ref), -1)
-    if good_rows is not None:
-        got, ref2 = got[good_rows], ref2[good_rows]
-        if scale_floor is not None:
-            scale_floor = np.asarray(scale_floor).reshape(len(ref), -1)[good_rows]
-    mag = np.abs(ref2) if scale_floor is None else np.maximum(np.abs(ref2), scale_floor)
-    d = np.abs(got - ref2)
-    bad = d > atol + rtol * mag
-    assert not bad.any(), (f"{name}: {int(bad.sum())}/{bad.size} out of tolerance; worst abs {d.max():.3e}, "
-                           f"worst ratio {(d / (atol + rtol * mag)).max():.2f}")
-    return float((d / (atol + rtol * mag)).max()) if d.size else 0.0
+    got2 = np.asarray(got, np.float64).reshape(len(ref), -1)
+    assert np.isfinite(got2).all(), f"{name}: non-finite values"
+    d = np.abs(got2 - ref2)
+    tol = atol + rtol * np.abs(ref2)
+    viol = d > tol
+    taint = np.zeros(len(ref2), bool) if tainted is None else np.asarray(tainted, bool)
+    block = np.abs(ref2).max(axis=1, keepdims=True)
+    v = viol & ~taint[:, None]
+    over = d > atol + rtol * np.broadcast_to(block, d.shape)
+    assert not (v & over).any(), (f"{name}: {int((v & over).sum())} elements out of tolerance even against their block "
+                                  f"norm; worst abs {d[v & over].max():.3e}")
+    assert v.sum() <= 2 + 1e-4 * v.size, f"{name}: {int(v.sum())}/{v.size} elements miss the elementwise bar"
+    vt = viol & taint[:, None]
+    if vt.any():
+        assert d[vt].max() <= atol + rtol * np.abs(ref2).max(), f"{name}: tainted row off by {d[vt].max():.3e}"
+    return dict(miss=int(v.sum()), miss_tainted=int(vt.sum()), worst_ratio=float((d / tol)[~taint].max()) if (~taint).any() else 0.0)
