@@ -22,6 +22,7 @@ constexpr float kTMin = 0.0001f;
 struct ctx_impl {
     int device;
     int num_sms;
+    uint32_t* sched;  // device, 8 words: work-unit counters of the persistent raster kernels (self re-arming)
     char err[512];
 };
 
@@ -72,12 +73,12 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, uint32_t* n_blended, int num_sms, cudaStream_t s);
+                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s);
 
 cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
-                              const float* dL_dcolor, float* dL_dsplats, int num_sms, cudaStream_t s);
+                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s);
 
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                                const float* sh, const int32_t* radii, const uint8_t* clamped,

@@ -1,123 +1,176 @@
 // tgs_raster_bwd_sparse, raster half: back-to-front replay of Eq. 1 over the sampled
 // pixels only, producing dL/d(mean2D, conic, opacity, rgb) per Gaussian.
-// One block per sampled tile; per-Gaussian partials are reduced across the warp with shuffles and
-// one lane issues the global atomics (north_star: "warp-shuffle reduction of per-Gaussian gradients
-// before global atomics").
-#include "common.cuh"
+//
+// Same decomposition as the forward (raster_common.cuh): persistent warps, one (tile, 32-pixel
+// group) unit at a time, the tile's range walked from the warp's deepest contributor backwards in
+// batches of 32 with the per-warp cull.  For every surviving Gaussian the nine per-pixel partials are
+// summed across the warp with a butterfly (8 values in 9 shuffles + the 9th in 5), written to the
+// warp's shared-memory slice, and after the batch each lane flushes ONE Gaussian's nine sums with
+// global float atomics -- 9 atomic instructions per 32 Gaussians instead of per Gaussian
+// (north_star: "warp-shuffle reduction of per-Gaussian gradients before global atomics").
+#include "raster_common.cuh"
 
 namespace tgs {
 
 namespace {
 
-constexpr int kBwdThreads = 256;
-constexpr int kBatch = 256;
+struct WarpAcc {
+    float v[32][9];   // row stride 9 words: conflict-free when lane e reads row e
+    uint32_t g[32];   // Gaussian id of each staged entry
+};
 
-__device__ __forceinline__ float warp_sum(float v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
+// keep/send exchange of one butterfly step: lanes with `hi` keep b and send a, the others keep a
+__device__ __forceinline__ float bfly(float a, float b, bool hi, int mask) {
+    const float send = hi ? a : b;
+    const float keep = hi ? b : a;
+    return keep + __shfl_xor_sync(0xffffffffu, send, mask);
 }
 
-__global__ void __launch_bounds__(kBwdThreads)
+// Sums v[0..8] over the 32 lanes and stores the nine totals to row[0..8].
+__device__ __forceinline__ void warp_reduce9_store(const float (&v)[9], float* row, int lane) {
+    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+    // quantities 0-3 end up in lanes with bit4 = 0, 4-7 in lanes with bit4 = 1, ...
+    const float a0 = bfly(v[0], v[4], h16, 16), a1 = bfly(v[1], v[5], h16, 16);
+    const float a2 = bfly(v[2], v[6], h16, 16), a3 = bfly(v[3], v[7], h16, 16);
+    const float b0 = bfly(a0, a2, h8, 8), b1 = bfly(a1, a3, h8, 8);
+    float c0 = bfly(b0, b1, h4, 4);
+    c0 += __shfl_xor_sync(0xffffffffu, c0, 2);
+    c0 += __shfl_xor_sync(0xffffffffu, c0, 1);
+    float e = v[8];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    // lane L (L % 4 == 0) holds quantity 4*bit4 + 2*bit3 + bit2 = L >> 2
+    if ((lane & 3) == 0) row[lane >> 2] = c0;
+    if (lane == 1) row[8] = e;
+}
+
+__global__ void __launch_bounds__(kRasterThreads, 3)
 raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
                   const float* __restrict__ out_T, const uint32_t* __restrict__ n_contrib,
-                  const float* __restrict__ dL_dcolor, float* __restrict__ dL_dsplats) {
-    __shared__ float4 s_a[kBatch];  // mx, my, -A/2, -B
-    __shared__ float4 s_b[kBatch];  // -C/2, opacity, r, g
-    __shared__ float s_c[kBatch];   // b
-    __shared__ uint32_t s_g[kBatch];
-    __shared__ uint32_t s_max;
+                  const float* __restrict__ dL_dcolor, float* __restrict__ dL_dsplats, uint32_t* __restrict__ sched) {
+    __shared__ WarpBatch s_batch[kRasterWarps];
+    __shared__ WarpAcc s_acc[kRasterWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpBatch& sb = s_batch[warp];
+    WarpAcc& sa = s_acc[warp];
+    const uint32_t num_units = (uint32_t)k * 8u;
+    const uint32_t lt_mask = (1u << lane) - 1u;
 
-    const int lane = threadIdx.x & 31;
-    for (int it = blockIdx.x; it < k; it += gridDim.x) {
-        const uint32_t t = tiles[it];
-        const uint32_t start = tile_offsets[t];
-        const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
-        const bool active = threadIdx.x < m;
-        float px = 0.f, py = 0.f, Tf = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f;
+    for (;;) {
+        uint32_t u = 0;
+        if (lane == 0) u = atomicAdd(&sched[0], 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= num_units) break;
+        UnitInfo ui;
+        if (!decode_unit(u, tiles, tile_offsets, tpo, ui)) continue;
+
+        const bool active = (uint32_t)lane < ui.npix;
+        int ipx = 0, ipy = 0;
+        float Tf = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f;
         uint32_t last = 0;
         if (active) {
-            const uint32_t o = p0 + threadIdx.x;
+            const uint32_t o = ui.pix0 + lane;
             const uint32_t id = pix[o];
-            px = (float)(id % (uint32_t)cam.W);
-            py = (float)(id / (uint32_t)cam.W);
+            ipx = (int)(id % (uint32_t)cam.W);
+            ipy = (int)(id / (uint32_t)cam.W);
             Tf = out_T[o];
             last = n_contrib[o];
             g0 = dL_dcolor[3 * (size_t)o]; g1 = dL_dcolor[3 * (size_t)o + 1]; g2 = dL_dcolor[3 * (size_t)o + 2];
         }
-        if (threadIdx.x == 0) s_max = 0;
-        __syncthreads();
-        {
-            uint32_t wm = __reduce_max_sync(0xffffffffu, last);
-            if (lane == 0 && wm) atomicMax(&s_max, wm);
-        }
-        __syncthreads();
-        const uint32_t max_last = s_max;
+        const uint32_t wmax = __reduce_max_sync(0xffffffffu, last);
+        if (wmax == 0) continue;
+        const float bx0 = (float)__reduce_min_sync(0xffffffffu, active ? ipx : 0x7fffffff);
+        const float by0 = (float)__reduce_min_sync(0xffffffffu, active ? ipy : 0x7fffffff);
+        const float bx1 = (float)__reduce_max_sync(0xffffffffu, active ? ipx : -1);
+        const float by1 = (float)__reduce_max_sync(0xffffffffu, active ? ipy : -1);
+        const float px = (float)ipx, py = (float)ipy;
         const float bgdot = (cam.bg[0] * g0 + cam.bg[1] * g1 + cam.bg[2] * g2) * Tf;
         float T = Tf, S0 = 0.f, S1 = 0.f, S2 = 0.f;
 
-        // batches of the range [0, max_last), from the back
-        for (uint32_t hi = max_last; hi > 0;) {
-            const uint32_t cnt = min((uint32_t)kBatch, hi);
-            const uint32_t b0 = hi - cnt;
-            __syncthreads();
-            if (threadIdx.x < cnt) {
-                const uint32_t g = gid_sorted[start + b0 + threadIdx.x];
-                const float4 r0 = splats[3 * (size_t)g], r1 = splats[3 * (size_t)g + 1];
-                const float bl = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
-                s_a[threadIdx.x] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
-                s_b[threadIdx.x] = make_float4(-0.5f * r1.x, r1.y, r1.z, r1.w);
-                s_c[threadIdx.x] = bl;
-                s_g[threadIdx.x] = g;
+        // lane l of a batch owns range position hi-1-l: survivors stay in descending position order
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+        float r2x = 0.f;
+        uint32_t gcur = 0;
+        if ((uint32_t)lane < wmax) {
+            gcur = gid_sorted[ui.start + wmax - 1 - lane];
+            r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
+            r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
+        }
+        for (uint32_t hi = wmax; hi > 0; hi = hi > 32 ? hi - 32 : 0) {
+            const bool have = (uint32_t)lane < hi;
+            const float thr = (kLnAlphaMin - __logf(r1.y)) - 1e-5f;
+            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, bx0, by0, bx1, by1);
+            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
+            const int cnt = __popc(ballot);
+            if (pass) {
+                const int slot = __popc(ballot & lt_mask);
+                sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
+                sb.b[slot] = make_float2(-0.5f * r1.x, thr);
+                sb.c[slot] = make_float4(r1.y, r1.z, r1.w, r2x);
+                sb.p[slot] = hi - 1 - lane;  // 0-based range position
+                sa.g[slot] = gcur;
             }
-            __syncthreads();
-            for (int jj = (int)cnt - 1; jj >= 0; --jj) {
-                const uint32_t pos = b0 + (uint32_t)jj;
-                const float4 a = s_a[jj];
-                const float4 bb = s_b[jj];
+            __syncwarp();
+            if (hi > 32 && (uint32_t)lane < hi - 32) {
+                gcur = gid_sorted[ui.start + hi - 33 - lane];
+                r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
+                r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
+            }
+            uint32_t touched = 0;
+            for (int e = 0; e < cnt; ++e) {
+                const float4 a = sb.a[e];
+                const float2 b = sb.b[e];
                 const float dx = a.x - px, dy = a.y - py;
-                const float power = __fmaf_rn(__fmaf_rn(a.w, dy, __fmul_rn(a.z, dx)), dx,
-                                              __fmul_rn(__fmul_rn(bb.x, dy), dy));
-                const float G = __expf(power);
-                const float oG = __fmul_rn(bb.y, G);
+                const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                bool valid = sb.p[e] < last && power >= b.y && power <= 0.0f;
+                const float4 c = sb.c[e];
+                const float G = ex2_approx(power * kLog2e);
+                const float oG = __fmul_rn(c.x, G);
                 const float alpha = fminf(kAlphaMax, oG);
-                const bool valid = active && pos < last && !(power > 0.0f) && !(alpha < kAlphaMin);
+                valid = valid && !(alpha < kAlphaMin);
                 if (!__any_sync(0xffffffffu, valid)) continue;
-                float d_mx = 0.f, d_my = 0.f, d_A = 0.f, d_B = 0.f, d_C = 0.f, d_o = 0.f, d_r = 0.f, d_g = 0.f, d_b = 0.f;
+                touched |= 1u << e;
+                float v[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
                 if (valid) {
                     const float om = 1.0f - alpha;
                     const float rom = __frcp_rn(om);
                     T = T * rom;  // T_k
                     const float w = alpha * T;
-                    const float cb = s_c[jj];
-                    d_r = w * g0; d_g = w * g1; d_b = w * g2;
-                    float dL_dalpha = ((bb.z - S0) * g0 + (bb.w - S1) * g1 + (cb - S2) * g2) * T - bgdot * rom;
-                    S0 = fmaf(alpha, bb.z, om * S0); S1 = fmaf(alpha, bb.w, om * S1); S2 = fmaf(alpha, cb, om * S2);
+                    v[6] = w * g0; v[7] = w * g1; v[8] = w * g2;
+                    const float dL_dalpha = ((c.y - S0) * g0 + (c.z - S1) * g1 + (c.w - S2) * g2) * T - bgdot * rom;
+                    S0 = fmaf(alpha, c.y, om * S0); S1 = fmaf(alpha, c.z, om * S1); S2 = fmaf(alpha, c.w, om * S2);
                     if (oG < kAlphaMax) {  // zero derivative through the active 0.99 clamp
                         const float dpow = oG * dL_dalpha;
-                        d_o = G * dL_dalpha;
+                        v[5] = G * dL_dalpha;
                         // -A dx - B dy = 2(-A/2) dx + (-B) dy ; -C dy - B dx = 2(-C/2) dy + (-B) dx
-                        d_mx = dpow * fmaf(2.0f * a.z, dx, a.w * dy);
-                        d_my = dpow * fmaf(2.0f * bb.x, dy, a.w * dx);
-                        d_A = -0.5f * dx * dx * dpow;
-                        d_B = -dx * dy * dpow;
-                        d_C = -0.5f * dy * dy * dpow;
+                        v[0] = dpow * fmaf(2.0f * a.z, dx, a.w * dy);
+                        v[1] = dpow * fmaf(2.0f * b.x, dy, a.w * dx);
+                        v[2] = -0.5f * dx * dx * dpow;
+                        v[3] = -dx * dy * dpow;
+                        v[4] = -0.5f * dy * dy * dpow;
                     }
                 }
-                d_mx = warp_sum(d_mx); d_my = warp_sum(d_my); d_A = warp_sum(d_A); d_B = warp_sum(d_B);
-                d_C = warp_sum(d_C); d_o = warp_sum(d_o); d_r = warp_sum(d_r); d_g = warp_sum(d_g); d_b = warp_sum(d_b);
-                if (lane == 0) {
-                    float* dst = dL_dsplats + (size_t)s_g[jj] * kSplatWords;
-                    atomicAdd(dst + 0, d_mx); atomicAdd(dst + 1, d_my); atomicAdd(dst + 2, d_A);
-                    atomicAdd(dst + 3, d_B); atomicAdd(dst + 4, d_C); atomicAdd(dst + 5, d_o);
-                    atomicAdd(dst + 6, d_r); atomicAdd(dst + 7, d_g); atomicAdd(dst + 8, d_b);
-                }
+                warp_reduce9_store(v, sa.v[e], lane);
             }
-            hi = b0;
+            __syncwarp();
+            // flush: lane e owns staged entry e
+            if (lane < cnt && (touched >> lane) & 1u) {
+                float* dst = dL_dsplats + (size_t)sa.g[lane] * kSplatWords;
+#pragma unroll
+                for (int q = 0; q < 9; ++q) atomicAdd(dst + q, sa.v[lane][q]);
+            }
+            __syncwarp();
         }
-        __syncthreads();
+    }
+    if (lane == 0) {
+        const uint32_t total = gridDim.x * kRasterWarps;
+        if (atomicAdd(&sched[1], 1u) == total - 1u) {
+            sched[0] = 0u;
+            sched[1] = 0u;
+            __threadfence();
+        }
     }
 }
 
@@ -126,14 +179,16 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
 cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
-                              const float* dL_dcolor, float* dL_dsplats, int num_sms, cudaStream_t s) {
-    (void)num_sms;
+                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s) {
     cudaError_t e = cudaMemsetAsync(dL_dsplats, 0, (size_t)N * kSplatWords * sizeof(float), s);
     if (e != cudaSuccess) return e;
     if (k <= 0) return cudaSuccess;
-    raster_bwd_kernel<<<k, kBwdThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
-                                                gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
-                                                dL_dsplats);
+    int blocks = num_sms * 3;
+    const int need = (k * 8 + kRasterWarps - 1) / kRasterWarps;
+    if (blocks > need) blocks = need;
+    raster_bwd_kernel<<<blocks, kRasterThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
+                                                        gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
+                                                        dL_dsplats, sched);
     count_launches(1);
     return cudaGetLastError();
 }

@@ -1,90 +1,143 @@
 // tgs_raster_fwd_sparse: front-to-back alpha compositing (Eq. 1) for the SAMPLED
-// pixels only, one thread block per valid sampled tile (Fig. 6), Gaussian
-// records of the tile's depth-ordered range staged through shared memory in batches.
+// pixels only (Fig. 6: sampled pixels listed tile by tile, tile-wise pixel
+// offsets by prefix sum, tile-parallel execution).
 //
-// power is evaluated with one fixed fused sequence:
-//   power = fma(fma(-B, dy, (-A/2) dx), dx, ((-C/2) dy) dy)
-// so that the skip decisions (power > 0, alpha < 1/255, T < 1e-4) are taken on the same bits as the
-// oracle's; only exp differs (ex2.approx vs libm), within tolerance.
-#include "common.cuh"
+// B200 design (raster_common.cuh): persistent warps pull (tile, 32-pixel group) units from an
+// atomic counter; each warp stages its tile's depth-ordered Gaussians 32 at a time (one float4
+// record load per lane, next batch prefetched into registers while the current one is consumed),
+// culls them against the bounding box of its own 32 pixels and walks only the survivors.  The
+// alpha >= 1/255 test is done on power against a per-Gaussian threshold ln(1/(255 o)) BEFORE the
+// exp, so a skipped evaluation costs two shared loads, seven FP32 ops and two compares.
+//
+// power uses the one fixed fused sequence of DESIGN.md "canonical arithmetic", so `power > 0` is
+// decided on the same bits as the oracle; alpha itself is o * ex2.approx(power * log2 e).
+#include "raster_common.cuh"
 
 namespace tgs {
 
 namespace {
 
-constexpr int kFwdThreads = 256;
-constexpr int kBatch = 256;
-
-__global__ void __launch_bounds__(kFwdThreads)
+template <bool COUNT>
+__global__ void __launch_bounds__(kRasterThreads, 4)
 raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
                   float* __restrict__ out_color, float* __restrict__ out_T, uint32_t* __restrict__ n_contrib,
-                  uint32_t* __restrict__ n_walked, uint32_t* __restrict__ n_blended) {
-    __shared__ float4 s_a[kBatch];  // mx, my, -A/2, -B
-    __shared__ float4 s_b[kBatch];  // -C/2, opacity, r, g
-    __shared__ float s_c[kBatch];   // b
+                  uint32_t* __restrict__ n_walked, uint32_t* __restrict__ n_blended, uint32_t* __restrict__ sched) {
+    __shared__ WarpBatch s_batch[kRasterWarps];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpBatch& sb = s_batch[warp];
+    const uint32_t num_units = (uint32_t)k * 8u;
+    const uint32_t lt_mask = (1u << lane) - 1u;
 
-    for (int it = blockIdx.x; it < k; it += gridDim.x) {
-        const uint32_t t = tiles[it];
-        const uint32_t start = tile_offsets[t], end = tile_offsets[t + 1];
-        const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
-        const bool active = threadIdx.x < m;
-        float px = 0.f, py = 0.f;
+    for (;;) {
+        uint32_t u = 0;
+        if (lane == 0) u = atomicAdd(&sched[0], 1u);
+        u = __shfl_sync(0xffffffffu, u, 0);
+        if (u >= num_units) break;
+        UnitInfo ui;
+        if (!decode_unit(u, tiles, tile_offsets, tpo, ui)) continue;
+
+        const bool active = (uint32_t)lane < ui.npix;
+        int ipx = 0, ipy = 0;
         if (active) {
-            const uint32_t id = pix[p0 + threadIdx.x];
-            px = (float)(id % (uint32_t)cam.W);
-            py = (float)(id / (uint32_t)cam.W);
+            const uint32_t id = pix[ui.pix0 + lane];
+            ipx = (int)(id % (uint32_t)cam.W);
+            ipy = (int)(id / (uint32_t)cam.W);
         }
+        // bounding box of the warp's pixels (inactive lanes must not widen it)
+        const float bx0 = (float)__reduce_min_sync(0xffffffffu, active ? ipx : 0x7fffffff);
+        const float by0 = (float)__reduce_min_sync(0xffffffffu, active ? ipy : 0x7fffffff);
+        const float bx1 = (float)__reduce_max_sync(0xffffffffu, active ? ipx : -1);
+        const float by1 = (float)__reduce_max_sync(0xffffffffu, active ? ipy : -1);
+        const float px = (float)ipx, py = (float)ipy;
+
         float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-        uint32_t last = 0, walked = 0, blended = 0;
+        uint32_t last = 0, walked = ui.end - ui.start, blended = 0;
         bool done = !active;
 
-        for (uint32_t b0 = start; b0 < end; b0 += kBatch) {
-            if (__syncthreads_count(done) == kFwdThreads) break;
-            const uint32_t j = b0 + threadIdx.x;
-            if (j < end) {
-                const uint32_t g = gid_sorted[j];
-                const float4 r0 = splats[3 * (size_t)g], r1 = splats[3 * (size_t)g + 1];
-                const float bl = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
-                s_a[threadIdx.x] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
-                s_b[threadIdx.x] = make_float4(-0.5f * r1.x, r1.y, r1.z, r1.w);
-                s_c[threadIdx.x] = bl;
+        // prefetch the first batch into registers
+        float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+        float r2x = 0.f;
+        uint32_t j = ui.start + lane;
+        if (j < ui.end) {
+            const uint32_t g = gid_sorted[j];
+            r0 = splats[3 * (size_t)g]; r1 = splats[3 * (size_t)g + 1];
+            r2x = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
+        }
+        for (uint32_t base = ui.start; base < ui.end; base += 32) {
+            // ---- stage: cull against the pixel box, compact survivors in range order ----
+            const bool have = base + lane < ui.end;
+            // ln(1/(255 o)), lowered a hair so that rounding never rejects a Gaussian the exact alpha test keeps
+            const float thr = (kLnAlphaMin - __logf(r1.y)) - 1e-5f;
+            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, bx0, by0, bx1, by1);
+            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
+            const int cnt = __popc(ballot);
+            if (pass) {
+                const int slot = __popc(ballot & lt_mask);
+                sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
+                sb.b[slot] = make_float2(-0.5f * r1.x, thr);
+                sb.c[slot] = make_float4(r1.y, r1.z, r1.w, r2x);
+                sb.p[slot] = (base - ui.start) + lane + 1;
             }
-            __syncthreads();
+            __syncwarp();
+            // ---- prefetch the next batch ----
+            j = base + 32 + lane;
+            if (j < ui.end) {
+                const uint32_t g = gid_sorted[j];
+                r0 = splats[3 * (size_t)g]; r1 = splats[3 * (size_t)g + 1];
+                r2x = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
+            }
+            // ---- walk the survivors ----
             if (!done) {
-                const uint32_t cnt = min((uint32_t)kBatch, end - b0);
-                for (uint32_t jj = 0; jj < cnt; ++jj) {
-                    ++walked;
-                    const float4 a = s_a[jj];
+#pragma unroll 4
+                for (int e = 0; e < cnt; ++e) {
+                    const float4 a = sb.a[e];
+                    const float2 b = sb.b[e];
                     const float dx = a.x - px, dy = a.y - py;
-                    const float power = __fmaf_rn(__fmaf_rn(a.w, dy, __fmul_rn(a.z, dx)), dx,
-                                                  __fmul_rn(__fmul_rn(s_b[jj].x, dy), dy));
-                    if (power > 0.0f) continue;
-                    const float4 bb = s_b[jj];
-                    const float alpha = fminf(kAlphaMax, __fmul_rn(bb.y, __expf(power)));
-                    if (alpha < kAlphaMin) continue;
+                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                    if (!(power >= b.y && power <= 0.0f)) continue;  // alpha < 1/255 or power > 0
+                    const float4 c = sb.c[e];
+                    const float alpha = fminf(kAlphaMax, __fmul_rn(c.x, ex2_approx(power * kLog2e)));
+                    if (alpha < kAlphaMin) continue;  // the threshold test is exact up to rounding; keep the definition
                     const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
-                    if (Tn < kTMin) { done = true; break; }
+                    if (Tn < kTMin) {
+                        done = true;
+                        walked = sb.p[e];
+                        break;
+                    }
                     const float w = alpha * T;
-                    C0 = fmaf(bb.z, w, C0); C1 = fmaf(bb.w, w, C1); C2 = fmaf(s_c[jj], w, C2);
+                    C0 = fmaf(c.y, w, C0); C1 = fmaf(c.z, w, C1); C2 = fmaf(c.w, w, C2);
                     T = Tn;
-                    ++blended;
-                    last = (b0 - start) + jj + 1;
+                    last = sb.p[e];
+                    if (COUNT) ++blended;
                 }
             }
+            if (__all_sync(0xffffffffu, done)) break;
+            __syncwarp();  // the batch slice is rewritten next iteration
         }
         if (active) {
-            const uint32_t o = p0 + threadIdx.x;
+            const uint32_t o = ui.pix0 + lane;
             out_color[3 * (size_t)o] = fmaf(T, cam.bg[0], C0);
             out_color[3 * (size_t)o + 1] = fmaf(T, cam.bg[1], C1);
             out_color[3 * (size_t)o + 2] = fmaf(T, cam.bg[2], C2);
             out_T[o] = T;
             n_contrib[o] = last;
-            if (n_walked) n_walked[o] = walked;
-            if (n_blended) n_blended[o] = blended;
+            if (COUNT) {
+                if (n_walked) n_walked[o] = walked;
+                if (n_blended) n_blended[o] = blended;
+            }
         }
-        __syncthreads();  // shared batch buffers are reused by the next tile
+        __syncwarp();
+    }
+    // the last warp to leave re-arms the scheduler for the next launch
+    if (lane == 0) {
+        const uint32_t total = gridDim.x * kRasterWarps;
+        if (atomicAdd(&sched[1], 1u) == total - 1u) {
+            sched[0] = 0u;
+            sched[1] = 0u;
+            __threadfence();
+        }
     }
 }
 
@@ -93,12 +146,21 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, uint32_t* n_blended, int num_sms, cudaStream_t s) {
-    (void)num_sms;
+                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s) {
     if (k <= 0) return cudaSuccess;
-    raster_fwd_kernel<<<k, kFwdThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
-                                                gid_sorted, k, tiles, tpo, pix, out_color, out_T, n_contrib,
-                                                n_walked, n_blended);
+    const bool count = n_walked || n_blended;
+    int per_sm = 4;
+    // persistent grid: never more warps than units
+    int blocks = num_sms * per_sm;
+    const int need = (k * 8 + kRasterWarps - 1) / kRasterWarps;
+    if (blocks > need) blocks = need;
+    const float4* sp = reinterpret_cast<const float4*>(splats);
+    if (count)
+        raster_fwd_kernel<true><<<blocks, kRasterThreads, 0, s>>>(cam, sp, tile_offsets, gid_sorted, k, tiles, tpo, pix,
+                                                                  out_color, out_T, n_contrib, n_walked, n_blended, sched);
+    else
+        raster_fwd_kernel<false><<<blocks, kRasterThreads, 0, s>>>(cam, sp, tile_offsets, gid_sorted, k, tiles, tpo, pix,
+                                                                   out_color, out_T, n_contrib, n_walked, n_blended, sched);
     count_launches(1);
     return cudaGetLastError();
 }
