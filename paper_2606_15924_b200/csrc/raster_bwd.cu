@@ -3,10 +3,12 @@
 //
 // Same decomposition as the forward (raster_common.cuh): persistent warps, one (tile, 32-pixel
 // group) unit at a time, the tile's range walked from the warp's deepest contributor backwards in
-// batches of 32 with the per-warp cull.  For every surviving Gaussian the nine per-pixel partials are
-// summed across the warp with a butterfly (8 values in 9 shuffles + the 9th in 5), written to the
-// warp's shared-memory slice, and after the batch each lane flushes ONE Gaussian's nine sums with
-// global float atomics -- 9 atomic instructions per 32 Gaussians instead of per Gaussian
+// batches of 32 with the per-warp cull.  Per surviving Gaussian each lane forms nine partial sums
+// for its pixel -- three colour terms, dL/dopacity and the five moments dpow*(dx, dy, dx^2, dx dy,
+// dy^2) from which the mean2D / conic gradients follow linearly -- which are summed across the warp
+// with a butterfly (8 values in 9 shuffles + the 9th in 5) into the warp's shared-memory slice;
+// after the batch each lane turns ONE Gaussian's sums into its nine gradient components and issues
+// the global float atomics: 9 atomic instructions per 32 Gaussians instead of per Gaussian
 // (north_star: "warp-shuffle reduction of per-Gaussian gradients before global atomics").
 #include "raster_common.cuh"
 
@@ -15,8 +17,7 @@ namespace tgs {
 namespace {
 
 struct WarpAcc {
-    float v[32][9];   // row stride 9 words: conflict-free when lane e reads row e
-    uint32_t g[32];   // Gaussian id of each staged entry
+    float v[32][9];  // row stride 9 words: conflict-free when lane e reads row e
 };
 
 // keep/send exchange of one butterfly step: lanes with `hi` keep b and send a, the others keep a
@@ -29,7 +30,6 @@ __device__ __forceinline__ float bfly(float a, float b, bool hi, int mask) {
 // Sums v[0..8] over the 32 lanes and stores the nine totals to row[0..8].
 __device__ __forceinline__ void warp_reduce9_store(const float (&v)[9], float* row, int lane) {
     const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
-    // quantities 0-3 end up in lanes with bit4 = 0, 4-7 in lanes with bit4 = 1, ...
     const float a0 = bfly(v[0], v[4], h16, 16), a1 = bfly(v[1], v[5], h16, 16);
     const float a2 = bfly(v[2], v[6], h16, 16), a3 = bfly(v[3], v[7], h16, 16);
     const float b0 = bfly(a0, a2, h8, 8), b1 = bfly(a1, a3, h8, 8);
@@ -44,7 +44,7 @@ __device__ __forceinline__ void warp_reduce9_store(const float (&v)[9], float* r
     if (lane == 1) row[8] = e;
 }
 
-__global__ void __launch_bounds__(kRasterThreads, 3)
+__global__ void __launch_bounds__(kRasterThreads, 4)
 raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
@@ -64,14 +64,13 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= num_units) break;
         UnitInfo ui;
-        if (!decode_unit(u, tiles, tile_offsets, tpo, ui)) continue;
+        if (!decode_unit(u, lane, tiles, tile_offsets, tpo, ui)) continue;
 
-        const bool active = (uint32_t)lane < ui.npix;
         int ipx = 0, ipy = 0;
         float Tf = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f;
         uint32_t last = 0;
-        if (active) {
-            const uint32_t o = ui.pix0 + lane;
+        if (ui.active) {
+            const uint32_t o = ui.slot;
             const uint32_t id = pix[o];
             ipx = (int)(id % (uint32_t)cam.W);
             ipy = (int)(id / (uint32_t)cam.W);
@@ -81,10 +80,7 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         }
         const uint32_t wmax = __reduce_max_sync(0xffffffffu, last);
         if (wmax == 0) continue;
-        const float bx0 = (float)__reduce_min_sync(0xffffffffu, active ? ipx : 0x7fffffff);
-        const float by0 = (float)__reduce_min_sync(0xffffffffu, active ? ipy : 0x7fffffff);
-        const float bx1 = (float)__reduce_max_sync(0xffffffffu, active ? ipx : -1);
-        const float by1 = (float)__reduce_max_sync(0xffffffffu, active ? ipy : -1);
+        const PixelBox box = warp_pixel_box(ui.active, ipx, ipy);
         const float px = (float)ipx, py = (float)ipy;
         const float bgdot = (cam.bg[0] * g0 + cam.bg[1] * g1 + cam.bg[2] * g2) * Tf;
         float T = Tf, S0 = 0.f, S1 = 0.f, S2 = 0.f;
@@ -92,86 +88,93 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         // lane l of a batch owns range position hi-1-l: survivors stay in descending position order
         float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
         float r2x = 0.f;
-        uint32_t gcur = 0;
+        uint32_t gcur = 0, g_next = 0;
         if ((uint32_t)lane < wmax) {
             gcur = gid_sorted[ui.start + wmax - 1 - lane];
             r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
             r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
         }
+        if ((uint32_t)lane + 32 < wmax) g_next = gid_sorted[ui.start + wmax - 33 - lane];
         for (uint32_t hi = wmax; hi > 0; hi = hi > 32 ? hi - 32 : 0) {
             const bool have = (uint32_t)lane < hi;
-            const float thr = (kLnAlphaMin - __logf(r1.y)) - 1e-5f;
-            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, bx0, by0, bx1, by1);
+            const float thr = blend_threshold(r1.y);
+            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, box);
             const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
             const int cnt = __popc(ballot);
             if (pass) {
                 const int slot = __popc(ballot & lt_mask);
                 sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
-                sb.b[slot] = make_float2(-0.5f * r1.x, thr);
-                sb.c[slot] = make_float4(r1.y, r1.z, r1.w, r2x);
-                sb.p[slot] = hi - 1 - lane;  // 0-based range position
-                sa.g[slot] = gcur;
+                sb.b[slot] = make_float4(-0.5f * r1.x, thr, r1.y, __uint_as_float(hi - 1 - lane));
+                sb.c[slot] = make_float4(r1.z, r1.w, r2x, __uint_as_float(gcur));
             }
             __syncwarp();
-            if (hi > 32 && (uint32_t)lane < hi - 32) {
-                gcur = gid_sorted[ui.start + hi - 33 - lane];
+            if ((uint32_t)lane + 32 < hi) {
+                gcur = g_next;
                 r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
                 r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
             }
+            if ((uint32_t)lane + 64 < hi) g_next = gid_sorted[ui.start + hi - 65 - lane];
+
             uint32_t touched = 0;
+#pragma unroll 2
             for (int e = 0; e < cnt; ++e) {
                 const float4 a = sb.a[e];
-                const float2 b = sb.b[e];
+                const float4 b = sb.b[e];
+                const float4 c = sb.c[e];
                 const float dx = a.x - px, dy = a.y - py;
                 const float power = splat_power(a.z, a.w, b.x, dx, dy);
-                bool valid = sb.p[e] < last && power >= b.y && power <= 0.0f;
-                const float4 c = sb.c[e];
-                const float G = ex2_approx(power * kLog2e);
-                const float oG = __fmul_rn(c.x, G);
+                // power is clamped for the exp only: G stays finite on lanes that fail the tests (no inf * 0)
+                const float G = ex2_approx(fminf(power, 0.0f) * kLog2e);
+                const float oG = __fmul_rn(b.z, G);
                 const float alpha = fminf(kAlphaMax, oG);
-                valid = valid && !(alpha < kAlphaMin);
+                const bool valid = (__float_as_uint(b.w) < last) && (power >= b.y) && (power <= 0.0f) &&
+                                   !(alpha < kAlphaMin);
                 if (!__any_sync(0xffffffffu, valid)) continue;
                 touched |= 1u << e;
-                float v[9] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                if (valid) {
+                float v[9];
+                {
                     const float om = 1.0f - alpha;
-                    const float rom = __frcp_rn(om);
-                    T = T * rom;  // T_k
-                    const float w = alpha * T;
+                    const float rom = rcp_approx(om);
+                    const float Tk = T * rom;  // T_k
+                    const float w = valid ? alpha * Tk : 0.0f;
                     v[6] = w * g0; v[7] = w * g1; v[8] = w * g2;
-                    const float dL_dalpha = ((c.y - S0) * g0 + (c.z - S1) * g1 + (c.w - S2) * g2) * T - bgdot * rom;
-                    S0 = fmaf(alpha, c.y, om * S0); S1 = fmaf(alpha, c.z, om * S1); S2 = fmaf(alpha, c.w, om * S2);
-                    if (oG < kAlphaMax) {  // zero derivative through the active 0.99 clamp
-                        const float dpow = oG * dL_dalpha;
-                        v[5] = G * dL_dalpha;
-                        // -A dx - B dy = 2(-A/2) dx + (-B) dy ; -C dy - B dx = 2(-C/2) dy + (-B) dx
-                        v[0] = dpow * fmaf(2.0f * a.z, dx, a.w * dy);
-                        v[1] = dpow * fmaf(2.0f * b.x, dy, a.w * dx);
-                        v[2] = -0.5f * dx * dx * dpow;
-                        v[3] = -dx * dy * dpow;
-                        v[4] = -0.5f * dy * dy * dpow;
+                    float dL_dalpha = ((c.x - S0) * g0 + (c.y - S1) * g1 + (c.z - S2) * g2) * Tk - bgdot * rom;
+                    dL_dalpha = valid ? dL_dalpha : 0.0f;
+                    if (valid) {
+                        T = Tk;
+                        S0 = fmaf(alpha, c.x, om * S0); S1 = fmaf(alpha, c.y, om * S1); S2 = fmaf(alpha, c.z, om * S2);
                     }
+                    // zero derivative through the active 0.99 clamp
+                    const float dLa = (oG < kAlphaMax) ? dL_dalpha : 0.0f;
+                    v[5] = G * dLa;               // dL/dopacity
+                    const float dpow = oG * dLa;  // dL/dpower
+                    v[0] = dpow * dx; v[1] = dpow * dy;
+                    v[2] = v[0] * dx; v[3] = v[0] * dy; v[4] = v[1] * dy;
                 }
                 warp_reduce9_store(v, sa.v[e], lane);
             }
             __syncwarp();
-            // flush: lane e owns staged entry e
+            // flush: lane e owns staged entry e; moments -> gradients
+            //   dL/dmx = sum dpow (-A dx - B dy),  dL/dA = -1/2 sum dpow dx^2,  dL/dB = -sum dpow dx dy, ...
             if (lane < cnt && (touched >> lane) & 1u) {
-                float* dst = dL_dsplats + (size_t)sa.g[lane] * kSplatWords;
-#pragma unroll
-                for (int q = 0; q < 9; ++q) atomicAdd(dst + q, sa.v[lane][q]);
+                const float4 a = sb.a[lane];
+                const float nC = sb.b[lane].x;
+                const float* m = sa.v[lane];
+                float* dst = dL_dsplats + (size_t)__float_as_uint(sb.c[lane].w) * kSplatWords;
+                atomicAdd(dst + 0, fmaf(2.0f * a.z, m[0], a.w * m[1]));
+                atomicAdd(dst + 1, fmaf(2.0f * nC, m[1], a.w * m[0]));
+                atomicAdd(dst + 2, -0.5f * m[2]);
+                atomicAdd(dst + 3, -m[3]);
+                atomicAdd(dst + 4, -0.5f * m[4]);
+                atomicAdd(dst + 5, m[5]);
+                atomicAdd(dst + 6, m[6]);
+                atomicAdd(dst + 7, m[7]);
+                atomicAdd(dst + 8, m[8]);
             }
             __syncwarp();
         }
     }
-    if (lane == 0) {
-        const uint32_t total = gridDim.x * kRasterWarps;
-        if (atomicAdd(&sched[1], 1u) == total - 1u) {
-            sched[0] = 0u;
-            sched[1] = 0u;
-            __threadfence();
-        }
-    }
+    scheduler_leave(sched, lane);
 }
 
 }  // namespace
@@ -183,7 +186,7 @@ cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const
     cudaError_t e = cudaMemsetAsync(dL_dsplats, 0, (size_t)N * kSplatWords * sizeof(float), s);
     if (e != cudaSuccess) return e;
     if (k <= 0) return cudaSuccess;
-    int blocks = num_sms * 3;
+    int blocks = num_sms * 4;
     const int need = (k * 8 + kRasterWarps - 1) / kRasterWarps;
     if (blocks > need) blocks = need;
     raster_bwd_kernel<<<blocks, kRasterThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,

@@ -4,10 +4,9 @@
 //
 // B200 design (raster_common.cuh): persistent warps pull (tile, 32-pixel group) units from an
 // atomic counter; each warp stages its tile's depth-ordered Gaussians 32 at a time (one float4
-// record load per lane, next batch prefetched into registers while the current one is consumed),
-// culls them against the bounding box of its own 32 pixels and walks only the survivors.  The
-// alpha >= 1/255 test is done on power against a per-Gaussian threshold ln(1/(255 o)) BEFORE the
-// exp, so a skipped evaluation costs two shared loads, seven FP32 ops and two compares.
+// record load per lane, prefetched into registers while the current batch is consumed), culls them
+// against the bounding box of its own 32 pixels and walks only the survivors with a branch-free,
+// unrolled inner loop (per survivor: three shared loads, ~25 FP32/ALU ops, one MUFU.EX2).
 //
 // power uses the one fixed fused sequence of DESIGN.md "canonical arithmetic", so `power > 0` is
 // decided on the same bits as the oracle; alpha itself is o * ex2.approx(power * log2 e).
@@ -18,7 +17,7 @@ namespace tgs {
 namespace {
 
 template <bool COUNT>
-__global__ void __launch_bounds__(kRasterThreads, 4)
+__global__ void __launch_bounds__(kRasterThreads, 5)
 raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
@@ -29,6 +28,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     WarpBatch& sb = s_batch[warp];
     const uint32_t num_units = (uint32_t)k * 8u;
     const uint32_t lt_mask = (1u << lane) - 1u;
+    const float kNaN = __int_as_float(0x7fc00000);
 
     for (;;) {
         uint32_t u = 0;
@@ -36,88 +36,86 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         u = __shfl_sync(0xffffffffu, u, 0);
         if (u >= num_units) break;
         UnitInfo ui;
-        if (!decode_unit(u, tiles, tile_offsets, tpo, ui)) continue;
+        if (!decode_unit(u, lane, tiles, tile_offsets, tpo, ui)) continue;
 
-        const bool active = (uint32_t)lane < ui.npix;
         int ipx = 0, ipy = 0;
-        if (active) {
-            const uint32_t id = pix[ui.pix0 + lane];
+        if (ui.active) {
+            const uint32_t id = pix[ui.slot];
             ipx = (int)(id % (uint32_t)cam.W);
             ipy = (int)(id / (uint32_t)cam.W);
         }
-        // bounding box of the warp's pixels (inactive lanes must not widen it)
-        const float bx0 = (float)__reduce_min_sync(0xffffffffu, active ? ipx : 0x7fffffff);
-        const float by0 = (float)__reduce_min_sync(0xffffffffu, active ? ipy : 0x7fffffff);
-        const float bx1 = (float)__reduce_max_sync(0xffffffffu, active ? ipx : -1);
-        const float by1 = (float)__reduce_max_sync(0xffffffffu, active ? ipy : -1);
-        const float px = (float)ipx, py = (float)ipy;
+        const PixelBox box = warp_pixel_box(ui.active, ipx, ipy);
+        // a finished (or inactive) lane carries px = NaN: power becomes NaN and every test fails
+        float px = ui.active ? (float)ipx : kNaN;
+        const float py = (float)ipy;
 
         float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
         uint32_t last = 0, walked = ui.end - ui.start, blended = 0;
-        bool done = !active;
 
-        // prefetch the first batch into registers
+        // software pipeline: ids two batches ahead, records one batch ahead
         float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
         float r2x = 0.f;
-        uint32_t j = ui.start + lane;
-        if (j < ui.end) {
-            const uint32_t g = gid_sorted[j];
-            r0 = splats[3 * (size_t)g]; r1 = splats[3 * (size_t)g + 1];
-            r2x = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
-        }
-        for (uint32_t base = ui.start; base < ui.end; base += 32) {
-            // ---- stage: cull against the pixel box, compact survivors in range order ----
-            const bool have = base + lane < ui.end;
-            // ln(1/(255 o)), lowered a hair so that rounding never rejects a Gaussian the exact alpha test keeps
-            const float thr = (kLnAlphaMin - __logf(r1.y)) - 1e-5f;
-            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, bx0, by0, bx1, by1);
-            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
-            const int cnt = __popc(ballot);
-            if (pass) {
-                const int slot = __popc(ballot & lt_mask);
-                sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
-                sb.b[slot] = make_float2(-0.5f * r1.x, thr);
-                sb.c[slot] = make_float4(r1.y, r1.z, r1.w, r2x);
-                sb.p[slot] = (base - ui.start) + lane + 1;
-            }
-            __syncwarp();
-            // ---- prefetch the next batch ----
-            j = base + 32 + lane;
+        uint32_t g_next = 0;
+        {
+            const uint32_t j = ui.start + lane;
             if (j < ui.end) {
                 const uint32_t g = gid_sorted[j];
                 r0 = splats[3 * (size_t)g]; r1 = splats[3 * (size_t)g + 1];
                 r2x = reinterpret_cast<const float*>(splats)[(size_t)g * kSplatWords + 8];
             }
-            // ---- walk the survivors ----
-            if (!done) {
-#pragma unroll 4
-                for (int e = 0; e < cnt; ++e) {
-                    const float4 a = sb.a[e];
-                    const float2 b = sb.b[e];
-                    const float dx = a.x - px, dy = a.y - py;
-                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
-                    if (!(power >= b.y && power <= 0.0f)) continue;  // alpha < 1/255 or power > 0
-                    const float4 c = sb.c[e];
-                    const float alpha = fminf(kAlphaMax, __fmul_rn(c.x, ex2_approx(power * kLog2e)));
-                    if (alpha < kAlphaMin) continue;  // the threshold test is exact up to rounding; keep the definition
-                    const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
-                    if (Tn < kTMin) {
-                        done = true;
-                        walked = sb.p[e];
-                        break;
-                    }
-                    const float w = alpha * T;
-                    C0 = fmaf(c.y, w, C0); C1 = fmaf(c.z, w, C1); C2 = fmaf(c.w, w, C2);
-                    T = Tn;
-                    last = sb.p[e];
-                    if (COUNT) ++blended;
-                }
+            if (j + 32 < ui.end) g_next = gid_sorted[j + 32];
+        }
+        for (uint32_t base = ui.start; base < ui.end; base += 32) {
+            // ---- stage: cull against the pixel box, compact survivors in range order ----
+            const bool have = base + lane < ui.end;
+            const float thr = blend_threshold(r1.y);
+            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, box);
+            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
+            const int cnt = __popc(ballot);
+            if (pass) {
+                const int slot = __popc(ballot & lt_mask);
+                sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
+                sb.b[slot] = make_float4(-0.5f * r1.x, thr, r1.y, __uint_as_float((base - ui.start) + lane + 1));
+                sb.c[slot] = make_float4(r1.z, r1.w, r2x, 0.f);
             }
-            if (__all_sync(0xffffffffu, done)) break;
+            __syncwarp();
+            // ---- prefetch ----
+            {
+                const uint32_t j = base + 32 + lane;
+                if (j < ui.end) {
+                    r0 = splats[3 * (size_t)g_next]; r1 = splats[3 * (size_t)g_next + 1];
+                    r2x = reinterpret_cast<const float*>(splats)[(size_t)g_next * kSplatWords + 8];
+                }
+                if (j + 32 < ui.end) g_next = gid_sorted[j + 32];
+            }
+            // ---- walk the survivors (branch free) ----
+#pragma unroll 4
+            for (int e = 0; e < cnt; ++e) {
+                const float4 a = sb.a[e];
+                const float4 b = sb.b[e];
+                const float4 c = sb.c[e];
+                const float dx = a.x - px, dy = a.y - py;
+                const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                const float alpha = fminf(kAlphaMax, __fmul_rn(b.z, ex2_approx(power * kLog2e)));
+                const bool blend = (power >= b.y) && (power <= 0.0f) && !(alpha < kAlphaMin);
+                const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
+                const bool term = blend && (Tn < kTMin);
+                const bool upd = blend && !term;
+                const float w = upd ? alpha * T : 0.0f;
+                C0 = fmaf(c.x, w, C0); C1 = fmaf(c.y, w, C1); C2 = fmaf(c.z, w, C2);
+                T = upd ? Tn : T;
+                last = upd ? __float_as_uint(b.w) : last;
+                if (COUNT) {
+                    blended += upd ? 1u : 0u;
+                    walked = term ? __float_as_uint(b.w) : walked;
+                }
+                px = term ? kNaN : px;
+            }
+            if (__all_sync(0xffffffffu, px != px)) break;
             __syncwarp();  // the batch slice is rewritten next iteration
         }
-        if (active) {
-            const uint32_t o = ui.pix0 + lane;
+        if (ui.active) {
+            const uint32_t o = ui.slot;
             out_color[3 * (size_t)o] = fmaf(T, cam.bg[0], C0);
             out_color[3 * (size_t)o + 1] = fmaf(T, cam.bg[1], C1);
             out_color[3 * (size_t)o + 2] = fmaf(T, cam.bg[2], C2);
@@ -130,15 +128,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         }
         __syncwarp();
     }
-    // the last warp to leave re-arms the scheduler for the next launch
-    if (lane == 0) {
-        const uint32_t total = gridDim.x * kRasterWarps;
-        if (atomicAdd(&sched[1], 1u) == total - 1u) {
-            sched[0] = 0u;
-            sched[1] = 0u;
-            __threadfence();
-        }
-    }
+    scheduler_leave(sched, lane);
 }
 
 }  // namespace
@@ -149,9 +139,8 @@ cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32
                               uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s) {
     if (k <= 0) return cudaSuccess;
     const bool count = n_walked || n_blended;
-    int per_sm = 4;
     // persistent grid: never more warps than units
-    int blocks = num_sms * per_sm;
+    int blocks = num_sms * 5;
     const int need = (k * 8 + kRasterWarps - 1) / kRasterWarps;
     if (blocks > need) blocks = need;
     const float4* sp = reinterpret_cast<const float4*>(splats);
