@@ -53,7 +53,7 @@ enum {
     TGS_ERR_INVALID_ARG = 1, /* NULL required pointer, non-positive size, bad fraction ...       */
     TGS_ERR_CAPACITY = 2,    /* a caller buffer / workspace is too small (message says how much) */
     TGS_ERR_CUDA = 3,        /* a CUDA runtime call or launch failed                             */
-    TGS_ERR_UNSUPPORTED = 4  /* sh_degree > 3, T > 2^20, P_capacity >= 2^32, ...                 */
+    TGS_ERR_UNSUPPORTED = 4  /* sh_degree > 3, T > 2^20, N or P_capacity >= 2^30, ...            */
 };
 
 enum { TGS_PIXELS_ALL = 0, TGS_PIXELS_BERNOULLI_ERR = 1 };

@@ -107,24 +107,21 @@ tile_reduce_kernel(const CamK cam, const float* __restrict__ err, const float* _
 }
 
 // rank by counting: tile t is selected iff fewer than k tiles precede it in the order
-// (score descending, tile id ascending).  O(T^2) compares spread over the whole GPU.
+// (score descending, tile id ascending).  One warp per tile, lanes stride over all T scores:
+// O(T^2) compares spread over the whole GPU, no sort needed for T of a few thousand.
 __global__ void __launch_bounds__(256)
 tile_select_kernel(int T, int k, const uint64_t* __restrict__ tile_score, uint32_t* __restrict__ selected) {
-    __shared__ uint64_t sc[1024];
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    const uint64_t mine = t < T ? tile_score[t] : 0;
+    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (t >= T) return;
+    const int lane = threadIdx.x & 31;
+    const uint64_t mine = tile_score[t];
     uint32_t rank = 0;
-    for (int b0 = 0; b0 < T; b0 += 1024) {
-        __syncthreads();
-        for (int j = threadIdx.x; j < 1024; j += blockDim.x) sc[j] = (b0 + j < T) ? tile_score[b0 + j] : 0;
-        __syncthreads();
-        const int lim = min(1024, T - b0);
-        for (int j = 0; j < lim; ++j) {
-            const uint64_t o = sc[j];
-            rank += (o > mine || (o == mine && (b0 + j) < t)) ? 1u : 0u;
-        }
+    for (int j = lane; j < T; j += 32) {
+        const uint64_t o = __ldg(tile_score + j);
+        rank += (o > mine || (o == mine && j < t)) ? 1u : 0u;
     }
-    if (t < T) selected[t] = rank < (uint32_t)k ? 1u : 0u;
+    rank = __reduce_add_sync(0xffffffffu, rank);
+    if (lane == 0) selected[t] = rank < (uint32_t)k ? 1u : 0u;
 }
 
 // single block: compaction of the selected tiles (ascending id) and exclusive prefix sum of their
@@ -219,7 +216,7 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
     TileMeta* meta = (TileMeta*)ws;
     uint32_t* selected = (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
     tile_reduce_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, err, render, target, mode, rnum, rden, seed, tile_score, meta);
-    tile_select_kernel<<<(T + 255) / 256, 256, 0, s>>>(T, k, tile_score, selected);
+    tile_select_kernel<<<(T + 7) / 8, 256, 0, s>>>(T, k, tile_score, selected);
     tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);
     write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);
     count_launches(4);

@@ -113,7 +113,8 @@ int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats
     if (!ctx) return TGS_ERR_INVALID_ARG;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: bad camera");
     if (N < 0 || P_capacity < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: negative size");
-    if (P_capacity >= (int64_t)0xffffffffll) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_bin_sort: P_capacity >= 2^32-1");
+    if (P_capacity >= (1ll << 30) || (int64_t)N >= (1ll << 30))
+        return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_bin_sort: N and P_capacity must be < 2^30");
     const int T = num_tiles(cam);
     if (T > (1 << 20)) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_bin_sort: T > 2^20");
     if (!gid_sorted || !tile_offsets || !P_dev || !workspace || (N > 0 && !splats))
