@@ -3,60 +3,51 @@
 //
 // Same decomposition as the forward (raster_common.cuh): persistent warps, one (tile, 32-pixel
 // group) unit at a time, the tile's range walked from the warp's deepest contributor backwards in
-// batches of 32 with the per-warp cull.  Per surviving Gaussian each lane forms nine partial sums
-// for its pixel -- three colour terms, dL/dopacity and the five moments dpow*(dx, dy, dx^2, dx dy,
-// dy^2) from which the mean2D / conic gradients follow linearly -- which are summed across the warp
-// with a butterfly (8 values in 9 shuffles + the 9th in 5) into the warp's shared-memory slice;
-// after the batch each lane turns ONE Gaussian's sums into its nine gradient components and issues
-// the global float atomics: 9 atomic instructions per 32 Gaussians instead of per Gaussian
-// (north_star: "warp-shuffle reduction of per-Gaussian gradients before global atomics").
+// batches of 32 with the per-warp cull.  The gradient of one Gaussian is a sum over pixels; summing
+// it with a shuffle tree per Gaussian costs more issue slots than the math itself (profiles/r1b),
+// so the warp TRANSPOSES instead:
+//   phase 1 (lane = pixel): per surviving Gaussian every lane replays its pixel and stores only the
+//            two per-(pixel, Gaussian) scalars everything else is linear in -- dpow = dL/dpower and
+//            w = alpha * T_k -- into a [16 Gaussians][32 pixels] shared-memory tile;
+//   phase 2 (lane = Gaussian): when 16 Gaussians are pending, lane e (and lane e + 16 for the other
+//            half of the pixels) sums Gaussian e's nine gradient components over the pixels in
+//            registers -- plain FMAs, no shuffles -- and issues the global float atomics.
+// So the per-Gaussian gradients are reduced over the warp's 32 pixels before any global atomic
+// (north_star), with 9 shuffles per 16 Gaussians instead of 14 per Gaussian.
 #include "raster_common.cuh"
 
 namespace tgs {
 
 namespace {
 
-struct WarpAcc {
-    float v[32][9];  // row stride 9 words: conflict-free when lane e reads row e
+__device__ __forceinline__ void red_add_v4(float4* p, float x, float y, float z, float w) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(x), "f"(y), "f"(z), "f"(w) : "memory");
+}
+
+constexpr int kSlots = 16;     // Gaussians per transposed tile
+constexpr int kTStride = 33;   // float2 row stride: conflict-free for both phases
+
+struct WarpXpose {
+    float2 v[kSlots * kTStride];  // [slot][pixel] = (dpow, w)
+    float4 ma[kSlots];            // mx, my, -A/2, -B
+    float4 mb[kSlots];            // -C/2, opacity, bits: Gaussian id, unused
+    float4 pa[32];                // per pixel: px, py, g0, g1
+    float pb[32];                 // per pixel: g2
 };
 
-// keep/send exchange of one butterfly step: lanes with `hi` keep b and send a, the others keep a
-__device__ __forceinline__ float bfly(float a, float b, bool hi, int mask) {
-    const float send = hi ? a : b;
-    const float keep = hi ? b : a;
-    return keep + __shfl_xor_sync(0xffffffffu, send, mask);
-}
-
-// Sums v[0..8] over the 32 lanes and stores the nine totals to row[0..8].
-__device__ __forceinline__ void warp_reduce9_store(const float (&v)[9], float* row, int lane) {
-    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
-    const float a0 = bfly(v[0], v[4], h16, 16), a1 = bfly(v[1], v[5], h16, 16);
-    const float a2 = bfly(v[2], v[6], h16, 16), a3 = bfly(v[3], v[7], h16, 16);
-    const float b0 = bfly(a0, a2, h8, 8), b1 = bfly(a1, a3, h8, 8);
-    float c0 = bfly(b0, b1, h4, 4);
-    c0 += __shfl_xor_sync(0xffffffffu, c0, 2);
-    c0 += __shfl_xor_sync(0xffffffffu, c0, 1);
-    float e = v[8];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
-    // lane L (L % 4 == 0) holds quantity 4*bit4 + 2*bit3 + bit2 = L >> 2
-    if ((lane & 3) == 0) row[lane >> 2] = c0;
-    if (lane == 1) row[8] = e;
-}
-
-__global__ void __launch_bounds__(kRasterThreads, 4)
+__global__ void __launch_bounds__(kRasterThreads, 3)
 raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
                   const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
                   const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
                   const float* __restrict__ out_T, const uint32_t* __restrict__ n_contrib,
                   const float* __restrict__ dL_dcolor, float* __restrict__ dL_dsplats, uint32_t* __restrict__ sched) {
-    __shared__ WarpBatch s_batch[kRasterWarps];
-    __shared__ WarpAcc s_acc[kRasterWarps];
+    extern __shared__ __align__(16) unsigned char smem_raw[];  // > 48 KB: dynamic, opted in by the launcher
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpBatch& sb = s_batch[warp];
-    WarpAcc& sa = s_acc[warp];
+    WarpBatch& sb = reinterpret_cast<WarpBatch*>(smem_raw)[warp];
+    WarpXpose& sx = reinterpret_cast<WarpXpose*>(smem_raw + kRasterWarps * sizeof(WarpBatch))[warp];
     const uint32_t num_units = (uint32_t)k * 8u;
     const uint32_t lt_mask = (1u << lane) - 1u;
+    const int slot2 = lane & (kSlots - 1), half = lane >> 4;  // phase-2 role of this lane
 
     for (;;) {
         uint32_t u = 0;
@@ -84,6 +75,8 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         const float px = (float)ipx, py = (float)ipy;
         const float bgdot = (cam.bg[0] * g0 + cam.bg[1] * g1 + cam.bg[2] * g2) * Tf;
         float T = Tf, S0 = 0.f, S1 = 0.f, S2 = 0.f;
+        sx.pa[lane] = make_float4(px, py, g0, g1);
+        sx.pb[lane] = g2;
 
         // lane l of a batch owns range position hi-1-l: survivors stay in descending position order
         float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
@@ -95,84 +88,123 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
             r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
         }
         if ((uint32_t)lane + 32 < wmax) g_next = gid_sorted[ui.start + wmax - 33 - lane];
-        for (uint32_t hi = wmax; hi > 0; hi = hi > 32 ? hi - 32 : 0) {
-            const bool have = (uint32_t)lane < hi;
-            const float thr = blend_threshold(r1.y);
-            const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, box);
-            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
-            const int cnt = __popc(ballot);
-            if (pass) {
-                const int slot = __popc(ballot & lt_mask);
-                sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
-                sb.b[slot] = make_float4(-0.5f * r1.x, thr, r1.y, __uint_as_float(hi - 1 - lane));
-                sb.c[slot] = make_float4(r1.z, r1.w, r2x, __uint_as_float(gcur));
-            }
-            __syncwarp();
-            if ((uint32_t)lane + 32 < hi) {
-                gcur = g_next;
-                r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
-                r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
-            }
-            if ((uint32_t)lane + 64 < hi) g_next = gid_sorted[ui.start + hi - 65 - lane];
 
-            uint32_t touched = 0;
+        uint32_t hi = wmax;  // entries [0, hi) of the range are still to be staged
+        int cnt = 0, e = 0;  // survivors staged in sb / next one to replay
+        int m = 0;           // Gaussians pending in the transposed tile
+        bool done = false;
+        while (!done) {
+            // ---- phase 1: replay survivors until kSlots Gaussians are pending or the range is exhausted ----
+            while (m < kSlots) {
+                if (e == cnt) {
+                    if (hi == 0) { done = true; break; }
+                    __syncwarp();
+                    // stage the next 32 range entries: cull against the pixel box, compact the survivors
+                    const bool have = (uint32_t)lane < hi;
+                    const float thr = blend_threshold(r1.y);
+                    const bool pass = have && splat_may_touch(r0.x, r0.y, r0.z, r0.w, r1.x, thr, box);
+                    const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
+                    cnt = __popc(ballot);
+                    e = 0;
+                    if (pass) {
+                        const int slot = __popc(ballot & lt_mask);
+                        sb.a[slot] = make_float4(r0.x, r0.y, -0.5f * r0.z, -r0.w);
+                        sb.b[slot] = make_float4(-0.5f * r1.x, thr, r1.y, __uint_as_float(hi - 1 - lane));
+                        sb.c[slot] = make_float4(r1.z, r1.w, r2x, __uint_as_float(gcur));
+                    }
+                    __syncwarp();
+                    if ((uint32_t)lane + 32 < hi) {
+                        gcur = g_next;
+                        r0 = splats[3 * (size_t)gcur]; r1 = splats[3 * (size_t)gcur + 1];
+                        r2x = reinterpret_cast<const float*>(splats)[(size_t)gcur * kSplatWords + 8];
+                    }
+                    if ((uint32_t)lane + 64 < hi) g_next = gid_sorted[ui.start + hi - 65 - lane];
+                    hi = hi > 32 ? hi - 32 : 0;
+                    continue;
+                }
+                // replay the next survivors (as many as fit in the transposed tile), branch free
+                const int take = min(cnt - e, kSlots - m);
+                const float4* sa = sb.a + e;
+                float2* vdst = sx.v + m * kTStride + lane;
+                float4* mdst = sx.ma + m;
 #pragma unroll 2
-            for (int e = 0; e < cnt; ++e) {
-                const float4 a = sb.a[e];
-                const float4 b = sb.b[e];
-                const float4 c = sb.c[e];
-                const float dx = a.x - px, dy = a.y - py;
-                const float power = splat_power(a.z, a.w, b.x, dx, dy);
-                // power is clamped for the exp only: G stays finite on lanes that fail the tests (no inf * 0)
-                const float G = ex2_approx(fminf(power, 0.0f) * kLog2e);
-                const float oG = __fmul_rn(b.z, G);
-                const float alpha = fminf(kAlphaMax, oG);
-                const bool valid = (__float_as_uint(b.w) < last) && (power >= b.y) && (power <= 0.0f) &&
-                                   !(alpha < kAlphaMin);
-                if (!__any_sync(0xffffffffu, valid)) continue;
-                touched |= 1u << e;
-                float v[9];
-                {
+                for (int i = 0; i < take; ++i) {
+                    const float4 a = sa[i];
+                    const float4 b = sa[32 + i];
+                    const float4 c = sa[64 + i];
+                    const float dx = a.x - px, dy = a.y - py;
+                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                    // power is clamped for the exp only: G stays finite on lanes that fail the tests (no inf * 0)
+                    const float G = ex2_approx(fminf(power, 0.0f) * kLog2e);
+                    const float oG = __fmul_rn(b.z, G);
+                    const float alpha = fminf(kAlphaMax, oG);
+                    const bool valid = (__float_as_uint(b.w) < last) && (power >= b.y) && (power <= 0.0f) &&
+                                       !(alpha < kAlphaMin);
                     const float om = 1.0f - alpha;
                     const float rom = rcp_approx(om);
                     const float Tk = T * rom;  // T_k
+                    const float dL_dalpha = ((c.x - S0) * g0 + (c.y - S1) * g1 + (c.z - S2) * g2) * Tk - bgdot * rom;
+                    // zero derivative through the active 0.99 clamp; invalid lanes contribute exact zeros
+                    const float dpow = (valid && oG < kAlphaMax) ? oG * dL_dalpha : 0.0f;  // dL/dpower
                     const float w = valid ? alpha * Tk : 0.0f;
-                    v[6] = w * g0; v[7] = w * g1; v[8] = w * g2;
-                    float dL_dalpha = ((c.x - S0) * g0 + (c.y - S1) * g1 + (c.z - S2) * g2) * Tk - bgdot * rom;
-                    dL_dalpha = valid ? dL_dalpha : 0.0f;
-                    if (valid) {
-                        T = Tk;
-                        S0 = fmaf(alpha, c.x, om * S0); S1 = fmaf(alpha, c.y, om * S1); S2 = fmaf(alpha, c.z, om * S2);
+                    T = valid ? Tk : T;
+                    S0 = valid ? fmaf(alpha, c.x, om * S0) : S0;
+                    S1 = valid ? fmaf(alpha, c.y, om * S1) : S1;
+                    S2 = valid ? fmaf(alpha, c.z, om * S2) : S2;
+                    vdst[i * kTStride] = make_float2(dpow, w);
+                    if (lane == 0) {  // predicated single-lane stores: one wavefront each
+                        mdst[i] = a;
+                        mdst[kSlots + i] = make_float4(b.x, b.z, c.w, 0.f);
                     }
-                    // zero derivative through the active 0.99 clamp
-                    const float dLa = (oG < kAlphaMax) ? dL_dalpha : 0.0f;
-                    v[5] = G * dLa;               // dL/dopacity
-                    const float dpow = oG * dLa;  // dL/dpower
-                    v[0] = dpow * dx; v[1] = dpow * dy;
-                    v[2] = v[0] * dx; v[3] = v[0] * dy; v[4] = v[1] * dy;
                 }
-                warp_reduce9_store(v, sa.v[e], lane);
+                e += take;
+                m += take;
             }
+            if (m == 0) break;
             __syncwarp();
-            // flush: lane e owns staged entry e; moments -> gradients
-            //   dL/dmx = sum dpow (-A dx - B dy),  dL/dA = -1/2 sum dpow dx^2,  dL/dB = -sum dpow dx dy, ...
-            if (lane < cnt && (touched >> lane) & 1u) {
-                const float4 a = sb.a[lane];
-                const float nC = sb.b[lane].x;
-                const float* m = sa.v[lane];
-                float* dst = dL_dsplats + (size_t)__float_as_uint(sb.c[lane].w) * kSplatWords;
-                atomicAdd(dst + 0, fmaf(2.0f * a.z, m[0], a.w * m[1]));
-                atomicAdd(dst + 1, fmaf(2.0f * nC, m[1], a.w * m[0]));
-                atomicAdd(dst + 2, -0.5f * m[2]);
-                atomicAdd(dst + 3, -m[3]);
-                atomicAdd(dst + 4, -0.5f * m[4]);
-                atomicAdd(dst + 5, m[5]);
-                atomicAdd(dst + 6, m[6]);
-                atomicAdd(dst + 7, m[7]);
-                atomicAdd(dst + 8, m[8]);
+            // ---- phase 2: lane = (Gaussian slot2, pixel half); nine sums over 16 pixels in registers ----
+            {
+                const float4 ga = sx.ma[slot2];
+                float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f, a4 = 0.f, a5 = 0.f, a6 = 0.f, a7 = 0.f, a8 = 0.f;
+                const float2* vrow = sx.v + slot2 * kTStride + half * 16;
+                const float4* prow = sx.pa + half * 16;
+                const float* qrow = sx.pb + half * 16;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) {
+                    const float2 v = vrow[i];
+                    const float4 q = prow[i];
+                    const float h2 = qrow[i];
+                    const float dx = ga.x - q.x, dy = ga.y - q.y;
+                    const float t0 = v.x * dx, t1 = v.x * dy;
+                    a0 += t0; a1 += t1;
+                    a2 = fmaf(t0, dx, a2); a3 = fmaf(t0, dy, a3); a4 = fmaf(t1, dy, a4);
+                    a5 += v.x;
+                    a6 = fmaf(v.y, q.z, a6); a7 = fmaf(v.y, q.w, a7); a8 = fmaf(v.y, h2, a8);
+                }
+                a0 += __shfl_xor_sync(0xffffffffu, a0, 16); a1 += __shfl_xor_sync(0xffffffffu, a1, 16);
+                a2 += __shfl_xor_sync(0xffffffffu, a2, 16); a3 += __shfl_xor_sync(0xffffffffu, a3, 16);
+                a4 += __shfl_xor_sync(0xffffffffu, a4, 16); a5 += __shfl_xor_sync(0xffffffffu, a5, 16);
+                a6 += __shfl_xor_sync(0xffffffffu, a6, 16); a7 += __shfl_xor_sync(0xffffffffu, a7, 16);
+                a8 += __shfl_xor_sync(0xffffffffu, a8, 16);
+                // moments -> gradients:  dL/dmx = sum dpow (-A dx - B dy),  dL/dA = -1/2 sum dpow dx^2, ...
+                // 16-byte vector reductions (red.global.add.v4.f32): 3 per Gaussian instead of 9 scalar ones
+                if (slot2 < m) {
+                    const float4 gb = sx.mb[slot2];
+                    float4* dst = reinterpret_cast<float4*>(dL_dsplats + (size_t)__float_as_uint(gb.z) * kSplatWords);
+                    const float dmx = fmaf(2.0f * ga.z, a0, ga.w * a1), dmy = fmaf(2.0f * gb.x, a1, ga.w * a0);
+                    const float dop = a5 / gb.y;  // dL/dopacity = sum G dL/dalpha = (sum dpow) / o
+                    if (half == 0) {
+                        red_add_v4(dst + 0, dmx, dmy, -0.5f * a2, -a3);
+                        red_add_v4(dst + 2, a8, 0.f, 0.f, 0.f);
+                    } else {
+                        red_add_v4(dst + 1, -0.5f * a4, dop, a6, a7);
+                    }
+                }
             }
+            m = 0;
             __syncwarp();
         }
+        __syncwarp();
     }
     scheduler_leave(sched, lane);
 }
@@ -186,10 +218,17 @@ cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const
     cudaError_t e = cudaMemsetAsync(dL_dsplats, 0, (size_t)N * kSplatWords * sizeof(float), s);
     if (e != cudaSuccess) return e;
     if (k <= 0) return cudaSuccess;
-    int blocks = num_sms * 4;
+    int blocks = num_sms * 3;
     const int need = (k * 8 + kRasterWarps - 1) / kRasterWarps;
     if (blocks > need) blocks = need;
-    raster_bwd_kernel<<<blocks, kRasterThreads, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
+    constexpr size_t smem = kRasterWarps * (sizeof(WarpBatch) + sizeof(WarpXpose));
+    static bool opted_in = false;  // attribute of the function, set once per process
+    if (!opted_in) {
+        e = cudaFuncSetAttribute(raster_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        opted_in = true;
+    }
+    raster_bwd_kernel<<<blocks, kRasterThreads, smem, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                         gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
                                                         dL_dsplats, sched);
     count_launches(1);
