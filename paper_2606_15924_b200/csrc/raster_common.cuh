@@ -1,14 +1,26 @@
-// Shared pieces of the two raster kernels: the per-warp staged Gaussian batch, the conservative
-// warp-level cull and the work-unit decoding.
+// Shared pieces of the two raster kernels: work decomposition, the producer warp that stages a
+// sampled tile's depth-ordered Gaussians through a shared-memory ring, the conservative per-warp
+// cull and the unit decoding.
 //
-// Work decomposition (both kernels): a WORK UNIT is one group of 32 sampled pixels of one sampled
-// tile (PAPER.md:156 -- pixels are listed tile by tile).  Warps are persistent and pull units from
-// a global atomic counter, so a tile with a long Gaussian range does not pin a whole block, and a
-// launch with few sampled tiles still spreads over all SMs.  Each warp walks its tile's
-// depth-ordered range in batches of 32: every lane loads one Gaussian record (float4 loads, ids
-// prefetched two batches ahead, records one batch ahead), tests it against the bounding box of the
-// warp's 32 pixels, and the survivors are compacted into the warp's shared-memory slice in range
-// order; the inner loop then runs over survivors only.
+// Work decomposition (both kernels).  A thread block is persistent and handles one SAMPLED TILE at
+// a time (sampled pixels are listed tile by tile; tile-parallel execution).  It has
+// one PRODUCER warp and eight CONSUMER warps:
+//   * consumer w owns unit w of the tile = 32 sampled pixels (an 8x4 block of a full tile, or 32
+//     consecutive entries of a partial tile's pixel list), so warps stay full on a sparse pixel set;
+//   * the producer pulls tiles from a global atomic counter, walks the tile's range in gid_sorted
+//     and gathers each Gaussian's 48-byte splat record ONCE per tile into a ring of shared-memory
+//     stages (kStages x 64..128 records), pre-scaled for the inner loops.  Full / empty
+//     mbarriers per stage decouple it from the consumers, and the consumers from each other, by up
+//     to kStages stages; it runs ahead into the next tile while the consumers finish the current one.
+//     (profiles/r1b: with every warp gathering its own records the L1 LSU data pipe was ~70-80 %
+//     busy, mostly on 32-line gathers repeated by the 8 warps of a tile, and was the limiter.)
+//   * each consumer reads a stage 32 records at a time (conflict-free float4 planes), tests them
+//     against the bounding box of ITS 32 pixels, compacts the survivors into its private slice in
+//     range order and runs its inner loop over survivors only.
+//   * the stream of stages carries the control flow: a stage's header names the sampled tile it
+//     starts (or "continuation" / "end of work"), so only the producer talks to the scheduler.
+//   * forward early termination: a consumer whose pixels are all saturated publishes the tile's
+//     sequence number; the producer stops a tile's stream as soon as all eight have.
 //
 // The cull is conservative: it only drops a Gaussian when NO point of the box can reach
 // alpha >= 1/255 (so the result is identical to walking the full range).
@@ -17,15 +29,41 @@
 
 namespace tgs {
 
-constexpr int kRasterWarps = 8;                 // warps per block
-constexpr int kRasterThreads = kRasterWarps * 32;
+constexpr int kConsumers = 8;                        // consumer warps per block = units per tile
+constexpr int kRasterThreads = (kConsumers + 1) * 32;  // + 1 producer warp
+constexpr int kStages = 4;
+constexpr uint32_t kHdrCont = 0xfffffffeu, kHdrEnd = 0xffffffffu;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kLnAlphaMin = -5.541263545158426f;  // ln(1/255)
 
+// one staged record, as three float4 planes per stage:
+//   p0 = mx, my, -A/2, -B     p1 = -C/2, thr = ln(1/(255 o)) - 1e-5, opacity, red     p2 = green, blue, bits: Gaussian id, 0
+template <int ENTRIES>
+struct Stage {
+    float4 p0[ENTRIES];
+    float4 p1[ENTRIES];
+    float4 p2[ENTRIES];
+};
+struct StageInfo {
+    uint32_t cnt;   // valid records in this stage
+    uint32_t hdr;   // index into tiles[] of the sampled tile this stage STARTS, kHdrCont, or kHdrEnd
+    uint32_t base;  // range position (0-based) of record 0; forward ascending, backward descending
+    uint32_t pad;
+};
+template <int ENTRIES>
+struct Ring {
+    static constexpr int kEntries = ENTRIES;
+    Stage<ENTRIES> st[kStages];
+    unsigned long long full[kStages], empty[kStages];
+    StageInfo info[kStages];
+    uint32_t done_seq[kConsumers];  // consumer w needs nothing more of the block's done_seq[w]-th tile
+};
+
+// a consumer's private survivors of one 32-record batch
 struct WarpBatch {
     float4 a[32];  // mx, my, -A/2, -B
-    float4 b[32];  // -C/2, thr = ln(1/(255 o)) - 1e-5, opacity, bits: 1-based range position (fwd) / 0-based (bwd)
+    float4 b[32];  // -C/2, thr, opacity, bits: range position (fwd: 1-based, bwd: 0-based)
     float4 c[32];  // r, g, b, bits: Gaussian id
 };
 
@@ -45,6 +83,28 @@ __device__ __forceinline__ float rcp_approx(float x) {
     return y;
 }
 
+// ---- mbarrier (shared::cta) ------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {  // release.cta
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t parity) {  // acquire.cta
+    const uint32_t a = smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n\t.reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t}"
+            : "=r"(ok)
+            : "r"(a), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+
 // Canonical power: fma(fma(-B, dy, (-A/2) dx), dx, ((-C/2) dy) dy)
 __device__ __forceinline__ float splat_power(float nA, float nB, float nC, float dx, float dy) {
     return __fmaf_rn(__fmaf_rn(nB, dy, __fmul_rn(nA, dx)), dx, __fmul_rn(__fmul_rn(nC, dy), dy));
@@ -59,20 +119,21 @@ __device__ __forceinline__ float blend_threshold(float opacity) {
 struct PixelBox { float x0, y0, x1, y1; };
 
 // Conservative test: can the splat reach alpha >= 1/255 anywhere in the pixel box?
-// q(d) = A dx^2 + 2 B dx dy + C dy^2 is minimised over the box exactly (the minimum of a convex
-// quadratic over a box that does not contain its centre lies on an edge facing the centre: two 1-D
-// minimisations with clamping); the splat may touch iff q_min <= 2 |thr|.  Slack 0.1 % + 1e-3.
-__device__ __forceinline__ bool splat_may_touch(float mx, float my, float A, float B, float C, float thr,
+// power(d) = nA dx^2 + nB dx dy + nC dy^2 (nA = -A/2, nB = -B, nC = -C/2) is maximised over the box
+// exactly (the maximum of a concave quadratic over a box that does not contain its centre lies on
+// an edge facing the centre: two 1-D maximisations with clamping); the splat may touch iff
+// power_max >= thr.  Slack 0.1 % + 5e-4.
+__device__ __forceinline__ bool splat_may_touch(float mx, float my, float nA, float nB, float nC, float thr,
                                                 const PixelBox& bx) {
     if (thr > 0.0f) return false;  // opacity < 1/255: never blends
     const float X0 = bx.x0 - mx, X1 = bx.x1 - mx, Y0 = bx.y0 - my, Y1 = bx.y1 - my;
     const float dxc = fminf(fmaxf(0.0f, X0), X1), dyc = fminf(fmaxf(0.0f, Y0), Y1);
-    const float xs = fminf(fmaxf(-B * dyc * rcp_approx(A), X0), X1);
-    const float ys = fminf(fmaxf(-B * dxc * rcp_approx(C), Y0), Y1);
-    const float q1 = A * xs * xs + 2.0f * B * xs * dyc + C * dyc * dyc;
-    const float q2 = A * dxc * dxc + 2.0f * B * dxc * ys + C * ys * ys;
-    const float lim = -2.002f * thr + 1e-3f;
-    return !(fminf(q1, q2) > lim);  // NaN anywhere keeps the Gaussian
+    const float xs = fminf(fmaxf(-0.5f * nB * dyc * rcp_approx(nA), X0), X1);
+    const float ys = fminf(fmaxf(-0.5f * nB * dxc * rcp_approx(nC), Y0), Y1);
+    const float h1 = nA * xs * xs + nB * xs * dyc + nC * dyc * dyc;
+    const float h2 = nA * dxc * dxc + nB * dxc * ys + nC * ys * ys;
+    const float lim = 1.001f * thr - 5e-4f;
+    return !(fmaxf(h1, h2) < lim);  // NaN anywhere keeps the Gaussian
 }
 
 struct UnitInfo {
@@ -81,12 +142,11 @@ struct UnitInfo {
     bool active;
 };
 
-// unit u -> (sampled tile u/8, pixel group u%8).  A full tile (256 pixels) is cut into 8x4-pixel
-// blocks (compact boxes cull better); a partial tile into runs of 32 consecutive list entries.
-__device__ __forceinline__ bool decode_unit(uint32_t u, int lane, const uint32_t* __restrict__ tiles,
+// (sampled tile `it`, pixel group `gi`).  A full tile (256 pixels) is cut into 8x4-pixel blocks
+// (compact boxes cull better); a partial tile into runs of 32 consecutive list entries.
+__device__ __forceinline__ bool decode_unit(uint32_t it, uint32_t gi, int lane, const uint32_t* __restrict__ tiles,
                                             const uint32_t* __restrict__ tile_offsets,
                                             const uint32_t* __restrict__ tpo, UnitInfo& ui) {
-    const uint32_t it = u >> 3, gi = u & 7u;
     const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
     if (gi * 32u >= m) return false;
     const uint32_t t = tiles[it];
@@ -113,11 +173,111 @@ __device__ __forceinline__ PixelBox warp_pixel_box(bool active, int ipx, int ipy
     return b;
 }
 
-// the last warp to leave re-arms the scheduler counters for the next launch
-__device__ __forceinline__ void scheduler_leave(uint32_t* sched, int lane) {
+template <class RingT>
+__device__ __forceinline__ void ring_init(RingT& R) {
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kStages; ++s) {
+            mbar_init(&R.full[s], 1u);
+            mbar_init(&R.empty[s], (uint32_t)kConsumers);
+        }
+        for (int w = 0; w < kConsumers; ++w) R.done_seq[w] = 0u;
+    }
+    __syncthreads();
+}
+
+// The producer warp.  BWD = false: ranges front to back, stops a tile early once every consumer is
+// saturated.  BWD = true: from the tile's deepest contributor (max n_contrib) back to front.
+template <bool BWD, class RingT>
+__device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict__ splats,
+                                              const uint32_t* __restrict__ tile_offsets,
+                                              const uint32_t* __restrict__ gid_sorted, uint32_t k,
+                                              const uint32_t* __restrict__ tiles, const uint32_t* __restrict__ tpo,
+                                              const uint32_t* __restrict__ n_contrib, uint32_t* __restrict__ sched,
+                                              int lane) {
+    uint32_t gchunk = 0, seq = 0;
+    for (;;) {
+        uint32_t it = 0;
+        if (lane == 0) it = atomicAdd(&sched[0], 1u);
+        it = __shfl_sync(0xffffffffu, it, 0);
+        if (it >= k) break;
+        ++seq;
+        const uint32_t t = tiles[it];
+        const uint32_t start = tile_offsets[t];
+        uint32_t len = tile_offsets[t + 1] - start;
+        if (BWD) {
+            const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
+            uint32_t mx = 0;
+            for (uint32_t i = lane; i < m; i += 32) mx = max(mx, n_contrib[p0 + i]);
+            len = __reduce_max_sync(0xffffffffu, mx);
+        }
+        uint32_t produced = 0;
+        bool first = true;
+        do {
+            if (!BWD && !first) {
+                const uint32_t d = lane < kConsumers ? *(volatile uint32_t*)&R.done_seq[lane] : seq;
+                if (__all_sync(0xffffffffu, d >= seq)) break;
+            }
+            const uint32_t s = gchunk % kStages;
+            mbar_wait(&R.empty[s], ((gchunk / kStages) & 1u) ^ 1u);
+            constexpr int kStageEntries = RingT::kEntries;
+            const uint32_t cnt = min((uint32_t)kStageEntries, len - produced);
+            auto& st = R.st[s];
+            // two batches of 32 records at a time: six independent gathers in flight per lane
+#pragma unroll 1
+            for (int h = 0; h < kStageEntries / 64; ++h) {
+                if ((uint32_t)h * 64u >= cnt) break;
+                uint32_t g[2];
+                float4 r0[2], r1[2];
+                float r2x[2];
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const uint32_t i = h * 64 + j * 32 + lane;
+                    const uint32_t pos = BWD ? (len - 1u - produced - i) : (produced + i);
+                    g[j] = i < cnt ? gid_sorted[start + pos] : 0xffffffffu;
+                }
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    if (g[j] != 0xffffffffu) {
+                        r0[j] = splats[3 * (size_t)g[j]];
+                        r1[j] = splats[3 * (size_t)g[j] + 1];
+                        r2x[j] = reinterpret_cast<const float*>(splats)[(size_t)g[j] * kSplatWords + 8];
+                    }
+                }
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    if (g[j] != 0xffffffffu) {
+                        const int i = h * 64 + j * 32 + lane;
+                        st.p0[i] = make_float4(r0[j].x, r0[j].y, -0.5f * r0[j].z, -r0[j].w);
+                        st.p1[i] = make_float4(-0.5f * r1[j].x, blend_threshold(r1[j].y), r1[j].y, r1[j].z);
+                        st.p2[i] = make_float4(r1[j].w, r2x[j], __uint_as_float(g[j]), 0.f);
+                    }
+                }
+            }
+            if (lane == 0) {
+                StageInfo inf;
+                inf.cnt = cnt;
+                inf.hdr = first ? it : kHdrCont;
+                inf.base = BWD ? (len - 1u - produced) : produced;
+                inf.pad = 0;
+                R.info[s] = inf;
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&R.full[s]);
+            ++gchunk;
+            produced += cnt;
+            first = false;
+        } while (produced < len);
+    }
+    // end of work
+    const uint32_t s = gchunk % kStages;
+    mbar_wait(&R.empty[s], ((gchunk / kStages) & 1u) ^ 1u);
     if (lane == 0) {
-        const uint32_t total = gridDim.x * kRasterWarps;
-        if (atomicAdd(&sched[1], 1u) == total - 1u) {
+        StageInfo inf;
+        inf.cnt = 0; inf.hdr = kHdrEnd; inf.base = 0; inf.pad = 0;
+        R.info[s] = inf;
+        mbar_arrive(&R.full[s]);
+        // the last producer to leave re-arms the scheduler counters for the next launch
+        if (atomicAdd(&sched[1], 1u) == gridDim.x - 1u) {
             sched[0] = 0u;
             sched[1] = 0u;
             __threadfence();
