@@ -2,6 +2,10 @@
 // Gaussian through the EWA projection and the SH colour to dL/d(mean3D, scale, quaternion,
 // opacity, SH) ("This pipeline is differentiable", 441).
 // One thread per Gaussian, no atomics; HBM-bound (reads 236 + 48 B, writes 236 B at degree 3).
+// The SH block (192 B in, 192 B out per Gaussian -- three quarters of the traffic) moves through
+// shared memory: the block's 128 x K x 3 coefficients are one contiguous span in HBM, copied with
+// coalesced float4 accesses into rows of odd stride (conflict-free for one-row-per-thread access),
+// overwritten in place by dL/dsh and copied back the same way.
 #include "common.cuh"
 
 namespace tgs {
@@ -61,18 +65,39 @@ __device__ __forceinline__ void sh_basis_and_grad(float x, float y, float z, flo
     }
 }
 
+constexpr int kPBThreads = 128;
+
 template <int D>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(kPBThreads)
 project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const float* __restrict__ sc,
                    const float* __restrict__ qt, const float* __restrict__ sh, const int32_t* __restrict__ radii,
                    const uint8_t* __restrict__ clamped, const float4* __restrict__ dsp,
                    float* __restrict__ dmu, float* __restrict__ dsc, float* __restrict__ dqt,
                    float* __restrict__ dop, float* __restrict__ dsh) {
     constexpr int K = (D + 1) * (D + 1);
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+    constexpr int KC = K * 3;                       // floats per Gaussian
+    constexpr int STRIDE = (KC % 2) ? KC : KC + 1;  // odd row stride: lane i -> bank (STRIDE * i + j) % 32, all distinct
+    __shared__ float s_sh[kPBThreads * STRIDE];
+    const int base = blockIdx.x * kPBThreads;
+    const int nvalid = min(kPBThreads, N - base);
+    {   // coalesced copy in: float4 body (the span starts 16-byte aligned), scalar tail
+        const int total = nvalid * KC;
+        const float* src = sh + (size_t)base * KC;
+        const float4* src4 = reinterpret_cast<const float4*>(src);
+        for (int v = threadIdx.x; v < total / 4; v += kPBThreads) {
+            const float4 f = __ldg(src4 + v);
+            const int e = 4 * v;
+            const float vals[4] = {f.x, f.y, f.z, f.w};
+#pragma unroll
+            for (int c = 0; c < 4; ++c) s_sh[((e + c) / KC) * STRIDE + (e + c) % KC] = vals[c];
+        }
+        for (int e = (total / 4) * 4 + threadIdx.x; e < total; e += kPBThreads) s_sh[(e / KC) * STRIDE + e % KC] = __ldg(src + e);
+    }
+    __syncthreads();
+    const int i = base + threadIdx.x;
+    if (i < N) {
     float gmu[3] = {0.f, 0.f, 0.f}, gs[3] = {0.f, 0.f, 0.f}, gq[4] = {0.f, 0.f, 0.f, 0.f}, gop = 0.f;
-    float* gsh = dsh + (size_t)i * (K * 3);
+    float* gsh = s_sh + threadIdx.x * STRIDE;  // SH in, dL/dsh out (in place)
     bool live = radii[i] > 0;
     const float* W = cam.R;
     float m0 = 0.f, m1 = 0.f, m2 = 0.f, t0 = 0.f, t1 = 0.f, tz = 1.f;
@@ -205,12 +230,11 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
 #pragma unroll
         for (int ch = 0; ch < 3; ++ch) gch[ch] = (cl & (1u << ch)) ? 0.f : grgb[ch];
         float dd[3] = {0.f, 0.f, 0.f};
-        const float* s_i = sh + (size_t)i * (K * 3);
 #pragma unroll
         for (int k = 0; k < K; ++k) {
 #pragma unroll
             for (int ch = 0; ch < 3; ++ch) {
-                const float sv = __ldg(s_i + 3 * k + ch) * gch[ch];
+                const float sv = gsh[3 * k + ch] * gch[ch];
                 gsh[3 * k + ch] = Bk[k] * gch[ch];
                 dd[0] = fmaf(dB[k][0], sv, dd[0]); dd[1] = fmaf(dB[k][1], sv, dd[1]); dd[2] = fmaf(dB[k][2], sv, dd[2]);
             }
@@ -223,6 +247,21 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
     dsc[3 * i] = gs[0]; dsc[3 * i + 1] = gs[1]; dsc[3 * i + 2] = gs[2];
     reinterpret_cast<float4*>(dqt)[i] = make_float4(gq[0], gq[1], gq[2], gq[3]);
     dop[i] = gop;
+    }
+    __syncthreads();
+    {   // coalesced copy out
+        const int total = nvalid * KC;
+        float* dst = dsh + (size_t)base * KC;
+        float4* dst4 = reinterpret_cast<float4*>(dst);
+        for (int v = threadIdx.x; v < total / 4; v += kPBThreads) {
+            const int e = 4 * v;
+            float vals[4];
+#pragma unroll
+            for (int c = 0; c < 4; ++c) vals[c] = s_sh[((e + c) / KC) * STRIDE + (e + c) % KC];
+            dst4[v] = make_float4(vals[0], vals[1], vals[2], vals[3]);
+        }
+        for (int e = (total / 4) * 4 + threadIdx.x; e < total; e += kPBThreads) dst[e] = s_sh[(e / KC) * STRIDE + e % KC];
+    }
 }
 
 }  // namespace
@@ -231,7 +270,7 @@ cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, c
                                const float* sh, const int32_t* radii, const uint8_t* clamped,
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
                                float* dsh, cudaStream_t s) {
-    const int threads = 128, blocks = (N + threads - 1) / threads;
+    const int threads = kPBThreads, blocks = (N + threads - 1) / threads;
     const float4* dsp = reinterpret_cast<const float4*>(dL_dsplats);
 #define TGS_PB(DD) project_bwd_kernel<DD><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, sh, radii, clamped, dsp, dmu, dsc, dqt, dop, dsh)
     switch (D) {
