@@ -104,11 +104,11 @@ def time_oracle(scene, steps, warmup):
     g = None
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        r = o.pipeline(scene, dL_dcolor=g, backward=g is not None)
+        r = o.pipeline(scene, dL_dcolor=g, backward=g is not None, restrict=True)
         if g is None:  # first pass only sizes the upstream gradient (outside the timing)
             g = workloads.dl_dcolor(0, r.samp.n)
             t0 = time.perf_counter()
-            r = o.pipeline(scene, dL_dcolor=g, backward=True)
+            r = o.pipeline(scene, dL_dcolor=g, backward=True, restrict=True)
         dt = time.perf_counter() - t0
         n = r.samp.n
         if i >= warmup:
@@ -141,7 +141,7 @@ def run_reference(args):
 def workload_config(scene, args, P, k, n):
     return {"workload": f"BASELINE.json configs[{args.config - 1}] ({scene.name})", "gaussians": scene.N,
             "sh_degree": scene.sh_degree, "image": [scene.cam.width, scene.cam.height],
-            "tiles": scene.cam.num_tiles, "tile_pct": list(scene.tile_pct),
+            "tiles": scene.cam.num_tiles, "tile_pct": list(scene.tile_pct), "binning": "sampled tiles only (tile_select)",
             "pixel_mode": "all" if scene.pixel_mode == 0 else "bernoulli_err", "pairs_P": int(P),
             "sampled_tiles_k": int(k), "sampled_pixels_n": int(n), "parallelism": f"replicas x{args.gpus}"}
 
@@ -240,7 +240,7 @@ def run_tgs(args):
     value = n_total * args.steps / (total_ms * 1e-3)
 
     # ---- per-call breakdown (separate pass; events between the calls) ----
-    names = ["preprocess", "bin_sort", "sample", "raster_fwd", "raster_bwd", "project_bwd"]
+    names = ["preprocess", "sample", "bin_sort", "raster_fwd", "raster_bwd", "project_bwd"]
     acc = {k_: 0.0 for k_ in names}
     tgs_, st = tg, step
     for _ in range(args.steps):
@@ -249,10 +249,11 @@ def run_tgs(args):
         e_[0].record()
         tgs_.preprocess(cam, scene.sh_degree, D["means3D"], D["scales"], D["quats"], D["opacities"], D["sh"], out=st.pre)
         e_[1].record()
-        tgs_.bin_sort(cam, st.pre.splats, st.P_capacity, out=st.binned, workspace=st.ws_sort, sync=False)
-        e_[2].record()
         tgs_.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed, err=D["err"], out=st.samp,
                     workspace=st.ws_sample, sync=False)
+        e_[2].record()
+        tgs_.bin_sort(cam, st.pre.splats, st.P_capacity, out=st.binned, workspace=st.ws_sort, sync=False,
+                      tile_select=st.samp.tile_select)
         e_[3].record()
         tgs_.raster_fwd_sparse(cam, st.pre.splats, st.binned, st.samp, out=st.fwd)
         e_[4].record()
@@ -275,7 +276,8 @@ def run_tgs(args):
     bwd_flops = BWD_FLOPS_WALK * replayed + BWD_FLOPS_BLEND * blended
     K = (scene.sh_degree + 1) ** 2
     hbm_bytes = {"preprocess": scene.N * (4 * (11 + 3 * K) + 48 + 5), "project_bwd": scene.N * (4 * (10 + 3 * K) + 48 + 5 + 4 * (11 + 3 * K)),
-                 "bin_sort": scene.N * (12 + 4 * 16 + 8 + 8 + 16) + P * (8 + 2 * 16 + 8)}
+                 # rect/depth words of every record, then per emitted pair: segment write + read, gid_sorted write
+                 "bin_sort": scene.N * 16 + P * (8 + 8 + 4) + cam.num_tiles * 12}
     kernels = {
         "raster_fwd": {"bound": "alu", "achieved": fwd_flops / (per_call_ms["raster_fwd"] * 1e-3) / 1e12,
                        "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"},

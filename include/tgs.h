@@ -92,14 +92,19 @@ int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree,
  * Produces the list of all (tile, Gaussian) pairs ordered by (tile_id, depth bits, Gaussian id):
  *   gid_sorted[P], tile_offsets[T+1] (CSR: tile t owns [tile_offsets[t], tile_offsets[t+1])),
  *   keys_sorted[P] = tile_id<<32 | float_bits(depth)   (optional, may be NULL).
- * P = sum of tiles touched is data dependent: P_dev[0] = P, P_dev[1] = 1 if P > P_capacity (then
+ * tile_select[T] (nullable; as written by tgs_sample): when given, only pairs whose tile has
+ * tile_select[t] != 0 are emitted; every other tile gets an empty range (the method never reads
+ * the ranges of tiles it does not sample; R14).  NULL bins every tile.
+ * P = number of emitted pairs is data dependent: P_dev[0] = P, P_dev[1] = 1 if P > P_capacity (then
  * the lists are invalid and, if P_host != NULL, the call returns TGS_ERR_CAPACITY).  P_host (host,
  * nullable) receives P and forces one stream synchronisation.
- * The sort is a hand-written stable LSD radix sort; because the low 32 key bits (depth) depend on
- * the Gaussian only, those digit passes run on the N Gaussians BEFORE duplication and only the
- * tile-id digits run on the P pairs (same result as sorting the 64-bit keys). */
+ * The sort is a hand-written radix sort: a counting sort on the tile id (most significant digit)
+ * followed by an LSD radix sort of every tile's segment in shared memory over the varying depth
+ * bits, ties by Gaussian id.  workspace: tgs_bin_sort_workspace_bytes (16 B per pair + 12 B per
+ * tile), contents undefined on return. */
 int tgs_bin_sort_workspace_bytes(int N, int64_t P_capacity, int num_tiles, size_t* bytes);
 int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                 const uint32_t* tile_select,
                  int64_t P_capacity, uint64_t* keys_sorted, uint32_t* gid_sorted,
                  uint32_t* tile_offsets, int64_t* P_dev, int64_t* P_host,
                  void* workspace, size_t workspace_bytes, void* stream);
@@ -111,7 +116,9 @@ int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats
  * ascending in tiles[k]; per selected tile the pixel list (ALL in-image pixels, or
  * BERNOULLI_ERR: keep iff u16(p)*S*den < num*cnt*q16(p)*2^16, at least one pixel per tile), in
  * ascending local index, concatenated in pix[n]; tile_pix_offsets[k+1] is its CSR.
- * Capacities: tile_score[T], tiles[T], tile_pix_offsets[T+1], pix[W*H].  kn_dev[0]=k, kn_dev[1]=n. */
+ * Capacities: tile_score[T], tiles[T], tile_pix_offsets[T+1], pix[W*H].  kn_dev[0]=k, kn_dev[1]=n.
+ * tile_select[T] (nullable output): 1 for a selected tile, 0 otherwise -- the mask tgs_bin_sort
+ * takes to restrict binning to the sampled tiles. */
 int tgs_sample_num_tiles(const tgs_camera* cam, int tile_pct_num, int tile_pct_den);
 int tgs_sample_workspace_bytes(const tgs_camera* cam, size_t* bytes);
 int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam,
@@ -119,7 +126,7 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam,
                int tile_pct_num, int tile_pct_den, int pixel_mode,
                int pix_rate_num, int pix_rate_den, uint64_t seed,
                uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
-               int32_t* kn_dev, int32_t* kn_host,
+               uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host,
                void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- a4: sparse forward (Eq. 1, 154-166) ---------------------------------------

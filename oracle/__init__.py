@@ -111,18 +111,21 @@ class Oracle:
         return o
 
     # ---- O2 ------------------------------------------------------------------------------
-    def bin_sort(self, cam, pre):
+    def bin_sort(self, cam, pre, tile_select=None):
+        """tile_select: optional [T] mask (nonzero = bin this tile); None bins every tile."""
         N = pre.depths.shape[0]
         gx, gy = self.grid(cam)
-        P = int(pre.tiles_touched.astype(np.int64).sum())
-        keys = np.zeros(max(P, 1), np.uint64)
-        gid = np.zeros(max(P, 1), np.uint32)
+        cap = int(pre.tiles_touched.astype(np.int64).sum())
+        keys = np.zeros(max(cap, 1), np.uint64)
+        gid = np.zeros(max(cap, 1), np.uint32)
         offs = np.zeros(gx * gy + 1, np.uint32)
+        sel = None if tile_select is None else np.ascontiguousarray(tile_select, dtype=np.uint32)
+        assert sel is None or sel.shape == (gx * gy,)
         c = self.cam(cam)
-        P2 = self.lib.orc_bin_sort(C.byref(c), N, _ptr(self.r(pre.depths)), _ptr(pre.rect),
-                                   _ptr(pre.tiles_touched), _ptr(keys), _ptr(gid), _ptr(offs))
-        assert P2 == P
-        return SimpleNamespace(P=P, keys_sorted=keys[:P], gid_sorted=gid[:P], tile_offsets=offs)
+        P = int(self.lib.orc_bin_sort(C.byref(c), N, _ptr(self.r(pre.depths)), _ptr(pre.rect),
+                                      _ptr(pre.tiles_touched), _ptr(sel), _ptr(keys), _ptr(gid), _ptr(offs)))
+        assert P <= cap and (sel is not None or P == cap)
+        return SimpleNamespace(P=P, keys_sorted=keys[:P].copy(), gid_sorted=gid[:P].copy(), tile_offsets=offs)
 
     # ---- O3 ------------------------------------------------------------------------------
     def sample(self, cam, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, err=None, render=None, target=None):
@@ -218,19 +221,29 @@ class Oracle:
         return int(self.lib.orc_mix64(seed, idx))
 
     # ---- whole path --------------------------------------------------------------------------
-    def pipeline(self, scene, dL_dcolor=None, backward=True):
-        """preprocess -> bin_sort -> sample -> fwd -> (bwd) on a ``workloads.Scene``."""
+    def pipeline(self, scene, dL_dcolor=None, backward=True, restrict=False):
+        """preprocess -> bin_sort -> sample -> fwd -> (bwd) on a ``workloads.Scene``.  restrict=True
+        (needs an error map): sample first, then bin only the selected tiles (R14)."""
         cam = scene.cam
         pre = self.preprocess(cam, scene.sh_degree, scene.means3D, scene.scales, scene.quats,
                               scene.opacities, scene.sh)
-        binned = self.bin_sort(cam, pre)
-        if scene.err is not None:
+        if restrict and scene.err is not None:
             samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
                                err=scene.err)
+            gx, gy = self.grid(cam)
+            sel = np.zeros(gx * gy, np.uint32)
+            sel[samp.tiles] = 1
+            samp.tile_select = sel
+            binned = self.bin_sort(cam, pre, tile_select=sel)
         else:
-            render = self.render_dense(cam, binned, pre)
-            samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
-                               render=render, target=scene.target)
+            binned = self.bin_sort(cam, pre)
+            if scene.err is not None:
+                samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
+                                   err=scene.err)
+            else:
+                render = self.render_dense(cam, binned, pre)
+                samp = self.sample(cam, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed,
+                                   render=render, target=scene.target)
         fwd = self.raster_fwd(cam, binned, pre, samp)
         out = SimpleNamespace(pre=pre, binned=binned, samp=samp, fwd=fwd, rbwd=None, pbwd=None)
         if backward:

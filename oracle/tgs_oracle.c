@@ -303,23 +303,29 @@ static int pair_cmp(const void* a, const void* b) {
 }
 static uint32_t depth_bits(real z) { float f = (float)z; uint32_t u; memcpy(&u, &f, 4); return u; }
 
-/* keys/gid have room for P = sum(touched); tile_offsets has T+1 entries. Returns P. */
+/* keys/gid have room for sum(touched) pairs; tile_offsets has T+1 entries. Returns P, the number
+ * of pairs emitted.  tile_select (nullable, [T]): when given, only pairs whose tile has
+ * tile_select[t] != 0 are emitted and every other tile gets an empty range -- the sparse step
+ * never reads the ranges of tiles it does not sample (reading R14). */
 int64_t orc_bin_sort(const orc_cam* cam, int N, const real* depth, const int32_t* rect,
-                     const uint32_t* touched, uint64_t* keys, uint32_t* gid, uint32_t* tile_offsets) {
+                     const uint32_t* touched, const uint32_t* tile_select, uint64_t* keys, uint32_t* gid,
+                     uint32_t* tile_offsets) {
     const int gx = (cam->W + TILE - 1) / TILE, gy = (cam->H + TILE - 1) / TILE;
     const int T = gx * gy;
+    int64_t cap = 0;
+    for (int i = 0; i < N; ++i) cap += touched[i];
+    pair_t* pr = (pair_t*)malloc(sizeof(pair_t) * (size_t)(cap > 0 ? cap : 1));
     int64_t P = 0;
-    for (int i = 0; i < N; ++i) P += touched[i];
-    pair_t* pr = (pair_t*)malloc(sizeof(pair_t) * (size_t)(P > 0 ? P : 1));
-    int64_t w = 0;
     for (int i = 0; i < N; ++i) {
         if (!touched[i]) continue;
         uint64_t db = depth_bits(depth[i]);
         for (int ty = rect[4 * i + 1]; ty < rect[4 * i + 3]; ++ty)
             for (int tx = rect[4 * i]; tx < rect[4 * i + 2]; ++tx) {
-                pr[w].key = ((uint64_t)(uint32_t)(ty * gx + tx) << 32) | db;
-                pr[w].gid = (uint32_t)i;
-                ++w;
+                const uint32_t t = (uint32_t)(ty * gx + tx);
+                if (tile_select && !tile_select[t]) continue;
+                pr[P].key = ((uint64_t)t << 32) | db;
+                pr[P].gid = (uint32_t)i;
+                ++P;
             }
     }
     qsort(pr, (size_t)P, sizeof(pair_t), pair_cmp);

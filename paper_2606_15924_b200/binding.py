@@ -80,10 +80,10 @@ def load_library() -> C.CDLL:
     cam = C.POINTER(Camera)
     lib.tgs_preprocess.argtypes = [vp, cam, i32, i32] + [vp] * 5 + [vp] * 3 + [vp]
     lib.tgs_bin_sort_workspace_bytes.argtypes = [i32, i64, i32, C.POINTER(C.c_size_t)]
-    lib.tgs_bin_sort.argtypes = [vp, cam, i32, vp, i64, vp, vp, vp, vp, C.POINTER(i64), vp, C.c_size_t, vp]
+    lib.tgs_bin_sort.argtypes = [vp, cam, i32, vp, vp, i64, vp, vp, vp, vp, C.POINTER(i64), vp, C.c_size_t, vp]
     lib.tgs_sample_num_tiles.argtypes = [cam, i32, i32]
     lib.tgs_sample_workspace_bytes.argtypes = [cam, C.POINTER(C.c_size_t)]
-    lib.tgs_sample.argtypes = [vp, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp,
+    lib.tgs_sample.argtypes = [vp, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp, vp,
                                C.POINTER(C.c_int32), vp, C.c_size_t, vp]
     lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
@@ -153,7 +153,8 @@ class TGS:
             raise TgsError(rc, "tgs_bin_sort_workspace_bytes")
         return b.value
 
-    def bin_sort(self, cam, splats, P_capacity, want_keys=False, out=None, workspace=None, sync=True, stream=None):
+    def bin_sort(self, cam, splats, P_capacity, want_keys=False, out=None, workspace=None, sync=True, stream=None,
+                 tile_select=None):
         cam = Camera.of(cam)
         N = splats.shape[0]
         T = cam.num_tiles
@@ -167,7 +168,7 @@ class TGS:
         if workspace is None:
             workspace = torch.empty(need, dtype=torch.uint8, device=self.device)
         ph = C.c_int64(-1)
-        rc = self.lib.tgs_bin_sort(self._h, C.byref(cam), N, _p(splats), P_capacity, _p(out.keys_sorted),
+        rc = self.lib.tgs_bin_sort(self._h, C.byref(cam), N, _p(splats), _p(tile_select), P_capacity, _p(out.keys_sorted),
                                    _p(out.gid_sorted), _p(out.tile_offsets), _p(out.P_dev),
                                    C.byref(ph) if sync else None, _p(workspace), workspace.numel(), _stream(stream))
         if sync:
@@ -197,6 +198,7 @@ class TGS:
                                   tiles=torch.empty(T, dtype=torch.int32, device=self.device),
                                   tile_pix_offsets=torch.empty(T + 1, dtype=torch.int32, device=self.device),
                                   pix=torch.empty(cam.width * cam.height, dtype=torch.int32, device=self.device),
+                                  tile_select=torch.empty(T, dtype=torch.int32, device=self.device),
                                   kn_dev=torch.zeros(2, dtype=torch.int32, device=self.device), k=None, n=None)
         if workspace is None:
             workspace = torch.empty(self.sample_workspace_bytes(cam), dtype=torch.uint8, device=self.device)
@@ -204,7 +206,8 @@ class TGS:
         self._check(self.lib.tgs_sample(self._h, C.byref(cam), _p(err), _p(render), _p(target), int(tile_pct[0]),
                                         int(tile_pct[1]), int(pixel_mode), int(pix_rate[0]), int(pix_rate[1]),
                                         C.c_uint64(seed), _p(out.tile_score), _p(out.tiles), _p(out.tile_pix_offsets),
-                                        _p(out.pix), _p(out.kn_dev), kn if sync else None, _p(workspace),
+                                        _p(out.pix), _p(getattr(out, "tile_select", None)), _p(out.kn_dev),
+                                        kn if sync else None, _p(workspace),
                                         workspace.numel(), _stream(stream)))
         out.k = self.sample_num_tiles(cam, tile_pct[0], tile_pct[1])
         if sync:

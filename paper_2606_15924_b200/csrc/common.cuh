@@ -61,14 +61,16 @@ cudaError_t launch_preprocess(const CamK& cam, int N, int D, const float* mu, co
                               uint8_t* clamped, cudaStream_t s);
 
 size_t binsort_workspace_bytes(int N, int64_t Pcap, int T);
-cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats, int64_t Pcap, uint64_t* keys_sorted,
+cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats, const uint32_t* tile_select, int64_t Pcap,
+                            uint64_t* keys_sorted,
                             uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev, void* ws,
                             size_t ws_bytes, int num_sms, cudaStream_t s);
 
 size_t sample_workspace_bytes(int T);
 cudaError_t launch_sample(const CamK& cam, const float* err, const float* render, const float* target, int k,
                           int mode, int rnum, int rden, uint64_t seed, uint64_t* tile_score, uint32_t* tiles,
-                          uint32_t* tpo, uint32_t* pix, int32_t* kn_dev, void* ws, cudaStream_t s);
+                          uint32_t* tpo, uint32_t* pix, uint32_t* tile_select, int32_t* kn_dev, void* ws,
+                          cudaStream_t s);
 
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,

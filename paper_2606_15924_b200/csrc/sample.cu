@@ -211,10 +211,11 @@ size_t sample_workspace_bytes(int T) {
 
 cudaError_t launch_sample(const CamK& cam, const float* err, const float* render, const float* target, int k,
                           int mode, int rnum, int rden, uint64_t seed, uint64_t* tile_score, uint32_t* tiles,
-                          uint32_t* tpo, uint32_t* pix, int32_t* kn_dev, void* ws, cudaStream_t s) {
+                          uint32_t* tpo, uint32_t* pix, uint32_t* tile_select, int32_t* kn_dev, void* ws,
+                          cudaStream_t s) {
     const int T = cam.gx * cam.gy;
     TileMeta* meta = (TileMeta*)ws;
-    uint32_t* selected = (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
+    uint32_t* selected = tile_select ? tile_select : (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
     tile_reduce_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, err, render, target, mode, rnum, rden, seed, tile_score, meta);
     tile_select_kernel<<<(T + 7) / 8, 256, 0, s>>>(T, k, tile_score, selected);
     tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);

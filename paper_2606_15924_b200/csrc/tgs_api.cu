@@ -107,7 +107,8 @@ int tgs_bin_sort_workspace_bytes(int N, int64_t P_capacity, int T, size_t* bytes
     return TGS_OK;
 }
 
-int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats, int64_t P_capacity,
+int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats, const uint32_t* tile_select,
+                 int64_t P_capacity,
                  uint64_t* keys_sorted, uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev,
                  int64_t* P_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
@@ -123,7 +124,7 @@ int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats
     if (workspace_bytes < need)
         return fail(ctx, TGS_ERR_CAPACITY, "tgs_bin_sort: workspace %zu B < required %zu B", workspace_bytes, need);
     cudaStream_t s = (cudaStream_t)stream;
-    cudaError_t e = launch_bin_sort(make_camk(cam), N, splats, P_capacity, keys_sorted, gid_sorted, tile_offsets,
+    cudaError_t e = launch_bin_sort(make_camk(cam), N, splats, tile_select, P_capacity, keys_sorted, gid_sorted, tile_offsets,
                                     P_dev, workspace, workspace_bytes, ctx->num_sms, s);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_bin_sort", e);
     if (P_host) {
@@ -156,7 +157,7 @@ int tgs_sample_workspace_bytes(const tgs_camera* cam, size_t* bytes) {
 int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const float* render, const float* target,
                int tile_pct_num, int tile_pct_den, int pixel_mode, int pix_rate_num, int pix_rate_den,
                uint64_t seed, uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
-               int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
+               uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: bad camera");
     if (tile_pct_den <= 0 || tile_pct_num < 0 || tile_pct_num > tile_pct_den)
@@ -177,7 +178,7 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const floa
     const int k = tgs_sample_num_tiles(cam, tile_pct_num, tile_pct_den);
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e = launch_sample(make_camk(cam), err, render, target, k, pixel_mode, pix_rate_num, pix_rate_den, seed,
-                                  tile_score, tiles, tile_pix_offsets, pix, kn_dev, workspace, s);
+                                  tile_score, tiles, tile_pix_offsets, pix, tile_select, kn_dev, workspace, s);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_sample", e);
     if (kn_host) {
         e = cudaMemcpyAsync(kn_host, kn_dev, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);

@@ -28,7 +28,8 @@ class SparseRasterStep:
                                       gid_sorted=e(max(P_capacity, 1), i32), tile_offsets=e(T + 1, i32),
                                       P_dev=torch.zeros(2, dtype=i64, device=dev), P=None)
         self.samp = SimpleNamespace(tile_score=e(T, i64), tiles=e(T, i32), tile_pix_offsets=e(T + 1, i32),
-                                    pix=e(npx, i32), kn_dev=torch.zeros(2, dtype=i32, device=dev), k=None, n=None)
+                                    pix=e(npx, i32), tile_select=e(T, i32),
+                                    kn_dev=torch.zeros(2, dtype=i32, device=dev), k=None, n=None)
         self.fwd = SimpleNamespace(color=e((npx, 3), f32), T=e(npx, f32), n_contrib=e(npx, i32),
                                    n_walked=e(npx, i32) if want_walked else None,
                                    n_blended=e(npx, i32) if want_walked else None)
@@ -39,13 +40,21 @@ class SparseRasterStep:
         self.ws_sample = e(tgs.sample_workspace_bytes(self.cam), u8)
 
     def forward(self, means3D, scales, quats, opacities, sh, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0,
-                err=None, render=None, target=None, stream=None):
+                err=None, render=None, target=None, stream=None, restrict=True):
+        """restrict=True: sample first and bin only the selected tiles (tgs_bin_sort's tile_select;
+        DESIGN.md R14).  restrict=False: bin every tile, then sample (the call order of north_star)."""
         t = self.tgs
         t.preprocess(self.cam, self.D, means3D, scales, quats, opacities, sh, out=self.pre, stream=stream)
-        t.bin_sort(self.cam, self.pre.splats, self.P_capacity, out=self.binned, workspace=self.ws_sort, sync=False,
-                   stream=stream)
-        t.sample(self.cam, tile_pct, pixel_mode, pix_rate, seed, err=err, render=render, target=target,
-                 out=self.samp, workspace=self.ws_sample, sync=False, stream=stream)
+        if restrict:
+            t.sample(self.cam, tile_pct, pixel_mode, pix_rate, seed, err=err, render=render, target=target,
+                     out=self.samp, workspace=self.ws_sample, sync=False, stream=stream)
+            t.bin_sort(self.cam, self.pre.splats, self.P_capacity, out=self.binned, workspace=self.ws_sort, sync=False,
+                       stream=stream, tile_select=self.samp.tile_select)
+        else:
+            t.bin_sort(self.cam, self.pre.splats, self.P_capacity, out=self.binned, workspace=self.ws_sort, sync=False,
+                       stream=stream)
+            t.sample(self.cam, tile_pct, pixel_mode, pix_rate, seed, err=err, render=render, target=target,
+                     out=self.samp, workspace=self.ws_sample, sync=False, stream=stream)
         t.raster_fwd_sparse(self.cam, self.pre.splats, self.binned, self.samp, out=self.fwd, stream=stream)
         self._inputs = (means3D, scales, quats, sh)
         return self.fwd

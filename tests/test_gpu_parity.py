@@ -100,6 +100,15 @@ def test_bin_sort_parity(name, orc32, tgs, torch):
     with pytest.raises(pk.TgsError) as ei:
         tgs.bin_sort(sc.cam, splats, P - 1)
     assert ei.value.code == 2 and str(P) in str(ei.value)
+    # restricted to the sampled tiles (tile_select): same lists for those tiles, empty ranges elsewhere
+    sel = np.zeros(sc.cam.num_tiles, np.uint32)
+    sel[r.samp.tiles] = 1
+    rb = orc32.bin_sort(sc.cam, r.pre, tile_select=sel)
+    out3 = tgs.bin_sort(sc.cam, splats, rb.P + 5, want_keys=True, tile_select=dev(sel.astype(np.int32), torch))
+    assert out3.P == rb.P and rb.P < P
+    assert np.array_equal(u32(out3.tile_offsets), rb.tile_offsets)
+    assert np.array_equal(u32(out3.gid_sorted)[:rb.P], rb.gid_sorted)
+    assert np.array_equal(out3.keys_sorted.cpu().numpy().view(np.uint64)[:rb.P], rb.keys_sorted)
 
 
 @pytest.mark.parametrize("name", SCENES)
@@ -119,6 +128,9 @@ def test_sample_parity(name, orc32, tgs, torch):
     assert np.array_equal(u32(out.tiles)[:s.k], s.tiles)
     assert np.array_equal(u32(out.tile_pix_offsets)[:s.k + 1], s.tile_pix_offsets)
     assert np.array_equal(u32(out.pix)[:s.n], s.pix)
+    sel = np.zeros(sc.cam.num_tiles, np.uint32)
+    sel[s.tiles] = 1
+    assert np.array_equal(u32(out.tile_select), sel)
 
 
 @pytest.mark.parametrize("mode,pct,rate", [(0, (100, 100), (1, 1)), (0, (5, 100), (1, 1)), (1, (100, 100), (1, 2)),
@@ -206,8 +218,15 @@ def test_end_to_end_all_gpu(name, orc32, tgs, torch):
     step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
                  sc.sample_seed, **kw)
     P, k, n = step.counts()
-    assert (P, k) == (r.binned.P, r.samp.k)
+    assert k == r.samp.k
     if sc.err is not None:
+        # the step bins only the sampled tiles (restrict=True): same ranges for those tiles
+        sel = np.zeros(sc.cam.num_tiles, np.uint32)
+        sel[r.samp.tiles] = 1
+        rb = orc32.bin_sort(sc.cam, r.pre, tile_select=sel)
+        assert P == rb.P
+        assert np.array_equal(u32(step.binned.tile_offsets), rb.tile_offsets)
+        assert np.array_equal(u32(step.binned.gid_sorted)[:P], rb.gid_sorted)
         assert n == r.samp.n and np.array_equal(u32(step.samp.pix)[:n], r.samp.pix)
         rep = check_forward(step.fwd.color[:n].cpu().numpy(), step.fwd.T[:n].cpu().numpy(),
                             u32(step.fwd.n_contrib)[:n], r.fwd)
@@ -286,3 +305,69 @@ def test_sort_stability_with_duplicate_depths(orc32, tgs, torch):
     assert np.array_equal(u32(out.gid_sorted)[:b.P], b.gid_sorted)
     assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:b.P], b.keys_sorted)
     assert np.array_equal(u32(out.tile_offsets), b.tile_offsets)
+
+
+def _fake_pre(rng, N, gx, gy, rect_fn, depth_fn):
+    """Synthetic preprocess output (only rect / depth / radii matter to bin_sort)."""
+    from types import SimpleNamespace
+    rect = np.zeros((N, 4), np.int32)
+    x0, y0, w, h = rect_fn(rng, N)
+    rect[:, 0], rect[:, 1] = x0, y0
+    rect[:, 2], rect[:, 3] = np.minimum(x0 + w, gx), np.minimum(y0 + h, gy)
+    touched = ((rect[:, 2] - rect[:, 0]) * (rect[:, 3] - rect[:, 1])).astype(np.uint32)
+    return SimpleNamespace(means2D=np.zeros((N, 2), np.float32), conic_opacity=np.ones((N, 4), np.float32),
+                           rgb=np.zeros((N, 3), np.float32), depths=depth_fn(rng, N).astype(np.float32), rect=rect,
+                           tiles_touched=touched, radii=(touched > 0).astype(np.int32))
+
+
+@pytest.mark.parametrize("case", ["huge_segment", "equal_depths", "few_depths", "many_tiles", "wide_rects"])
+def test_bin_sort_segment_paths(case, orc32, tgs, torch):
+    """Every path of the segment sort: shared-memory small / big blocks, the global ping-pong for
+    oversized segments, the tie step and the full-LSD fallback on long tie runs, the global-atomic
+    histogram for very large tile grids, warp-cooperative walks of wide rects."""
+    rng = np.random.default_rng(11)
+    W, H = 128, 96
+    uni = lambda lo, hi: (lambda r, n: r.uniform(lo, hi, n))
+    if case == "huge_segment":      # one tile with ~45 k pairs, its neighbours 3-24 k
+        N = 70000
+        rect_fn = lambda r, n: (np.where(r.random(n) < 0.7, 3, r.integers(0, 8, n)), np.where(r.random(n) < 0.8, 2, r.integers(0, 6, n)),
+                                r.integers(1, 3, n), r.integers(1, 3, n))
+        depth_fn = uni(0.3, 40.0)
+    elif case == "equal_depths":    # all depths equal: order is by Gaussian id only
+        N = 30000
+        rect_fn = lambda r, n: (r.integers(0, 8, n), r.integers(0, 6, n), r.integers(1, 3, n), r.integers(1, 2, n))
+        depth_fn = lambda r, n: np.full(n, 2.5)
+    elif case == "few_depths":      # 7 distinct depths: tie runs of thousands, in a 20 k segment too
+        N = 50000
+        rect_fn = lambda r, n: (np.where(r.random(n) < 0.4, 1, r.integers(0, 8, n)), np.where(r.random(n) < 0.5, 1, r.integers(0, 6, n)),
+                                r.integers(1, 2, n), r.integers(1, 2, n))
+        depth_fn = lambda r, n: 1.0 + r.integers(0, 7, n) * 0.37
+    elif case == "many_tiles":      # T = 14124 > 12288: tile histogram in global memory
+        W, H, N = 2100, 1700, 40000
+        rect_fn = lambda r, n: (r.integers(0, 132, n), r.integers(0, 107, n), r.integers(1, 6, n), r.integers(1, 6, n))
+        depth_fn = uni(0.5, 30.0)
+    else:                           # wide_rects: splats covering up to the whole grid
+        W, H, N = 640, 480, 3000
+        rect_fn = lambda r, n: (r.integers(0, 20, n), r.integers(0, 15, n), r.integers(1, 41, n), r.integers(1, 31, n))
+        depth_fn = lambda r, n: np.round(r.uniform(1, 3, n), 2)  # with exact ties
+    cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    gx, gy = cam.grid
+    pre = _fake_pre(rng, N, gx, gy, rect_fn, depth_fn)
+    b = orc32.bin_sort(cam, pre)
+    splats = dev(pack_splats(pre), torch)
+    out = tgs.bin_sort(cam, splats, b.P + 3, want_keys=True)
+    assert out.P == b.P
+    assert np.array_equal(u32(out.tile_offsets), b.tile_offsets)
+    assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:b.P], b.keys_sorted)
+    assert np.array_equal(u32(out.gid_sorted)[:b.P], b.gid_sorted)
+    seg = np.diff(b.tile_offsets.astype(np.int64))
+    if case == "huge_segment":
+        assert seg.max() > 8192 and ((seg > 3072) & (seg <= 8192)).any()
+    # restricted to a random half of the tiles
+    sel = (rng.random(gx * gy) < 0.5).astype(np.uint32)
+    rb = orc32.bin_sort(cam, pre, tile_select=sel)
+    out = tgs.bin_sort(cam, splats, rb.P, want_keys=True, tile_select=dev(sel.astype(np.int32), torch))
+    assert out.P == rb.P
+    assert np.array_equal(u32(out.tile_offsets), rb.tile_offsets)
+    assert np.array_equal(u32(out.gid_sorted)[:rb.P], rb.gid_sorted)
+    assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:rb.P], rb.keys_sorted)
