@@ -1,34 +1,40 @@
-// tgs_bin_sort: tile-overlap duplication, hand-written radix sort of the (tile, depth) keys and
-// per-tile CSR ranges ("K(p) ... sorted by depth").
+// tgs_bin_sort: tile-overlap duplication, hand-written sort of the (tile, depth) keys and per-tile
+// CSR ranges ("K(p) ... sorted by depth").
 //
 // Required result: all (tile, Gaussian) pairs ordered by (tile_id, depth bits, Gaussian id) --
 // i.e. the 64-bit keys tile_id<<32 | float_bits(depth) sorted, ties by Gaussian id.  The key has
-// structure a generic 64-bit sort does not use: its high word is a BIN (a few thousand tiles) and
-// only the low word needs ordering, inside one bin at a time.  So the sort is an MSD radix sort
-// whose first digit is the whole tile id, done as a counting sort, followed by an independent
-// LSD radix sort of every tile's segment in SHARED MEMORY:
+// structure a generic 64-bit sort does not use: its high word is a BIN (a few thousand tiles), only
+// the low word needs ordering inside one bin, and the bins a Gaussian falls into form a small
+// rectangle.  Shared-memory and global atomics cost ~2 cycles per LANE on this machine, i.e. one
+// atomic per pair is as expensive as all the memory traffic of the sort, so the design avoids
+// per-pair atomics altogether:
 //
-//   K1 bin_count    per Gaussian, per covered (selected) tile: count.  Counts are privatised in a
-//                   shared-memory histogram per block (hot tiles of a clustered scene would
-//                   serialise same-address global atomics).  The last block to finish turns the
-//                   counts into the CSR tile_offsets[T+1], P, and the list of oversized tiles.
-//   K2 bin_scatter  same walk; a block reserves its share of every tile's segment with one global
-//                   atomic per (block, tile) and its threads take slots with shared-memory atomics;
-//                   writes (depth bits, Gaussian id) into the tile's segment, in arbitrary order.
-//   K3 seg_sort     persistent blocks pull tiles; a segment is loaded into shared memory, sorted by
-//                   LSD radix passes over the VARYING depth bits only (per-warp private histograms,
-//                   match-any ranking: stable), and written out as gid_sorted.  Only the top
-//                   ~log2(m)+5 varying bits are radix-sorted (usually 2 passes of <= 9 bits); the
-//                   few elements that still tie on those bits are ordered by a local full
-//                   (depth, id) comparison.  A segment whose ties run longer than 32 falls back to
-//                   the full LSD sort on all 64 bits (id digits first).  Segments larger than the
-//                   shared-memory capacity are sorted by a second launch with 1024-thread blocks
-//                   (shared memory up to 8192 entries, global ping-pong beyond).
+//   K0 topleft_count  one RED per visible Gaussian: histogram of the rect's top-left tile.
+//   K1 bin_scan       (one block) exclusive scan of that histogram; summed-area table of tile_select.
+//   K2 reorder        a 16-byte record {depth bits, id, rect} per visible Gaussian, grouped by
+//                     top-left tile.  Gaussians whose rect holds no selected tile get an empty rect.
+//                     From here on a warp's 32 records are neighbours on screen.
+//   K3 pair_count     per warp: the lanes that share a top-left ROW span a window of a few tiles;
+//                     for every window tile ONE ballot gives the covering lanes, so the warp
+//                     issues one RED per (warp, tile) instead of one per pair.  Rects wider than
+//                     4x4 tiles are walked by the whole warp, one atomic per pair (few Gaussians).
+//   K4 tile_scan      (one block) CSR tile_offsets[T+1], P, and the work lists of the sort by size.
+//   K5 pair_scatter   same walk as K3: one ATOM per (warp, tile) reserves a run of the tile's
+//                     segment, the covering lanes write (depth bits, id) at consecutive slots.
+//   K6 giant_split    segments above the shared-memory capacity are split by depth into
+//                     sub-segments (monotone interpolation between the segment's min and max key).
+//   K7 seg_sort       a block sorts a segment in shared memory in ONE distribution step: bucket =
+//                     monotone interpolation of the depth bits between the segment's min and max
+//                     (about one element per bucket); the slot inside a bucket is found WITHOUT
+//                     atomics by write-then-check rounds on a 16-bit table (the last writer of a
+//                     round wins a slot; ~6 rounds); buckets are then ordered by counting, inside
+//                     each bucket, the elements with a smaller (depth, id).  A segment whose keys
+//                     pile up (> 64 in a bucket: equal depths) falls back to a stable LSD radix
+//                     sort on (id, depth) in global memory.
 //
-// The final order is unique, so the result is deterministic although K2's intra-segment order is
-// not.  With `tile_select` (written by tgs_sample) only pairs of selected tiles are counted and
-// scattered: every cost after reading the 16 rect/depth bytes per Gaussian scales with the sampled
-// tile fraction (R14).
+// The final order is unique, so the result is deterministic although the slot assignment of K2/K5
+// is not.  With `tile_select` (written by tgs_sample) only pairs of selected tiles are counted and
+// scattered: everything after K2 scales with the sampled tile fraction (R14).
 //
 // Every kernel reads its element counts from device memory (P is data dependent), so the whole
 // call is asynchronous and graph-capturable.
@@ -38,20 +44,28 @@ namespace tgs {
 
 namespace {
 
-constexpr int kBinThreads = 256;
-constexpr int kSmemTilesMax = 12288;   // tile histogram kept in shared memory up to this many tiles (48 KB)
-constexpr int kSmallRect = 6;          // rects up to this many tiles are walked by their own thread
-constexpr int kMaxDigitBits = 9;
-constexpr int kTieRun = 32;            // longest tie run resolved by local comparison
+constexpr int kScanThreads = 1024;
+constexpr int kWalkThreads = 256;
+constexpr int kSmallW = 4, kSmallH = 4;  // rects up to this size go through the ballot window
+constexpr int kRounds = 12;              // write-then-check rounds before the atomic fallback
+constexpr uint32_t kMaxOcc = 64;         // bucket occupancy above which a segment takes the radix fallback
+constexpr int kFbBits = 8;               // digit width of the fallback radix sort
+constexpr uint32_t kSubTarget = 2048;    // expected sub-segment size of a giant split
+constexpr int kCoarseMax = 1024;         // sub-segments per giant tile (one per thread of giant_split)
 
 // zeroed words at the head of the workspace
 struct Counters {
-    uint32_t done_count;     // K1 blocks finished
-    uint32_t n_big;          // tiles with more than the small kernel's capacity
-    uint32_t sched_small;    // work tickets of the two seg_sort launches
-    uint32_t sched_big;
-    uint32_t done_small;     // blocks finished (self re-arm is not needed: zeroed per call)
-    uint32_t pad[3];
+    uint32_t n_vis;                       // visible Gaussians (records written by K2)
+    uint32_t n_small, n_large, n_giant;   // lengths of the work lists
+    uint32_t sched_small, sched_large, sched_giant;  // work tickets
+    uint32_t pad;
+};
+
+struct Seg {            // one unit of sort work
+    uint32_t start;     // offset in pairs / tmp / gid_sorted
+    uint32_t len;
+    uint32_t tile;
+    uint32_t in_tmp;    // 1: the unsorted pairs are in tmp (a sub-segment written by giant_split)
 };
 
 __device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v) {
@@ -84,91 +98,208 @@ __device__ __forceinline__ uint32_t block_excl_scan(uint32_t v, uint32_t* ws, ui
     return r;
 }
 
-// ---- the walk shared by K1 and K2: every (Gaussian, covered selected tile) pair of a chunk -------
-// f(tile, gid, depth_bits) is called once per pair.  Small rects are walked by their own thread,
-// large ones by the whole warp (a 30x30-tile splat must not stall 31 lanes).
-template <class F>
-__device__ __forceinline__ void walk_pairs(int begin, int end, int gx, const float4* __restrict__ splats,
-                                           const uint32_t* __restrict__ tile_select, F f) {
+__device__ __forceinline__ void load_rect(const float4* __restrict__ splats, int i, int gx, int gy, int& x0, int& y0,
+                                          int& x1, int& y1, uint32_t& dbits) {
+    const float4 r2 = splats[3 * (size_t)i + 2];
+    unpack_rect(__float_as_uint(r2.z), __float_as_uint(r2.w), x0, y0, x1, y1);
+    x1 = min(x1, gx);
+    y1 = min(y1, gy);
+    dbits = __float_as_uint(r2.y);
+}
+
+// ---- K0: histogram of the top-left tile ---------------------------------------------------------
+__global__ void __launch_bounds__(256)
+topleft_count_kernel(int N, int gx, int gy, const float4* __restrict__ splats, uint32_t* __restrict__ bin_count) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        int x0, y0, x1, y1;
+        uint32_t d;
+        load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
+        if (x1 > x0 && y1 > y0) atomicAdd(&bin_count[y0 * gx + x0], 1u);
+    }
+}
+
+// ---- K1: scan of the top-left histogram; summed-area table of tile_select -----------------------
+// sat[(gy+1) x (gx+1)]: sat[y][x] = number of selected tiles with ty < y and tx < x.
+__global__ void __launch_bounds__(kScanThreads)
+bin_scan_kernel(int gx, int gy, const uint32_t* __restrict__ bin_count, uint32_t* __restrict__ bin_offset,
+                const uint32_t* __restrict__ tile_select, uint32_t* sat, Counters* __restrict__ ctr) {
+    __shared__ uint32_t ws[33];
+    __shared__ uint32_t s_carry;
+    const int T = gx * gy;
+    if (threadIdx.x == 0) s_carry = 0u;
+    __syncthreads();
+    constexpr int kPer = 4;
+    for (int b0 = 0; b0 < T; b0 += kScanThreads * kPer) {
+        const int t0 = b0 + (int)threadIdx.x * kPer;
+        uint32_t c[kPer], sum = 0;
+#pragma unroll
+        for (int j = 0; j < kPer; ++j) {
+            c[j] = (t0 + j < T) ? bin_count[t0 + j] : 0u;
+            sum += c[j];
+        }
+        uint32_t tot;
+        uint32_t run = s_carry + block_excl_scan(sum, ws, tot);
+#pragma unroll
+        for (int j = 0; j < kPer; ++j) {
+            if (t0 + j < T) bin_offset[t0 + j] = run;
+            run += c[j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) ctr->n_vis = s_carry;
+    if (tile_select == nullptr) return;
+    // summed-area table: row prefixes (a warp per row), then column sums (a thread per column)
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, sx = gx + 1;
+    for (int x = threadIdx.x; x <= gx; x += kScanThreads) sat[x] = 0u;
+    for (int y = warp; y < gy; y += kScanThreads / 32) {
+        uint32_t running = 0;
+        if (lane == 0) sat[(size_t)(y + 1) * sx] = 0u;
+        for (int xb = 0; xb < gx; xb += 32) {
+            const int x = xb + lane;
+            const uint32_t v = (x < gx && tile_select[y * gx + x]) ? 1u : 0u;
+            const uint32_t inc = warp_incl_scan(v) + running;
+            if (x < gx) sat[(size_t)(y + 1) * sx + x + 1] = inc;
+            running = __shfl_sync(0xffffffffu, inc, 31);
+        }
+    }
+    __syncthreads();
+    for (int x = 1 + (int)threadIdx.x; x <= gx; x += kScanThreads) {
+        uint32_t acc = 0;
+#pragma unroll 8
+        for (int y = 1; y <= gy; ++y) {
+            acc += sat[(size_t)y * sx + x];
+            sat[(size_t)y * sx + x] = acc;
+        }
+    }
+}
+
+// ---- K2: records grouped by top-left tile -----------------------------------------------------------
+__global__ void __launch_bounds__(256)
+reorder_kernel(int N, int gx, int gy, const float4* __restrict__ splats, const uint32_t* __restrict__ bin_offset,
+               uint32_t* __restrict__ bin_cursor, const uint32_t* __restrict__ sat, uint4* __restrict__ rec) {
+    const int sx = gx + 1;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+        int x0, y0, x1, y1;
+        uint32_t d;
+        load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
+        if (x1 <= x0 || y1 <= y0) continue;
+        bool dead = false;
+        if (sat != nullptr) {
+            const uint32_t n_sel = sat[(size_t)y1 * sx + x1] - sat[(size_t)y0 * sx + x1] - sat[(size_t)y1 * sx + x0] +
+                                   sat[(size_t)y0 * sx + x0];
+            dead = n_sel == 0u;
+        }
+        const int t0 = y0 * gx + x0;
+        const uint32_t slot = bin_offset[t0] + atomicAdd(&bin_cursor[t0], 1u);
+        const uint32_t rx = dead ? 0u : ((uint32_t)x0 | ((uint32_t)x1 << 16));
+        const uint32_t ry = dead ? 0u : ((uint32_t)y0 | ((uint32_t)y1 << 16));
+        rec[slot] = make_uint4(d, (uint32_t)i, rx, ry);
+    }
+}
+
+// ---- K3 / K5: the pair walk over the regrouped records ------------------------------------------
+// SCATTER = false: tile_count[t] += pairs of tile t.  SCATTER = true: (depth bits, id) of every pair
+// is written into its tile's segment (arbitrary order inside the segment).
+template <bool SCATTER>
+__global__ void __launch_bounds__(kWalkThreads)
+pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restrict__ ctr,
+                 const uint32_t* __restrict__ tile_select, uint32_t* __restrict__ tile_count,
+                 const uint32_t* __restrict__ tile_offsets, uint32_t* __restrict__ cursor,
+                 const int64_t* __restrict__ P_dev, uint2* __restrict__ pairs) {
+    if (SCATTER && P_dev[1]) return;  // over capacity: nothing is written
+    const uint32_t n = ctr->n_vis;
     const int lane = threadIdx.x & 31;
-    for (int i0 = begin + (int)(threadIdx.x & ~31u); i0 < end; i0 += blockDim.x) {
-        const int i = i0 + lane;
-        int x0 = 0, y0 = 0, x1 = 0, y1 = 0;
-        uint32_t dbits = 0;
-        if (i < end) {
-            const float4 r2 = splats[3 * (size_t)i + 2];
-            unpack_rect(__float_as_uint(r2.z), __float_as_uint(r2.w), x0, y0, x1, y1);
-            dbits = __float_as_uint(r2.y);
-        }
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const uint32_t gwarp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, nwarps = (gridDim.x * blockDim.x) >> 5;
+    for (uint32_t base = gwarp * 32u; base < n; base += nwarps * 32u) {
+        const uint32_t i = base + lane;
+        uint4 r = make_uint4(0u, 0u, 0u, 0u);
+        if (i < n) r = rec[i];
+        int x0, y0, x1, y1;
+        unpack_rect(r.z, r.w, x0, y0, x1, y1);
         const int w = x1 - x0, h = y1 - y0;
-        const int area = (w > 0 && h > 0) ? w * h : 0;
-        if (area > 0 && area <= kSmallRect) {
-            for (int ty = y0; ty < y1; ++ty)
-                for (int tx = x0; tx < x1; ++tx) {
-                    const uint32_t t = (uint32_t)(ty * gx + tx);
-                    if (tile_select == nullptr || tile_select[t]) f(t, (uint32_t)i, dbits);
+        const bool live = w > 0 && h > 0;
+        const bool small = live && w <= kSmallW && h <= kSmallH;
+        // ---- small rects: lanes with the same top row share a window of tiles ----
+        uint32_t todo = __ballot_sync(0xffffffffu, small);
+        while (todo) {
+            const int row = __shfl_sync(0xffffffffu, y0, __ffs(todo) - 1);
+            const bool in = small && y0 == row;
+            todo &= ~__ballot_sync(0xffffffffu, in);
+            const int X0 = __reduce_min_sync(0xffffffffu, in ? x0 : 0x7fffffff);
+            const int X1 = __reduce_max_sync(0xffffffffu, in ? x1 : 0);
+            const int Hw = __reduce_max_sync(0xffffffffu, in ? h : 0);
+            const int Ww = X1 - X0, win = Ww * Hw;
+            for (int c0 = 0; c0 < win; c0 += 32) {
+                const int cnt = min(32, win - c0);
+                int tyj = row + c0 / Ww, txj = X0 + c0 % Ww;
+                uint32_t mine = 0;  // lane j: the lanes whose rect covers window tile c0 + j
+                for (int j = 0; j < cnt; ++j) {
+                    const bool cov = in && txj >= x0 && txj < x1 && tyj < y1;
+                    const uint32_t bal = __ballot_sync(0xffffffffu, cov);
+                    if (lane == j) mine = bal;
+                    if (++txj == X1) { txj = X0; ++tyj; }
                 }
+                const int c = c0 + lane;
+                const uint32_t t = (uint32_t)((row + c / Ww) * gx + X0 + c % Ww);
+                bool has = c < win && mine != 0u;
+                if (has && tile_select != nullptr && tile_select[t] == 0u) has = false;
+                if (!SCATTER) {
+                    if (has) atomicAdd(&tile_count[t], (uint32_t)__popc(mine));
+                } else {
+                    uint32_t b = 0;
+                    if (has) b = tile_offsets[t] + atomicAdd(&cursor[t], (uint32_t)__popc(mine));
+                    uint32_t act = __ballot_sync(0xffffffffu, has);
+                    while (act) {
+                        const int j = __ffs(act) - 1;
+                        act &= act - 1u;
+                        const uint32_t mj = __shfl_sync(0xffffffffu, mine, j);
+                        const uint32_t bj = __shfl_sync(0xffffffffu, b, j);
+                        if ((mj >> lane) & 1u) pairs[bj + (uint32_t)__popc(mj & lt_mask)] = make_uint2(r.x, r.y);
+                    }
+                }
+            }
         }
-        uint32_t big = __ballot_sync(0xffffffffu, area > kSmallRect);
+        // ---- wide rects: the whole warp walks one rect, one atomic per pair ----
+        uint32_t big = __ballot_sync(0xffffffffu, live && !small);
         while (big) {
             const int src = __ffs(big) - 1;
-            big &= big - 1;
+            big &= big - 1u;
             const int bx0 = __shfl_sync(0xffffffffu, x0, src), by0 = __shfl_sync(0xffffffffu, y0, src);
-            const int bw = __shfl_sync(0xffffffffu, w, src), ba = __shfl_sync(0xffffffffu, area, src);
-            const uint32_t bd = __shfl_sync(0xffffffffu, dbits, src);
+            const int bw = __shfl_sync(0xffffffffu, w, src), ba = bw * __shfl_sync(0xffffffffu, h, src);
+            const uint32_t bd = __shfl_sync(0xffffffffu, r.x, src), bg = __shfl_sync(0xffffffffu, r.y, src);
             for (int j = lane; j < ba; j += 32) {
-                const int ty = by0 + j / bw, tx = bx0 + j % bw;
-                const uint32_t t = (uint32_t)(ty * gx + tx);
-                if (tile_select == nullptr || tile_select[t]) f(t, (uint32_t)(i0 + src), bd);
+                const uint32_t t = (uint32_t)((by0 + j / bw) * gx + bx0 + j % bw);
+                if (tile_select != nullptr && tile_select[t] == 0u) continue;
+                if (!SCATTER) {
+                    atomicAdd(&tile_count[t], 1u);
+                } else {
+                    const uint32_t slot = tile_offsets[t] + atomicAdd(&cursor[t], 1u);
+                    pairs[slot] = make_uint2(bd, bg);
+                }
             }
         }
     }
 }
 
-// ---- K1: per-tile pair counts, then (last block) CSR offsets, P and the oversized-tile list -----
-template <bool SMEM_HIST>
-__global__ void __launch_bounds__(kBinThreads)
-bin_count_kernel(int N, int chunk, int gx, int T, const float4* __restrict__ splats,
-                 const uint32_t* __restrict__ tile_select, uint32_t* __restrict__ tile_count,
-                 uint32_t* __restrict__ tile_offsets, int64_t Pcap, int64_t* __restrict__ P_dev,
-                 Counters* __restrict__ ctr, uint32_t* __restrict__ big_list, uint32_t small_cap) {
-    extern __shared__ __align__(16) uint32_t hist[];  // [T] when SMEM_HIST
+// ---- K4: CSR offsets, P, capacity flag and the work lists of the sort -------------------------------
+__global__ void __launch_bounds__(kScanThreads)
+tile_scan_kernel(int T, const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_offsets, int64_t Pcap,
+                 int64_t* __restrict__ P_dev, Counters* __restrict__ ctr, Seg* __restrict__ small_list,
+                 Seg* __restrict__ large_list, Seg* __restrict__ giant_list, uint32_t small_cap, uint32_t large_cap) {
     __shared__ uint32_t ws[33];
-    __shared__ uint32_t s_last;
     __shared__ unsigned long long s_carry;
-    if (SMEM_HIST) {
-        for (int t = threadIdx.x; t < T; t += blockDim.x) hist[t] = 0;
-        __syncthreads();
-    }
-    const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
-    if (SMEM_HIST)
-        walk_pairs(begin, end, gx, splats, tile_select, [&](uint32_t t, uint32_t, uint32_t) { atomicAdd(&hist[t], 1u); });
-    else
-        walk_pairs(begin, end, gx, splats, tile_select, [&](uint32_t t, uint32_t, uint32_t) { atomicAdd(&tile_count[t], 1u); });
-    __syncthreads();
-    if (SMEM_HIST) {
-        for (int t = threadIdx.x; t < T; t += blockDim.x) {
-            const uint32_t c = hist[t];
-            if (c) atomicAdd(&tile_count[t], c);
-        }
-    }
-    // ---- last block: exclusive scan of the counts ----
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(&ctr->done_count, 1u) == gridDim.x - 1u) ? 1u : 0u;
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
     if (threadIdx.x == 0) s_carry = 0ull;
     __syncthreads();
-    // each thread owns kPer consecutive tiles of a span of blockDim * kPer tiles
-    constexpr int kPer = 8;
-    for (int b0 = 0; b0 < T; b0 += kBinThreads * kPer) {
+    constexpr int kPer = 4;
+    for (int b0 = 0; b0 < T; b0 += kScanThreads * kPer) {
         const int t0 = b0 + (int)threadIdx.x * kPer;
         uint32_t c[kPer], sum = 0;
 #pragma unroll
         for (int j = 0; j < kPer; ++j) {
-            c[j] = (t0 + j < T) ? __ldcg(tile_count + t0 + j) : 0u;
+            c[j] = (t0 + j < T) ? tile_count[t0 + j] : 0u;
             sum += c[j];
         }
         uint32_t tot;
@@ -178,8 +309,15 @@ bin_count_kernel(int N, int chunk, int gx, int T, const float4* __restrict__ spl
         for (int j = 0; j < kPer; ++j) {
             if (t0 + j < T) {
                 // offsets are 32-bit; beyond capacity (< 2^30) nothing downstream runs
-                tile_offsets[t0 + j] = (uint32_t)(run < (1ull << 32) ? run : 0xffffffffull);
-                if (c[j] > small_cap) big_list[atomicAdd(&ctr->n_big, 1u)] = (uint32_t)(t0 + j);
+                const uint32_t st = (uint32_t)(run < (1ull << 32) ? run : 0xffffffffull);
+                tile_offsets[t0 + j] = st;
+                if (c[j] > 0u) {
+                    Seg sg;
+                    sg.start = st; sg.len = c[j]; sg.tile = (uint32_t)(t0 + j); sg.in_tmp = 0u;
+                    if (c[j] <= small_cap) small_list[atomicAdd(&ctr->n_small, 1u)] = sg;
+                    else if (c[j] <= large_cap) large_list[atomicAdd(&ctr->n_large, 1u)] = sg;
+                    else giant_list[atomicAdd(&ctr->n_giant, 1u)] = sg;
+                }
             }
             run += c[j];
         }
@@ -195,42 +333,78 @@ bin_count_kernel(int N, int chunk, int gx, int T, const float4* __restrict__ spl
     }
 }
 
-// ---- K2: scatter (depth bits, Gaussian id) into the tile segments ---------------------------------
-template <bool SMEM_HIST>
-__global__ void __launch_bounds__(kBinThreads)
-bin_scatter_kernel(int N, int chunk, int gx, int T, const float4* __restrict__ splats,
-                   const uint32_t* __restrict__ tile_select, const uint32_t* __restrict__ tile_offsets,
-                   uint32_t* __restrict__ cursor, const int64_t* __restrict__ P_dev, uint2* __restrict__ pairs) {
-    extern __shared__ __align__(16) uint32_t hist[];
-    if (P_dev[1]) return;  // over capacity: nothing is written
-    const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
-    if (SMEM_HIST) {
-        for (int t = threadIdx.x; t < T; t += blockDim.x) hist[t] = 0;
+// ---- monotone bucket map ------------------------------------------------------------------------
+// key in [kmin, kmax] -> bucket in [0, nb): every step (uint->float, multiply by a positive
+// constant, truncate, clamp) is non-decreasing, so bucket order never contradicts key order.
+__device__ __forceinline__ float bucket_scale(uint32_t kmin, uint32_t kmax, uint32_t nb) {
+    return (float)nb / ((float)(kmax - kmin) + 1.0f);
+}
+__device__ __forceinline__ uint32_t bucket_of(uint32_t key, uint32_t kmin, float scale, uint32_t nb) {
+    return min(nb - 1u, __float2uint_rz(__uint2float_rz(key - kmin) * scale));
+}
+
+// block-wide min / max of the depth bits; ws holds 66 words.  Ends with a barrier.
+__device__ __forceinline__ void block_minmax(uint32_t& lo, uint32_t& hi, uint32_t* ws) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+    lo = __reduce_min_sync(0xffffffffu, lo);
+    hi = __reduce_max_sync(0xffffffffu, hi);
+    if (lane == 0) { ws[warp] = lo; ws[33 + warp] = hi; }
+    __syncthreads();
+    lo = __reduce_min_sync(0xffffffffu, lane < nw ? ws[lane] : 0xffffffffu);
+    hi = __reduce_max_sync(0xffffffffu, lane < nw ? ws[33 + lane] : 0u);
+    __syncthreads();
+}
+
+// ---- K6: split the segments that exceed the shared-memory capacity ---------------------------------
+__global__ void __launch_bounds__(kCoarseMax)
+giant_split_kernel(const Seg* __restrict__ giant_list, Seg* __restrict__ large_list, Counters* __restrict__ ctr,
+                   const uint2* __restrict__ pairs, uint2* __restrict__ tmp, const int64_t* __restrict__ P_dev) {
+    __shared__ uint32_t hist[kCoarseMax];
+    __shared__ uint32_t ws[66];
+    __shared__ uint32_t s_ticket;
+    if (P_dev[1]) return;
+    const uint32_t n_work = *reinterpret_cast<volatile uint32_t*>(&ctr->n_giant);
+    for (;;) {
         __syncthreads();
-        walk_pairs(begin, end, gx, splats, tile_select, [&](uint32_t t, uint32_t, uint32_t) { atomicAdd(&hist[t], 1u); });
+        if (threadIdx.x == 0) s_ticket = atomicAdd(&ctr->sched_giant, 1u);
         __syncthreads();
-        // reserve this block's share of every segment it touches; hist[t] becomes the absolute cursor
-        for (int t = threadIdx.x; t < T; t += blockDim.x) {
-            const uint32_t c = hist[t];
-            if (c) hist[t] = tile_offsets[t] + atomicAdd(&cursor[t], c);
+        const uint32_t ticket = s_ticket;
+        if (ticket >= n_work) break;
+        const Seg sg = giant_list[ticket];
+        const uint2* src = pairs + sg.start;
+        uint32_t lo = 0xffffffffu, hi = 0u;
+        for (uint32_t i = threadIdx.x; i < sg.len; i += kCoarseMax) {
+            const uint32_t k = src[i].x;
+            lo = min(lo, k);
+            hi = max(hi, k);
+        }
+        block_minmax(lo, hi, ws);
+        const uint32_t nb = min((uint32_t)kCoarseMax, (sg.len + kSubTarget - 1u) / kSubTarget);
+        const float scale = bucket_scale(lo, hi, nb);
+        hist[threadIdx.x] = 0u;
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < sg.len; i += kCoarseMax) atomicAdd(&hist[bucket_of(src[i].x, lo, scale, nb)], 1u);
+        __syncthreads();
+        const uint32_t c = hist[threadIdx.x];
+        uint32_t tot;
+        const uint32_t off = block_excl_scan(c, ws, tot);
+        hist[threadIdx.x] = off;  // becomes the bucket's cursor
+        if (c > 0u) {
+            Seg sub;
+            sub.start = sg.start + off; sub.len = c; sub.tile = sg.tile; sub.in_tmp = 1u;
+            large_list[atomicAdd(&ctr->n_large, 1u)] = sub;
         }
         __syncthreads();
-        walk_pairs(begin, end, gx, splats, tile_select, [&](uint32_t t, uint32_t g, uint32_t d) {
-            const uint32_t slot = atomicAdd(&hist[t], 1u);
-            pairs[slot] = make_uint2(d, g);
-        });
-    } else {
-        walk_pairs(begin, end, gx, splats, tile_select, [&](uint32_t t, uint32_t g, uint32_t d) {
-            const uint32_t slot = tile_offsets[t] + atomicAdd(&cursor[t], 1u);
-            pairs[slot] = make_uint2(d, g);
-        });
+        for (uint32_t i = threadIdx.x; i < sg.len; i += kCoarseMax) {
+            const uint2 kv = src[i];
+            tmp[sg.start + atomicAdd(&hist[bucket_of(kv.x, lo, scale, nb)], 1u)] = kv;
+        }
     }
 }
 
-// ---- K3: per-tile segment sort ----------------------------------------------------------------------
-// One stable LSD pass src -> dst over `bits` bits at `shift` of word `word` (0 = depth, 1 = id).
-// Warp w owns the contiguous sub-range [w*per_warp, ...) and a private histogram row wh[w][*]:
-// count, scan in (digit, warp) order, then rank in range order with match-any.
+// ---- fallback: one stable LSD pass src -> dst over `bits` bits at `shift` of word `word` ------------
+// (0 = depth, 1 = id).  Warp w owns the contiguous sub-range [w*per_warp, ...) and a private
+// histogram row wh[w][*]: count, scan in (digit, warp) order, then rank in range order with match-any.
 template <int THREADS>
 __device__ __forceinline__ void radix_pass(const uint2* src, uint2* dst, uint32_t m, int word, int shift, int bits,
                                            uint32_t* wh, uint32_t* ws) {
@@ -294,136 +468,231 @@ __device__ __forceinline__ void radix_pass(const uint2* src, uint2* dst, uint32_
     __syncthreads();
 }
 
-__device__ __forceinline__ int ceil_log2_u32(uint32_t v) { return v <= 1u ? 0 : 32 - __clz(v - 1u); }
+// ---- K7: per-segment sort -----------------------------------------------------------------------------
+__device__ __forceinline__ bool pair_less(const uint2 a, const uint2 b) { return a.x < b.x || (a.x == b.x && a.y < b.y); }
 
-template <int THREADS, int CAP, bool BIG>
-__global__ void __launch_bounds__(THREADS)
-seg_sort_kernel(int T, const uint32_t* __restrict__ tile_offsets, uint2* pairs, uint2* tmp,
+template <int CAP, int NBMAX>
+struct SortSmem {
+    union {
+        uint2 B[CAP];             // the segment grouped by bucket (after the rounds)
+        uint16_t tab[2][NBMAX];   // write-then-check tables of the rounds
+    } u;
+    uint32_t cnt[NBMAX + 4];      // bucket counts -> exclusive offsets; histogram rows of the fallback
+};
+
+// KEEP: the segment's pairs stay in registers between the passes (otherwise they are re-read, L2 hits).
+template <int THREADS, int CAP, int NBMAX, bool KEEP, int MINB>
+__global__ void __launch_bounds__(THREADS, MINB)
+seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32_t* sched, uint2* pairs, uint2* tmp,
                 uint32_t* __restrict__ gid_sorted, uint64_t* __restrict__ keys_sorted,
-                const int64_t* __restrict__ P_dev, Counters* __restrict__ ctr, const uint32_t* __restrict__ big_list,
-                uint32_t small_cap, int gid_bits) {
-    constexpr int W = THREADS / 32;
+                const int64_t* __restrict__ P_dev, int gid_bits) {
+    constexpr int EPT = CAP / THREADS, PER = NBMAX / THREADS, W = THREADS / 32;
+    static_assert(PER % 4 == 0 && CAP <= 65535 && NBMAX <= 32768, "layout");
+    static_assert(sizeof(uint32_t) * (NBMAX + 4) >= sizeof(uint32_t) * W * (1 << kFbBits), "fallback histogram rows");
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint2* smA = reinterpret_cast<uint2*>(smem_raw);
-    uint2* smB = smA + CAP;
-    uint32_t* wh = reinterpret_cast<uint32_t*>(smB + CAP);  // [W][1 << kMaxDigitBits]
-    __shared__ uint32_t ws[33];
+    SortSmem<CAP, NBMAX>& sm = *reinterpret_cast<SortSmem<CAP, NBMAX>*>(smem_raw);
+    __shared__ uint32_t ws[66];
     __shared__ uint32_t s_ticket[2];
-    __shared__ uint32_t s_diff, s_flag;
     if (P_dev[1]) return;
-    uint32_t* sched = BIG ? &ctr->sched_big : &ctr->sched_small;
-    const uint32_t n_work = BIG ? *reinterpret_cast<volatile uint32_t*>(&ctr->n_big) : (uint32_t)T;
-    const int lane = threadIdx.x & 31;
-    if (threadIdx.x == 0) s_ticket[0] = atomicAdd(sched, 1u);
+    const uint32_t n_work = *reinterpret_cast<const volatile uint32_t*>(n_work_ptr);
+    const uint32_t tid = threadIdx.x;
+    if (tid == 0) s_ticket[0] = atomicAdd(sched, 1u);
     __syncthreads();
     for (uint32_t it = 0;; ++it) {
         const uint32_t ticket = s_ticket[it & 1u];
         if (ticket >= n_work) break;
-        if (threadIdx.x == 0) {  // prefetch the next ticket: its latency hides behind this tile
-            s_ticket[(it + 1u) & 1u] = atomicAdd(sched, 1u);
-            s_diff = 0u;
-            s_flag = 0u;
+        if (tid == 0) s_ticket[(it + 1u) & 1u] = atomicAdd(sched, 1u);  // prefetch: its latency hides behind this segment
+        const Seg sg = list[ticket];
+        uint2* src = (sg.in_tmp ? tmp : pairs) + sg.start;
+        uint2* oth = (sg.in_tmp ? pairs : tmp) + sg.start;
+        const uint32_t m = sg.len;
+        bool fb = m > (uint32_t)CAP;  // block-uniform from here on
+        uint2 kv[KEEP ? EPT : 1];
+        uint32_t lo = 0xffffffffu, hi = 0u;
+        if (!fb) {
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) {
+                const uint32_t i = (uint32_t)e * THREADS + tid;
+                if (i < m) {
+                    const uint2 v = src[i];
+                    if (KEEP) kv[KEEP ? e : 0] = v;
+                    lo = min(lo, v.x);
+                    hi = max(hi, v.x);
+                }
+            }
+        } else {
+            for (uint32_t i = tid; i < m; i += THREADS) {
+                const uint32_t k = src[i].x;
+                lo = min(lo, k);
+                hi = max(hi, k);
+            }
         }
-        const uint32_t t = BIG ? big_list[ticket] : ticket;
-        const uint32_t start = tile_offsets[t], m = tile_offsets[t + 1] - start;
-        __syncthreads();
-        if (m == 0u || (!BIG && m > small_cap)) { __syncthreads(); continue; }
-        const bool in_smem = BIG ? (m <= (uint32_t)CAP) : true;  // small kernel: always shared (address space known statically)
-        uint2* A = in_smem ? smA : pairs + start;
-        uint2* B = in_smem ? smB : tmp + start;
-        // ---- load (shared-memory path) and find the varying depth bits ----
-        {
-            const uint32_t k0 = pairs[start].x;
-            uint32_t diff = 0;
-            for (uint32_t i = threadIdx.x; i < m; i += THREADS) {
-                const uint2 kv = pairs[start + i];
-                if (in_smem) smA[i] = kv;
-                diff |= kv.x ^ k0;
+        block_minmax(lo, hi, ws);  // (its barriers also separate this segment's shared memory from the last one's)
+        if (lo == hi && m > kMaxOcc) fb = true;
+        if (!fb) {
+            uint32_t nb = 32u;
+            while (nb < 2u * m && nb < (uint32_t)NBMAX) nb <<= 1;
+            const float scale = bucket_scale(lo, hi, nb);
+            const uint32_t cbase = tid * PER;
+            if (cbase < nb) {
+#pragma unroll
+                for (int j = 0; j < PER; j += 4) *reinterpret_cast<uint4*>(&sm.cnt[cbase + j]) = make_uint4(0u, 0u, 0u, 0u);
             }
-            diff = __reduce_or_sync(0xffffffffu, diff);
-            if (lane == 0 && diff) atomicOr(&s_diff, diff);
-        }
-        __syncthreads();
-        const int nbits = 32 - __clz(s_diff);  // depth bits [0, nbits) vary inside this tile
-        int sb = min(nbits, max(8, min(27, ceil_log2_u32(m) + 5)));
-        int npass = (sb + kMaxDigitBits - 1) / kMaxDigitBits;
-        int bits = npass ? (sb + npass - 1) / npass : 0;
-        const int shift0 = max(0, nbits - npass * bits);  // bits below shift0 are left to the tie step
-        for (int p = 0; p < npass; ++p) {
-            radix_pass<THREADS>(A, B, m, 0, shift0 + p * bits, bits, wh, ws);
-            uint2* x = A; A = B; B = x;
-        }
-        // ---- ties on the sorted bits: local full (depth, id) comparison ----
-        for (uint32_t i = threadIdx.x; i < m; i += THREADS) {
-            const uint2 kv = A[i];
-            const uint32_t sk = shift0 < 32 ? (kv.x >> shift0) : 0u;
-            uint32_t s = i, e = i + 1;
-            while (s > 0 && i - s <= (uint32_t)kTieRun && (A[s - 1].x >> shift0) == sk) --s;
-            while (e < m && e - i <= (uint32_t)kTieRun && (A[e].x >> shift0) == sk) ++e;
-            if (i - s > (uint32_t)kTieRun || e - i > (uint32_t)kTieRun) {
-                s_flag = 1u;
-                continue;
+            // state of an element: bucket << 16 | slot inside the bucket (0xffff = pending); 0xffffffff = no element
+            uint32_t st[EPT];
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) {
+                const uint32_t i = (uint32_t)e * THREADS + tid;
+                st[e] = 0xffffffffu;
+                if (i < m) st[e] = (bucket_of(KEEP ? kv[KEEP ? e : 0].x : src[i].x, lo, scale, nb) << 16) | 0xffffu;
             }
-            uint32_t rank = 0;
-            for (uint32_t j = s; j < e; ++j) {
-                const uint2 o = A[j];
-                rank += (o.x < kv.x || (o.x == kv.x && o.y < kv.y)) ? 1u : 0u;
-            }
-            gid_sorted[start + s + rank] = kv.y;
-            if (keys_sorted) keys_sorted[start + s + rank] = ((uint64_t)t << 32) | (uint64_t)kv.x;
-        }
-        __syncthreads();
-        if (s_flag) {
-            // ---- fallback: full LSD sort on (depth, id): id digits first, then every varying depth bit ----
-            int np = (gid_bits + kMaxDigitBits - 1) / kMaxDigitBits, bt = (gid_bits + np - 1) / np;
-            for (int p = 0; p < np; ++p) {
-                radix_pass<THREADS>(A, B, m, 1, p * bt, bt, wh, ws);
-                uint2* x = A; A = B; B = x;
-            }
-            np = (nbits + kMaxDigitBits - 1) / kMaxDigitBits;
-            bt = np ? (nbits + np - 1) / np : 0;
-            for (int p = 0; p < np; ++p) {
-                radix_pass<THREADS>(A, B, m, 0, p * bt, bt, wh, ws);
-                uint2* x = A; A = B; B = x;
-            }
-            for (uint32_t i = threadIdx.x; i < m; i += THREADS) {
-                const uint2 kv = A[i];
-                gid_sorted[start + i] = kv.y;
-                if (keys_sorted) keys_sorted[start + i] = ((uint64_t)t << 32) | (uint64_t)kv.x;
+            // ---- rounds: the last writer of a bucket's table entry takes the bucket's next slot ----
+            for (int r = 0; r < kRounds; ++r) {
+                uint16_t* tab = sm.u.tab[r & 1];
+                bool any = false;
+#pragma unroll
+                for (int e = 0; e < EPT; ++e) {
+                    if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
+                        tab[st[e] >> 16] = (uint16_t)((uint32_t)e * THREADS + tid);
+                        any = true;
+                    }
+                }
+                if (!__syncthreads_or(any)) break;
+#pragma unroll
+                for (int e = 0; e < EPT; ++e) {
+                    if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
+                        const uint32_t b = st[e] >> 16;
+                        if (tab[b] == (uint16_t)((uint32_t)e * THREADS + tid)) {
+                            st[e] = (b << 16) | (uint32_t)r;
+                            sm.cnt[b] = (uint32_t)r + 1u;
+                        }
+                    }
+                }
             }
             __syncthreads();
+            // crowded buckets: the elements still pending take their slots with atomics
+#pragma unroll
+            for (int e = 0; e < EPT; ++e) {
+                if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
+                    const uint32_t b = st[e] >> 16;
+                    st[e] = (b << 16) | min(0xfffeu, atomicAdd(&sm.cnt[b], 1u));
+                }
+            }
+            __syncthreads();
+            // ---- counts -> exclusive offsets (in place), largest bucket ----
+            uint32_t c[PER], sum = 0, mx = 0;
+            if (cbase < nb) {
+#pragma unroll
+                for (int j = 0; j < PER; j += 4) {
+                    const uint4 q = *reinterpret_cast<const uint4*>(&sm.cnt[cbase + j]);
+                    c[j] = q.x; c[j + 1] = q.y; c[j + 2] = q.z; c[j + 3] = q.w;
+                }
+#pragma unroll
+                for (int j = 0; j < PER; ++j) {
+                    sum += c[j];
+                    mx = max(mx, c[j]);
+                }
+            }
+            uint32_t tot;
+            uint32_t run = block_excl_scan(sum, ws, tot);
+            if (cbase < nb) {
+#pragma unroll
+                for (int j = 0; j < PER; ++j) {
+                    sm.cnt[cbase + j] = run;
+                    run += c[j];
+                }
+            }
+            if (tid == 0) sm.cnt[nb] = m;
+            fb = __syncthreads_or(mx > kMaxOcc) != 0;
+            if (!fb) {
+                // ---- place by bucket, then order every bucket by counting smaller (depth, id) ----
+#pragma unroll
+                for (int e = 0; e < EPT; ++e) {
+                    if (st[e] != 0xffffffffu) {
+                        const uint2 v = KEEP ? kv[KEEP ? e : 0] : src[(uint32_t)e * THREADS + tid];
+                        sm.u.B[sm.cnt[st[e] >> 16] + (st[e] & 0xffffu)] = v;
+                    }
+                }
+                __syncthreads();
+#pragma unroll
+                for (int e = 0; e < EPT; ++e) {
+                    const uint32_t i = (uint32_t)e * THREADS + tid;
+                    if (i < m) {
+                        const uint2 v = sm.u.B[i];
+                        const uint32_t b = bucket_of(v.x, lo, scale, nb);
+                        const uint32_t s = sm.cnt[b], t = sm.cnt[b + 1];
+                        uint32_t rank = s;
+                        for (uint32_t j = s; j < t; ++j) rank += pair_less(sm.u.B[j], v) ? 1u : 0u;
+                        gid_sorted[sg.start + rank] = v.y;
+                        if (keys_sorted) keys_sorted[sg.start + rank] = ((uint64_t)sg.tile << 32) | (uint64_t)v.x;
+                    }
+                }
+            }
+        }
+        if (fb) {
+            // ---- fallback: stable LSD radix sort on (depth, id) in global memory: id digits first,
+            //      then every varying depth bit ----
+            __syncthreads();
+            uint32_t* wh = sm.cnt;
+            uint2 *A = src, *Bq = oth;
+            int np = (gid_bits + kFbBits - 1) / kFbBits, bt = (gid_bits + np - 1) / np;
+            for (int p = 0; p < np; ++p) {
+                radix_pass<THREADS>(A, Bq, m, 1, p * bt, bt, wh, ws);
+                uint2* x = A; A = Bq; Bq = x;
+            }
+            const int nbits = 32 - __clz(lo ^ hi);  // depth bits [0, nbits) vary inside this segment
+            np = (nbits + kFbBits - 1) / kFbBits;
+            bt = np ? (nbits + np - 1) / np : 0;
+            for (int p = 0; p < np; ++p) {
+                radix_pass<THREADS>(A, Bq, m, 0, p * bt, bt, wh, ws);
+                uint2* x = A; A = Bq; Bq = x;
+            }
+            for (uint32_t i = tid; i < m; i += THREADS) {
+                const uint2 v = A[i];
+                gid_sorted[sg.start + i] = v.y;
+                if (keys_sorted) keys_sorted[sg.start + i] = ((uint64_t)sg.tile << 32) | (uint64_t)v.x;
+            }
         }
     }
 }
 
-constexpr int kSmallThreads = 256, kSmallCap = 3072;
-constexpr int kBigThreads = 1024, kBigCap = 8192;
-constexpr size_t kSmallSmem = 2 * (size_t)kSmallCap * sizeof(uint2) + (kSmallThreads / 32) * (sizeof(uint32_t) << kMaxDigitBits);
-constexpr size_t kBigSmem = 2 * (size_t)kBigCap * sizeof(uint2) + (kBigThreads / 32) * (sizeof(uint32_t) << kMaxDigitBits);
+constexpr int kSmallThreads = 256, kSmallCap = 2048, kSmallNb = 4096;
+constexpr int kLargeThreads = 512, kLargeCap = 8192, kLargeNb = 8192;
+constexpr size_t kSmallSmem = sizeof(SortSmem<kSmallCap, kSmallNb>);
+constexpr size_t kLargeSmem = sizeof(SortSmem<kLargeCap, kLargeNb>);
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct Workspace {
-    // zeroed at the start of every call (one memset): counters, tile counts, scatter cursors
+    // zeroed at the start of every call (one memset): counters, histograms, cursors
     Counters* ctr;
-    uint32_t *tile_count, *cursor;
+    uint32_t *bin_count, *bin_cursor, *tile_count, *cursor;
     size_t zero_bytes;
-    uint32_t* big_list;   // [T]
-    uint2 *pairs, *tmp;   // [Pcap] each: unsorted segments; ping-pong partner for oversized segments
+    uint32_t *bin_offset, *sat;
+    uint4* rec;                                // [N] regrouped records
+    Seg *small_list, *large_list, *giant_list;
+    uint2 *pairs, *tmp;                        // [Pcap] each: unsorted segments; scratch of giant_split / the fallback
     size_t total;
 };
 
-Workspace carve(void* base, int T, int64_t Pcap) {
+Workspace carve(void* base, int N, int T_, int64_t Pcap) {
     Workspace w;
     size_t o = 0;
     char* p = (char*)base;
     auto take = [&](size_t bytes) { char* r = p + o; o += align256(bytes); return r; };
-    const size_t nt = (size_t)(T > 0 ? T : 1), pc = (size_t)(Pcap > 0 ? Pcap : 1);
+    const size_t nt = (size_t)(T_ > 0 ? T_ : 1), pc = (size_t)(Pcap > 0 ? Pcap : 1), nn = (size_t)(N > 0 ? N : 1);
     w.ctr = (Counters*)take(sizeof(Counters));
+    w.bin_count = (uint32_t*)take(nt * 4);
+    w.bin_cursor = (uint32_t*)take(nt * 4);
     w.tile_count = (uint32_t*)take(nt * 4);
     w.cursor = (uint32_t*)take(nt * 4);
     w.zero_bytes = o;
-    w.big_list = (uint32_t*)take(nt * 4);
+    w.bin_offset = (uint32_t*)take(nt * 4);
+    w.sat = (uint32_t*)take((2 * nt + 2) * 4);  // (gx+1)(gy+1) <= 2T+2
+    w.rec = (uint4*)take(nn * 16);
+    w.small_list = (Seg*)take(nt * sizeof(Seg));
+    w.large_list = (Seg*)take((2 * nt + pc / kSubTarget + 16) * sizeof(Seg));
+    w.giant_list = (Seg*)take(nt * sizeof(Seg));
     w.pairs = (uint2*)take(pc * 8);
     w.tmp = (uint2*)take(pc * 8);
     w.total = o;
@@ -432,65 +701,63 @@ Workspace carve(void* base, int T, int64_t Pcap) {
 
 }  // namespace
 
-size_t binsort_workspace_bytes(int N, int64_t Pcap, int T) {
-    (void)N;
-    return carve(nullptr, T, Pcap).total;
-}
+size_t binsort_workspace_bytes(int N, int64_t Pcap, int T) { return carve(nullptr, N, T, Pcap).total; }
 
 cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const uint32_t* tile_select, int64_t Pcap,
                             uint64_t* keys_sorted, uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev,
                             void* ws, size_t ws_bytes, int num_sms, cudaStream_t s) {
     (void)ws_bytes;
-    const int T = cam.gx * cam.gy;
-    const Workspace w = carve(ws, T, Pcap);
+    const int gx = cam.gx, gy = cam.gy, T = gx * gy;
+    const Workspace w = carve(ws, N, T, Pcap);
     const float4* splats = reinterpret_cast<const float4*>(splats_f);
     cudaError_t e = cudaMemsetAsync(w.ctr, 0, w.zero_bytes, s);
     if (e != cudaSuccess) return e;
 
     static bool opted_in = false;  // function attributes, set once per process
     if (!opted_in) {
-        e = cudaFuncSetAttribute(seg_sort_kernel<kSmallThreads, kSmallCap, false>,
+        e = cudaFuncSetAttribute(seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmallSmem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(seg_sort_kernel<kBigThreads, kBigCap, true>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBigSmem);
+        e = cudaFuncSetAttribute(seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, false, 2>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLargeSmem);
         if (e != cudaSuccess) return e;
         opted_in = true;
     }
 
-    // K1 / K2: a block owns a contiguous chunk of Gaussians
-    int blocks = (N + kBinThreads - 1) / kBinThreads;
-    if (blocks > num_sms * 4) blocks = num_sms * 4;
-    if (blocks < 1) blocks = 1;
-    const int chunk = (N + blocks - 1) / blocks;
-    const bool smem_hist = T <= kSmemTilesMax;
-    const size_t hist_bytes = smem_hist ? (size_t)T * 4 : 0;
-    if (smem_hist) {
-        bin_count_kernel<true><<<blocks, kBinThreads, hist_bytes, s>>>(N, chunk, cam.gx, T, splats, tile_select,
-            w.tile_count, tile_offsets, Pcap, P_dev, w.ctr, w.big_list, (uint32_t)kSmallCap);
-        bin_scatter_kernel<true><<<blocks, kBinThreads, hist_bytes, s>>>(N, chunk, cam.gx, T, splats, tile_select,
-            tile_offsets, w.cursor, P_dev, w.pairs);
-    } else {
-        bin_count_kernel<false><<<blocks, kBinThreads, 0, s>>>(N, chunk, cam.gx, T, splats, tile_select,
-            w.tile_count, tile_offsets, Pcap, P_dev, w.ctr, w.big_list, (uint32_t)kSmallCap);
-        bin_scatter_kernel<false><<<blocks, kBinThreads, 0, s>>>(N, chunk, cam.gx, T, splats, tile_select,
-            tile_offsets, w.cursor, P_dev, w.pairs);
-    }
-    count_launches(2);
+    // K0-K2: regroup the visible Gaussians by top-left tile
+    int nblk = (N + 255) / 256;
+    if (nblk > num_sms * 8) nblk = num_sms * 8;
+    if (nblk < 1) nblk = 1;
+    uint32_t* sat = tile_select ? w.sat : nullptr;
+    topleft_count_kernel<<<nblk, 256, 0, s>>>(N, gx, gy, splats, w.bin_count);
+    bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
+    reorder_kernel<<<nblk, 256, 0, s>>>(N, gx, gy, splats, w.bin_offset, w.bin_cursor, sat, w.rec);
+    // K3-K5: pair counts, CSR offsets, scatter
+    pair_walk_kernel<false><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, w.tile_count, nullptr, nullptr,
+                                                          P_dev, nullptr);
+    tile_scan_kernel<<<1, kScanThreads, 0, s>>>(T, w.tile_count, tile_offsets, Pcap, P_dev, w.ctr, w.small_list,
+                                                w.large_list, w.giant_list, (uint32_t)kSmallCap, (uint32_t)kLargeCap);
+    pair_walk_kernel<true><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, nullptr, tile_offsets, w.cursor,
+                                                         P_dev, w.pairs);
+    count_launches(6);
 
-    // K3: oversized segments first (1024-thread blocks), then everything else
+    // K6-K7: sort the segments; the large ones (and the pieces of the giant ones) first
     int gid_bits = 1;
     while (gid_bits < 30 && (1ll << gid_bits) < (long long)N) ++gid_bits;
-    if (Pcap > kSmallCap) {  // otherwise no segment can be oversized
-        int bb = num_sms < T ? num_sms : T;
-        seg_sort_kernel<kBigThreads, kBigCap, true><<<bb, kBigThreads, kBigSmem, s>>>(T, tile_offsets, w.pairs, w.tmp,
-            gid_sorted, keys_sorted, P_dev, w.ctr, w.big_list, (uint32_t)kSmallCap, gid_bits);
+    if (Pcap > kSmallCap) {  // otherwise every segment is small
+        if (Pcap > kLargeCap) {
+            int gb = num_sms < T ? num_sms : T;
+            giant_split_kernel<<<gb, kCoarseMax, 0, s>>>(w.giant_list, w.large_list, w.ctr, w.pairs, w.tmp, P_dev);
+            count_launches(1);
+        }
+        int lb = num_sms * 2 < T ? num_sms * 2 : T;
+        seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, false, 2><<<lb, kLargeThreads, kLargeSmem, s>>>(
+            w.large_list, &w.ctr->n_large, &w.ctr->sched_large, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
         count_launches(1);
     }
-    int sb = num_sms * 3;
-    if (sb > T) sb = T;
-    seg_sort_kernel<kSmallThreads, kSmallCap, false><<<sb, kSmallThreads, kSmallSmem, s>>>(T, tile_offsets, w.pairs,
-        w.tmp, gid_sorted, keys_sorted, P_dev, w.ctr, w.big_list, (uint32_t)kSmallCap, gid_bits);
+    int sb = num_sms * 6 < T ? num_sms * 6 : T;
+    seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4><<<sb, kSmallThreads, kSmallSmem, s>>>(
+        w.small_list, &w.ctr->n_small, &w.ctr->sched_small, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
     count_launches(1);
     return cudaGetLastError();
 }
