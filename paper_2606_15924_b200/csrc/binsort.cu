@@ -46,8 +46,10 @@ namespace {
 
 constexpr int kScanThreads = 1024;
 constexpr int kWalkThreads = 256;
+constexpr int kSmemTilesMax = 12288;     // top-left histogram kept in shared memory up to this many tiles (48 KB)
+constexpr int kRegroupBlocksMax = 160;   // blocks of K0 / K2 (one per SM)
 constexpr int kSmallW = 4, kSmallH = 4;  // rects up to this size go through the ballot window
-constexpr int kRounds = 12;              // write-then-check rounds before the atomic fallback
+constexpr int kRounds = 3;               // write-then-check rounds before the atomic fallback
 constexpr uint32_t kMaxOcc = 64;         // bucket occupancy above which a segment takes the radix fallback
 constexpr int kFbBits = 8;               // digit width of the fallback radix sort
 constexpr uint32_t kSubTarget = 2048;    // expected sub-segment size of a giant split
@@ -108,13 +110,34 @@ __device__ __forceinline__ void load_rect(const float4* __restrict__ splats, int
 }
 
 // ---- K0: histogram of the top-left tile ---------------------------------------------------------
-__global__ void __launch_bounds__(256)
-topleft_count_kernel(int N, int gx, int gy, const float4* __restrict__ splats, uint32_t* __restrict__ bin_count) {
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+// A block owns a contiguous chunk of Gaussians.  SMEM: the block counts into a private shared-memory
+// histogram (scattered global REDs are one L2 transaction each and ~5x slower), then adds its counts
+// to the global histogram with coalesced atomics whose RETURN value is the block's offset inside
+// every bin (blk_base[block][T]): K2 then needs no global atomic at all.
+template <bool SMEM>
+__global__ void __launch_bounds__(1024)
+topleft_count_kernel(int N, int chunk, int gx, int gy, const float4* __restrict__ splats,
+                     uint32_t* __restrict__ bin_count, uint32_t* __restrict__ blk_base) {
+    extern __shared__ __align__(16) uint32_t hist[];  // [T] when SMEM
+    const int T = gx * gy;
+    const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
+    if (SMEM) {
+        for (int t = threadIdx.x; t < T; t += blockDim.x) hist[t] = 0u;
+        __syncthreads();
+    }
+    for (int i = begin + (int)threadIdx.x; i < end; i += blockDim.x) {
         int x0, y0, x1, y1;
         uint32_t d;
         load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
-        if (x1 > x0 && y1 > y0) atomicAdd(&bin_count[y0 * gx + x0], 1u);
+        if (x1 > x0 && y1 > y0) atomicAdd(SMEM ? &hist[y0 * gx + x0] : &bin_count[y0 * gx + x0], 1u);
+    }
+    if (SMEM) {
+        __syncthreads();
+        uint32_t* mine = blk_base + (size_t)blockIdx.x * T;
+        for (int t = threadIdx.x; t < T; t += blockDim.x) {
+            const uint32_t c = hist[t];
+            mine[t] = c ? atomicAdd(&bin_count[t], c) : 0u;
+        }
     }
 }
 
@@ -176,11 +199,20 @@ bin_scan_kernel(int gx, int gy, const uint32_t* __restrict__ bin_count, uint32_t
 }
 
 // ---- K2: records grouped by top-left tile -----------------------------------------------------------
-__global__ void __launch_bounds__(256)
-reorder_kernel(int N, int gx, int gy, const float4* __restrict__ splats, const uint32_t* __restrict__ bin_offset,
-               uint32_t* __restrict__ bin_cursor, const uint32_t* __restrict__ sat, uint4* __restrict__ rec) {
-    const int sx = gx + 1;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+template <bool SMEM>
+__global__ void __launch_bounds__(1024)
+reorder_kernel(int N, int chunk, int gx, int gy, const float4* __restrict__ splats,
+               const uint32_t* __restrict__ bin_offset, uint32_t* __restrict__ bin_cursor,
+               const uint32_t* __restrict__ blk_base, const uint32_t* __restrict__ sat, uint4* __restrict__ rec) {
+    extern __shared__ __align__(16) uint32_t cur[];  // [T] when SMEM: this block's next slot in every bin
+    const int T = gx * gy, sx = gx + 1;
+    const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
+    if (SMEM) {
+        const uint32_t* mine = blk_base + (size_t)blockIdx.x * T;
+        for (int t = threadIdx.x; t < T; t += blockDim.x) cur[t] = bin_offset[t] + mine[t];
+        __syncthreads();
+    }
+    for (int i = begin + (int)threadIdx.x; i < end; i += blockDim.x) {
         int x0, y0, x1, y1;
         uint32_t d;
         load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
@@ -192,7 +224,7 @@ reorder_kernel(int N, int gx, int gy, const float4* __restrict__ splats, const u
             dead = n_sel == 0u;
         }
         const int t0 = y0 * gx + x0;
-        const uint32_t slot = bin_offset[t0] + atomicAdd(&bin_cursor[t0], 1u);
+        const uint32_t slot = SMEM ? atomicAdd(&cur[t0], 1u) : bin_offset[t0] + atomicAdd(&bin_cursor[t0], 1u);
         const uint32_t rx = dead ? 0u : ((uint32_t)x0 | ((uint32_t)x1 << 16));
         const uint32_t ry = dead ? 0u : ((uint32_t)y0 | ((uint32_t)y1 << 16));
         rec[slot] = make_uint4(d, (uint32_t)i, rx, ry);
@@ -232,6 +264,45 @@ pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restri
             const int X1 = __reduce_max_sync(0xffffffffu, in ? x1 : 0);
             const int Hw = __reduce_max_sync(0xffffffffu, in ? h : 0);
             const int Ww = X1 - X0, win = Ww * Hw;
+            if (win <= 32) {
+                // ---- fast path: the whole window fits one 32-bit mask per lane ----
+                uint32_t cover = 0;  // bit c = this lane's rect covers window tile c (row-major, Ww wide)
+                if (in) {
+                    const uint32_t rowmask = ((1u << w) - 1u) << (x0 - X0);
+#pragma unroll
+                    for (int rr = 0; rr < kSmallH; ++rr)
+                        if (rr < h) cover |= rowmask << (rr * Ww);
+                }
+                uint32_t mine = 0;  // lane j: the lanes whose rect covers window tile j
+                for (int j = 0; j < win; ++j) {
+                    const uint32_t bal = __ballot_sync(0xffffffffu, (cover >> j) & 1u);
+                    if (lane == j) mine = bal;
+                }
+                int ty = 0, tx = lane;  // lane's own window tile (win <= 32: at most 4 rows)
+#pragma unroll
+                for (int rr = 1; rr < kSmallH; ++rr)
+                    if (lane >= rr * Ww) { ty = rr; tx = lane - rr * Ww; }
+                const uint32_t t = (uint32_t)((row + ty) * gx + X0 + tx);
+                bool has = lane < win && mine != 0u;
+                if (has && tile_select != nullptr && tile_select[t] == 0u) has = false;
+                if (!SCATTER) {
+                    if (has) atomicAdd(&tile_count[t], (uint32_t)__popc(mine));
+                } else {
+                    uint32_t b = 0xffffffffu;
+                    if (has) b = tile_offsets[t] + atomicAdd(&cursor[t], (uint32_t)__popc(mine));
+                    // every lane walks ITS covered tiles; the run base and the covering mask come from the tile's lane
+                    const int most = __reduce_max_sync(0xffffffffu, __popc(cover));
+                    uint32_t left = cover;
+                    for (int q = 0; q < most; ++q) {
+                        const int j = left ? __ffs(left) - 1 : 0;
+                        const uint32_t mj = __shfl_sync(0xffffffffu, mine, j);
+                        const uint32_t bj = __shfl_sync(0xffffffffu, b, j);
+                        if (left && bj != 0xffffffffu) pairs[bj + (uint32_t)__popc(mj & lt_mask)] = make_uint2(r.x, r.y);
+                        left &= left - 1u;
+                    }
+                }
+                continue;
+            }
             for (int c0 = 0; c0 < win; c0 += 32) {
                 const int cnt = min(32, win - c0);
                 int tyj = row + c0 / Ww, txj = X0 + c0 % Ww;
@@ -506,12 +577,14 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
         uint2* src = (sg.in_tmp ? tmp : pairs) + sg.start;
         uint2* oth = (sg.in_tmp ? pairs : tmp) + sg.start;
         const uint32_t m = sg.len;
+        const int nE = (int)((m + THREADS - 1u) / THREADS);  // element slots in use per thread
         bool fb = m > (uint32_t)CAP;  // block-uniform from here on
         uint2 kv[KEEP ? EPT : 1];
         uint32_t lo = 0xffffffffu, hi = 0u;
         if (!fb) {
 #pragma unroll
             for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                 const uint32_t i = (uint32_t)e * THREADS + tid;
                 if (i < m) {
                     const uint2 v = src[i];
@@ -542,6 +615,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
             uint32_t st[EPT];
 #pragma unroll
             for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                 const uint32_t i = (uint32_t)e * THREADS + tid;
                 st[e] = 0xffffffffu;
                 if (i < m) st[e] = (bucket_of(KEEP ? kv[KEEP ? e : 0].x : src[i].x, lo, scale, nb) << 16) | 0xffffu;
@@ -552,6 +626,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
                 bool any = false;
 #pragma unroll
                 for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                     if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
                         tab[st[e] >> 16] = (uint16_t)((uint32_t)e * THREADS + tid);
                         any = true;
@@ -560,6 +635,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
                 if (!__syncthreads_or(any)) break;
 #pragma unroll
                 for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                     if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
                         const uint32_t b = st[e] >> 16;
                         if (tab[b] == (uint16_t)((uint32_t)e * THREADS + tid)) {
@@ -573,6 +649,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
             // crowded buckets: the elements still pending take their slots with atomics
 #pragma unroll
             for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                 if (st[e] != 0xffffffffu && (st[e] & 0xffffu) == 0xffffu) {
                     const uint32_t b = st[e] >> 16;
                     st[e] = (b << 16) | min(0xfffeu, atomicAdd(&sm.cnt[b], 1u));
@@ -608,6 +685,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
                 // ---- place by bucket, then order every bucket by counting smaller (depth, id) ----
 #pragma unroll
                 for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                     if (st[e] != 0xffffffffu) {
                         const uint2 v = KEEP ? kv[KEEP ? e : 0] : src[(uint32_t)e * THREADS + tid];
                         sm.u.B[sm.cnt[st[e] >> 16] + (st[e] & 0xffffu)] = v;
@@ -616,6 +694,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
                 __syncthreads();
 #pragma unroll
                 for (int e = 0; e < EPT; ++e) {
+                if (e >= nE) break;  // block-uniform
                     const uint32_t i = (uint32_t)e * THREADS + tid;
                     if (i < m) {
                         const uint2 v = sm.u.B[i];
@@ -668,7 +747,7 @@ struct Workspace {
     Counters* ctr;
     uint32_t *bin_count, *bin_cursor, *tile_count, *cursor;
     size_t zero_bytes;
-    uint32_t *bin_offset, *sat;
+    uint32_t *bin_offset, *sat, *blk_base;     // blk_base: [regroup blocks][T] when the tile histogram fits shared memory
     uint4* rec;                                // [N] regrouped records
     Seg *small_list, *large_list, *giant_list;
     uint2 *pairs, *tmp;                        // [Pcap] each: unsorted segments; scratch of giant_split / the fallback
@@ -689,6 +768,7 @@ Workspace carve(void* base, int N, int T_, int64_t Pcap) {
     w.zero_bytes = o;
     w.bin_offset = (uint32_t*)take(nt * 4);
     w.sat = (uint32_t*)take((2 * nt + 2) * 4);  // (gx+1)(gy+1) <= 2T+2
+    w.blk_base = (uint32_t*)take(nt <= (size_t)kSmemTilesMax ? (size_t)kRegroupBlocksMax * nt * 4 : 4);
     w.rec = (uint4*)take(nn * 16);
     w.small_list = (Seg*)take(nt * sizeof(Seg));
     w.large_list = (Seg*)take((2 * nt + pc / kSubTarget + 16) * sizeof(Seg));
@@ -729,9 +809,21 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
     if (nblk > num_sms * 8) nblk = num_sms * 8;
     if (nblk < 1) nblk = 1;
     uint32_t* sat = tile_select ? w.sat : nullptr;
-    topleft_count_kernel<<<nblk, 256, 0, s>>>(N, gx, gy, splats, w.bin_count);
-    bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
-    reorder_kernel<<<nblk, 256, 0, s>>>(N, gx, gy, splats, w.bin_offset, w.bin_cursor, sat, w.rec);
+    if (T <= kSmemTilesMax) {
+        int rb = num_sms < kRegroupBlocksMax ? num_sms : kRegroupBlocksMax;
+        if (rb > (N + 1023) / 1024) rb = (N + 1023) / 1024;
+        if (rb < 1) rb = 1;
+        const int chunk = (N + rb - 1) / rb;
+        const size_t hb = (size_t)T * 4;
+        topleft_count_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, w.bin_count, w.blk_base);
+        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
+        reorder_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, w.blk_base, sat, w.rec);
+    } else {
+        const int chunk = (N + nblk - 1) / nblk;
+        topleft_count_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, w.bin_count, nullptr);
+        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
+        reorder_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, nullptr, sat, w.rec);
+    }
     // K3-K5: pair counts, CSR offsets, scatter
     pair_walk_kernel<false><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, w.tile_count, nullptr, nullptr,
                                                           P_dev, nullptr);
