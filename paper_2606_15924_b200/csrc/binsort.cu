@@ -57,10 +57,11 @@ constexpr int kCoarseMax = 1024;         // sub-segments per giant tile (one per
 
 // zeroed words at the head of the workspace
 struct Counters {
-    uint32_t n_vis;                       // visible Gaussians (records written by K2)
+    uint32_t n_vis;                       // records written by K2 (rects of at most 4x4 tiles)
     uint32_t n_small, n_large, n_giant;   // lengths of the work lists
     uint32_t sched_small, sched_large, sched_giant;  // work tickets
     uint32_t pad;
+    unsigned long long p_total;           // P, known after K0 (sum of the records' selected tiles)
 };
 
 struct Seg {            // one unit of sort work
@@ -109,6 +110,24 @@ __device__ __forceinline__ void load_rect(const float4* __restrict__ splats, int
     dbits = __float_as_uint(r2.y);
 }
 
+// Selected tiles inside [x0,x1) x [y0,y1): from the summed-area table, or the area when every tile counts.
+__device__ __forceinline__ uint32_t rect_pairs(const uint32_t* __restrict__ sat, int sx, int x0, int y0, int x1, int y1) {
+    if (sat == nullptr) return (uint32_t)((x1 - x0) * (y1 - y0));
+    return sat[(size_t)y1 * sx + x1] - sat[(size_t)y0 * sx + x1] - sat[(size_t)y1 * sx + x0] + sat[(size_t)y0 * sx + x0];
+}
+
+// A rect is cut into pieces of at most kSmallW x kSmallH tiles; f(px0, py0, px1, py1, pairs) is called
+// for every piece that holds a selected tile.  (Most rects are one piece.)
+template <class F>
+__device__ __forceinline__ void for_each_piece(const uint32_t* __restrict__ sat, int gx, int x0, int y0, int x1, int y1, F f) {
+    for (int py = y0; py < y1; py += kSmallH)
+        for (int px = x0; px < x1; px += kSmallW) {
+            const int qx = min(px + kSmallW, x1), qy = min(py + kSmallH, y1);
+            const uint32_t np = rect_pairs(sat, gx + 1, px, py, qx, qy);
+            if (np) f(px, py, qx, qy, np);
+        }
+}
+
 // ---- K0: histogram of the top-left tile ---------------------------------------------------------
 // A block owns a contiguous chunk of Gaussians.  SMEM: the block counts into a private shared-memory
 // histogram (scattered global REDs are one L2 transaction each and ~5x slower), then adds its counts
@@ -117,22 +136,33 @@ __device__ __forceinline__ void load_rect(const float4* __restrict__ splats, int
 template <bool SMEM>
 __global__ void __launch_bounds__(1024)
 topleft_count_kernel(int N, int chunk, int gx, int gy, const float4* __restrict__ splats,
-                     uint32_t* __restrict__ bin_count, uint32_t* __restrict__ blk_base) {
+                     const uint32_t* __restrict__ sat, uint32_t* __restrict__ bin_count,
+                     uint32_t* __restrict__ blk_base, Counters* __restrict__ ctr) {
     extern __shared__ __align__(16) uint32_t hist[];  // [T] when SMEM
+    __shared__ unsigned long long s_pairs;
     const int T = gx * gy;
     const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
-    if (SMEM) {
+    if (threadIdx.x == 0) s_pairs = 0ull;
+    if (SMEM)
         for (int t = threadIdx.x; t < T; t += blockDim.x) hist[t] = 0u;
-        __syncthreads();
-    }
+    __syncthreads();
+    unsigned long long pairs = 0ull;
     for (int i = begin + (int)threadIdx.x; i < end; i += blockDim.x) {
         int x0, y0, x1, y1;
         uint32_t d;
         load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
-        if (x1 > x0 && y1 > y0) atomicAdd(SMEM ? &hist[y0 * gx + x0] : &bin_count[y0 * gx + x0], 1u);
+        for_each_piece(sat, gx, x0, y0, x1, y1, [&](int px, int py, int, int, uint32_t np) {
+            atomicAdd(SMEM ? &hist[py * gx + px] : &bin_count[py * gx + px], 1u);
+            pairs += np;
+        });
     }
+    // P = sum of the pieces' selected tiles: one 64-bit atomic per block
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) pairs += __shfl_xor_sync(0xffffffffu, pairs, o);
+    if ((threadIdx.x & 31) == 0 && pairs) atomicAdd(&s_pairs, pairs);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_pairs) atomicAdd(&ctr->p_total, s_pairs);
     if (SMEM) {
-        __syncthreads();
         uint32_t* mine = blk_base + (size_t)blockIdx.x * T;
         for (int t = threadIdx.x; t < T; t += blockDim.x) {
             const uint32_t c = hist[t];
@@ -141,39 +171,11 @@ topleft_count_kernel(int N, int chunk, int gx, int gy, const float4* __restrict_
     }
 }
 
-// ---- K1: scan of the top-left histogram; summed-area table of tile_select -----------------------
+// ---- Ks: summed-area table of tile_select (one block; only when a selection is given) -----------
 // sat[(gy+1) x (gx+1)]: sat[y][x] = number of selected tiles with ty < y and tx < x.
 __global__ void __launch_bounds__(kScanThreads)
-bin_scan_kernel(int gx, int gy, const uint32_t* __restrict__ bin_count, uint32_t* __restrict__ bin_offset,
-                const uint32_t* __restrict__ tile_select, uint32_t* sat, Counters* __restrict__ ctr) {
-    __shared__ uint32_t ws[33];
-    __shared__ uint32_t s_carry;
-    const int T = gx * gy;
-    if (threadIdx.x == 0) s_carry = 0u;
-    __syncthreads();
-    constexpr int kPer = 4;
-    for (int b0 = 0; b0 < T; b0 += kScanThreads * kPer) {
-        const int t0 = b0 + (int)threadIdx.x * kPer;
-        uint32_t c[kPer], sum = 0;
-#pragma unroll
-        for (int j = 0; j < kPer; ++j) {
-            c[j] = (t0 + j < T) ? bin_count[t0 + j] : 0u;
-            sum += c[j];
-        }
-        uint32_t tot;
-        uint32_t run = s_carry + block_excl_scan(sum, ws, tot);
-#pragma unroll
-        for (int j = 0; j < kPer; ++j) {
-            if (t0 + j < T) bin_offset[t0 + j] = run;
-            run += c[j];
-        }
-        __syncthreads();
-        if (threadIdx.x == 0) s_carry += tot;
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) ctr->n_vis = s_carry;
-    if (tile_select == nullptr) return;
-    // summed-area table: row prefixes (a warp per row), then column sums (a thread per column)
+select_sat_kernel(int gx, int gy, const uint32_t* __restrict__ tile_select, uint32_t* sat) {
+    // row prefixes (a warp per row), then column sums (a thread per column)
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, sx = gx + 1;
     for (int x = threadIdx.x; x <= gx; x += kScanThreads) sat[x] = 0u;
     for (int y = warp; y < gy; y += kScanThreads / 32) {
@@ -198,14 +200,53 @@ bin_scan_kernel(int gx, int gy, const uint32_t* __restrict__ bin_count, uint32_t
     }
 }
 
+// ---- K1: scan of the top-left histogram; P and the capacity flag -----------------------------------
+__global__ void __launch_bounds__(kScanThreads)
+bin_scan_kernel(int T, const uint32_t* __restrict__ bin_count, uint32_t* __restrict__ bin_offset,
+                Counters* __restrict__ ctr, int64_t Pcap, int64_t* __restrict__ P_dev) {
+    __shared__ uint32_t ws[33];
+    __shared__ uint32_t s_carry;
+    if (threadIdx.x == 0) s_carry = 0u;
+    __syncthreads();
+    constexpr int kPer = 4;
+    for (int b0 = 0; b0 < T; b0 += kScanThreads * kPer) {
+        const int t0 = b0 + (int)threadIdx.x * kPer;
+        uint32_t c[kPer], sum = 0;
+#pragma unroll
+        for (int j = 0; j < kPer; ++j) {
+            c[j] = (t0 + j < T) ? bin_count[t0 + j] : 0u;
+            sum += c[j];
+        }
+        uint32_t tot;
+        uint32_t run = s_carry + block_excl_scan(sum, ws, tot);
+#pragma unroll
+        for (int j = 0; j < kPer; ++j) {
+            if (t0 + j < T) bin_offset[t0 + j] = run;
+            run += c[j];
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry += tot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        // every record holds at least one pair, so records <= P <= Pcap whenever the call can proceed
+        const unsigned long long P = ctr->p_total;
+        ctr->n_vis = s_carry;
+        P_dev[0] = (int64_t)P;
+        P_dev[1] = ((int64_t)P > Pcap) ? 1 : 0;
+    }
+}
+
 // ---- K2: records grouped by top-left tile -----------------------------------------------------------
 template <bool SMEM>
 __global__ void __launch_bounds__(1024)
 reorder_kernel(int N, int chunk, int gx, int gy, const float4* __restrict__ splats,
                const uint32_t* __restrict__ bin_offset, uint32_t* __restrict__ bin_cursor,
-               const uint32_t* __restrict__ blk_base, const uint32_t* __restrict__ sat, uint4* __restrict__ rec) {
+               const uint32_t* __restrict__ blk_base, const uint32_t* __restrict__ sat,
+               const int64_t* __restrict__ P_dev, uint4* __restrict__ rec) {
     extern __shared__ __align__(16) uint32_t cur[];  // [T] when SMEM: this block's next slot in every bin
-    const int T = gx * gy, sx = gx + 1;
+    if (P_dev[1]) return;  // over capacity (the record buffer holds P_capacity records)
+    const int T = gx * gy;
     const int begin = min(N, (int)blockIdx.x * chunk), end = min(N, begin + chunk);
     if (SMEM) {
         const uint32_t* mine = blk_base + (size_t)blockIdx.x * T;
@@ -216,18 +257,11 @@ reorder_kernel(int N, int chunk, int gx, int gy, const float4* __restrict__ spla
         int x0, y0, x1, y1;
         uint32_t d;
         load_rect(splats, i, gx, gy, x0, y0, x1, y1, d);
-        if (x1 <= x0 || y1 <= y0) continue;
-        bool dead = false;
-        if (sat != nullptr) {
-            const uint32_t n_sel = sat[(size_t)y1 * sx + x1] - sat[(size_t)y0 * sx + x1] - sat[(size_t)y1 * sx + x0] +
-                                   sat[(size_t)y0 * sx + x0];
-            dead = n_sel == 0u;
-        }
-        const int t0 = y0 * gx + x0;
-        const uint32_t slot = SMEM ? atomicAdd(&cur[t0], 1u) : bin_offset[t0] + atomicAdd(&bin_cursor[t0], 1u);
-        const uint32_t rx = dead ? 0u : ((uint32_t)x0 | ((uint32_t)x1 << 16));
-        const uint32_t ry = dead ? 0u : ((uint32_t)y0 | ((uint32_t)y1 << 16));
-        rec[slot] = make_uint4(d, (uint32_t)i, rx, ry);
+        for_each_piece(sat, gx, x0, y0, x1, y1, [&](int px, int py, int qx, int qy, uint32_t) {
+            const int t0 = py * gx + px;
+            const uint32_t slot = SMEM ? atomicAdd(&cur[t0], 1u) : bin_offset[t0] + atomicAdd(&bin_cursor[t0], 1u);
+            rec[slot] = make_uint4(d, (uint32_t)i, (uint32_t)px | ((uint32_t)qx << 16), (uint32_t)py | ((uint32_t)qy << 16));
+        });
     }
 }
 
@@ -240,7 +274,7 @@ pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restri
                  const uint32_t* __restrict__ tile_select, uint32_t* __restrict__ tile_count,
                  const uint32_t* __restrict__ tile_offsets, uint32_t* __restrict__ cursor,
                  const int64_t* __restrict__ P_dev, uint2* __restrict__ pairs) {
-    if (SCATTER && P_dev[1]) return;  // over capacity: nothing is written
+    if (P_dev[1]) return;  // over capacity: nothing is written
     const uint32_t n = ctr->n_vis;
     const int lane = threadIdx.x & 31;
     const uint32_t lt_mask = (1u << lane) - 1u;
@@ -253,7 +287,7 @@ pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restri
         unpack_rect(r.z, r.w, x0, y0, x1, y1);
         const int w = x1 - x0, h = y1 - y0;
         const bool live = w > 0 && h > 0;
-        const bool small = live && w <= kSmallW && h <= kSmallH;
+        const bool small = live;  // K2 cuts every rect into pieces of at most kSmallW x kSmallH tiles
         // ---- small rects: lanes with the same top row share a window of tiles ----
         uint32_t todo = __ballot_sync(0xffffffffu, small);
         while (todo) {
@@ -333,25 +367,6 @@ pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restri
                 }
             }
         }
-        // ---- wide rects: the whole warp walks one rect, one atomic per pair ----
-        uint32_t big = __ballot_sync(0xffffffffu, live && !small);
-        while (big) {
-            const int src = __ffs(big) - 1;
-            big &= big - 1u;
-            const int bx0 = __shfl_sync(0xffffffffu, x0, src), by0 = __shfl_sync(0xffffffffu, y0, src);
-            const int bw = __shfl_sync(0xffffffffu, w, src), ba = bw * __shfl_sync(0xffffffffu, h, src);
-            const uint32_t bd = __shfl_sync(0xffffffffu, r.x, src), bg = __shfl_sync(0xffffffffu, r.y, src);
-            for (int j = lane; j < ba; j += 32) {
-                const uint32_t t = (uint32_t)((by0 + j / bw) * gx + bx0 + j % bw);
-                if (tile_select != nullptr && tile_select[t] == 0u) continue;
-                if (!SCATTER) {
-                    atomicAdd(&tile_count[t], 1u);
-                } else {
-                    const uint32_t slot = tile_offsets[t] + atomicAdd(&cursor[t], 1u);
-                    pairs[slot] = make_uint2(bd, bg);
-                }
-            }
-        }
     }
 }
 
@@ -399,8 +414,8 @@ tile_scan_kernel(int T, const uint32_t* __restrict__ tile_count, uint32_t* __res
     if (threadIdx.x == 0) {
         const unsigned long long P = s_carry;
         tile_offsets[T] = (uint32_t)(P < (1ull << 32) ? P : 0xffffffffull);
-        P_dev[0] = (int64_t)P;
-        P_dev[1] = ((int64_t)P > Pcap) ? 1 : 0;
+        (void)Pcap;  // P and the capacity flag were published by K1 (over capacity, K3 counted nothing)
+        (void)P_dev;
     }
 }
 
@@ -769,7 +784,7 @@ Workspace carve(void* base, int N, int T_, int64_t Pcap) {
     w.bin_offset = (uint32_t*)take(nt * 4);
     w.sat = (uint32_t*)take((2 * nt + 2) * 4);  // (gx+1)(gy+1) <= 2T+2
     w.blk_base = (uint32_t*)take(nt <= (size_t)kSmemTilesMax ? (size_t)kRegroupBlocksMax * nt * 4 : 4);
-    w.rec = (uint4*)take(nn * 16);
+    w.rec = (uint4*)take(pc * 16);  // every record holds at least one pair: records <= P <= Pcap
     w.small_list = (Seg*)take(nt * sizeof(Seg));
     w.large_list = (Seg*)take((2 * nt + pc / kSubTarget + 16) * sizeof(Seg));
     w.giant_list = (Seg*)take(nt * sizeof(Seg));
@@ -804,25 +819,32 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
         opted_in = true;
     }
 
-    // K0-K2: regroup the visible Gaussians by top-left tile
+    // Ks, K0-K2: cut the rects into pieces and regroup them by top-left tile
     int nblk = (N + 255) / 256;
     if (nblk > num_sms * 8) nblk = num_sms * 8;
     if (nblk < 1) nblk = 1;
-    uint32_t* sat = tile_select ? w.sat : nullptr;
+    uint32_t* sat = nullptr;
+    if (tile_select) {
+        sat = w.sat;
+        select_sat_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, tile_select, sat);
+        count_launches(1);
+    }
     if (T <= kSmemTilesMax) {
         int rb = num_sms < kRegroupBlocksMax ? num_sms : kRegroupBlocksMax;
         if (rb > (N + 1023) / 1024) rb = (N + 1023) / 1024;
         if (rb < 1) rb = 1;
         const int chunk = (N + rb - 1) / rb;
         const size_t hb = (size_t)T * 4;
-        topleft_count_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, w.bin_count, w.blk_base);
-        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
-        reorder_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, w.blk_base, sat, w.rec);
+        topleft_count_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, sat, w.bin_count, w.blk_base, w.ctr);
+        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(T, w.bin_count, w.bin_offset, w.ctr, Pcap, P_dev);
+        reorder_kernel<true><<<rb, 1024, hb, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, w.blk_base, sat,
+                                                   P_dev, w.rec);
     } else {
         const int chunk = (N + nblk - 1) / nblk;
-        topleft_count_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, w.bin_count, nullptr);
-        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(gx, gy, w.bin_count, w.bin_offset, tile_select, w.sat, w.ctr);
-        reorder_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, nullptr, sat, w.rec);
+        topleft_count_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, sat, w.bin_count, nullptr, w.ctr);
+        bin_scan_kernel<<<1, kScanThreads, 0, s>>>(T, w.bin_count, w.bin_offset, w.ctr, Pcap, P_dev);
+        reorder_kernel<false><<<nblk, 256, 0, s>>>(N, chunk, gx, gy, splats, w.bin_offset, w.bin_cursor, nullptr, sat,
+                                                    P_dev, w.rec);
     }
     // K3-K5: pair counts, CSR offsets, scatter
     pair_walk_kernel<false><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, w.tile_count, nullptr, nullptr,
