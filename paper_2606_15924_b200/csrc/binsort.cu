@@ -49,7 +49,7 @@ constexpr int kWalkThreads = 256;
 constexpr int kSmemTilesMax = 12288;     // top-left histogram kept in shared memory up to this many tiles (48 KB)
 constexpr int kRegroupBlocksMax = 160;   // blocks of K0 / K2 (one per SM)
 constexpr int kSmallW = 4, kSmallH = 4;  // rects up to this size go through the ballot window
-constexpr int kRounds = 3;               // write-then-check rounds before the atomic fallback
+constexpr int kRounds = 1;               // write-then-check rounds before the atomic fallback
 constexpr uint32_t kMaxOcc = 64;         // bucket occupancy above which a segment takes the radix fallback
 constexpr int kFbBits = 8;               // digit width of the fallback radix sort
 constexpr uint32_t kSubTarget = 2048;    // expected sub-segment size of a giant split
@@ -58,9 +58,9 @@ constexpr int kCoarseMax = 1024;         // sub-segments per giant tile (one per
 // zeroed words at the head of the workspace
 struct Counters {
     uint32_t n_vis;                       // records written by K2 (rects of at most 4x4 tiles)
-    uint32_t n_small, n_large, n_giant;   // lengths of the work lists
-    uint32_t sched_small, sched_large, sched_giant;  // work tickets
-    uint32_t pad;
+    uint32_t n_small, n_medium, n_large, n_giant;   // lengths of the work lists
+    uint32_t sched_small, sched_medium, sched_large, sched_giant;  // work tickets
+    uint32_t pad[3];
     unsigned long long p_total;           // P, known after K0 (sum of the records' selected tiles)
 };
 
@@ -374,7 +374,8 @@ pair_walk_kernel(int gx, const uint4* __restrict__ rec, const Counters* __restri
 __global__ void __launch_bounds__(kScanThreads)
 tile_scan_kernel(int T, const uint32_t* __restrict__ tile_count, uint32_t* __restrict__ tile_offsets, int64_t Pcap,
                  int64_t* __restrict__ P_dev, Counters* __restrict__ ctr, Seg* __restrict__ small_list,
-                 Seg* __restrict__ large_list, Seg* __restrict__ giant_list, uint32_t small_cap, uint32_t large_cap) {
+                 Seg* __restrict__ medium_list, Seg* __restrict__ large_list, Seg* __restrict__ giant_list,
+                 uint32_t small_cap, uint32_t medium_cap, uint32_t large_cap) {
     __shared__ uint32_t ws[33];
     __shared__ unsigned long long s_carry;
     if (threadIdx.x == 0) s_carry = 0ull;
@@ -401,6 +402,7 @@ tile_scan_kernel(int T, const uint32_t* __restrict__ tile_count, uint32_t* __res
                     Seg sg;
                     sg.start = st; sg.len = c[j]; sg.tile = (uint32_t)(t0 + j); sg.in_tmp = 0u;
                     if (c[j] <= small_cap) small_list[atomicAdd(&ctr->n_small, 1u)] = sg;
+                    else if (c[j] <= medium_cap) medium_list[atomicAdd(&ctr->n_medium, 1u)] = sg;
                     else if (c[j] <= large_cap) large_list[atomicAdd(&ctr->n_large, 1u)] = sg;
                     else giant_list[atomicAdd(&ctr->n_giant, 1u)] = sg;
                 }
@@ -555,7 +557,9 @@ __device__ __forceinline__ void radix_pass(const uint2* src, uint2* dst, uint32_
 }
 
 // ---- K7: per-segment sort -----------------------------------------------------------------------------
-__device__ __forceinline__ bool pair_less(const uint2 a, const uint2 b) { return a.x < b.x || (a.x == b.x && a.y < b.y); }
+__device__ __forceinline__ bool pair_less(const uint2 a, const uint2 b) {
+    return (((unsigned long long)a.x << 32) | a.y) < (((unsigned long long)b.x << 32) | b.y);
+}
 
 template <int CAP, int NBMAX>
 struct SortSmem {
@@ -751,8 +755,10 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
 }
 
 constexpr int kSmallThreads = 256, kSmallCap = 2048, kSmallNb = 4096;
-constexpr int kLargeThreads = 512, kLargeCap = 8192, kLargeNb = 8192;
+constexpr int kMediumThreads = 512, kMediumCap = 4096, kMediumNb = 8192;
+constexpr int kLargeThreads = 1024, kLargeCap = 8192, kLargeNb = 8192;
 constexpr size_t kSmallSmem = sizeof(SortSmem<kSmallCap, kSmallNb>);
+constexpr size_t kMediumSmem = sizeof(SortSmem<kMediumCap, kMediumNb>);
 constexpr size_t kLargeSmem = sizeof(SortSmem<kLargeCap, kLargeNb>);
 
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -764,7 +770,7 @@ struct Workspace {
     size_t zero_bytes;
     uint32_t *bin_offset, *sat, *blk_base;     // blk_base: [regroup blocks][T] when the tile histogram fits shared memory
     uint4* rec;                                // [N] regrouped records
-    Seg *small_list, *large_list, *giant_list;
+    Seg *small_list, *medium_list, *large_list, *giant_list;
     uint2 *pairs, *tmp;                        // [Pcap] each: unsorted segments; scratch of giant_split / the fallback
     size_t total;
 };
@@ -786,6 +792,7 @@ Workspace carve(void* base, int N, int T_, int64_t Pcap) {
     w.blk_base = (uint32_t*)take(nt <= (size_t)kSmemTilesMax ? (size_t)kRegroupBlocksMax * nt * 4 : 4);
     w.rec = (uint4*)take(pc * 16);  // every record holds at least one pair: records <= P <= Pcap
     w.small_list = (Seg*)take(nt * sizeof(Seg));
+    w.medium_list = (Seg*)take(nt * sizeof(Seg));
     w.large_list = (Seg*)take((2 * nt + pc / kSubTarget + 16) * sizeof(Seg));
     w.giant_list = (Seg*)take(nt * sizeof(Seg));
     w.pairs = (uint2*)take(pc * 8);
@@ -813,7 +820,10 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
         e = cudaFuncSetAttribute(seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmallSmem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, false, 2>,
+        e = cudaFuncSetAttribute(seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMediumSmem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1>,
                                  cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLargeSmem);
         if (e != cudaSuccess) return e;
         opted_in = true;
@@ -850,7 +860,8 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
     pair_walk_kernel<false><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, w.tile_count, nullptr, nullptr,
                                                           P_dev, nullptr);
     tile_scan_kernel<<<1, kScanThreads, 0, s>>>(T, w.tile_count, tile_offsets, Pcap, P_dev, w.ctr, w.small_list,
-                                                w.large_list, w.giant_list, (uint32_t)kSmallCap, (uint32_t)kLargeCap);
+                                                w.medium_list, w.large_list, w.giant_list, (uint32_t)kSmallCap,
+                                                (uint32_t)kMediumCap, (uint32_t)kLargeCap);
     pair_walk_kernel<true><<<nblk, kWalkThreads, 0, s>>>(gx, w.rec, w.ctr, tile_select, nullptr, tile_offsets, w.cursor,
                                                          P_dev, w.pairs);
     count_launches(6);
@@ -858,15 +869,21 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
     // K6-K7: sort the segments; the large ones (and the pieces of the giant ones) first
     int gid_bits = 1;
     while (gid_bits < 30 && (1ll << gid_bits) < (long long)N) ++gid_bits;
-    if (Pcap > kSmallCap) {  // otherwise every segment is small
+    if (Pcap > kMediumCap) {  // otherwise no segment is that long
         if (Pcap > kLargeCap) {
             int gb = num_sms < T ? num_sms : T;
             giant_split_kernel<<<gb, kCoarseMax, 0, s>>>(w.giant_list, w.large_list, w.ctr, w.pairs, w.tmp, P_dev);
             count_launches(1);
         }
-        int lb = num_sms * 2 < T ? num_sms * 2 : T;
-        seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, false, 2><<<lb, kLargeThreads, kLargeSmem, s>>>(
+        int lb = num_sms < T ? num_sms : T;
+        seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1><<<lb, kLargeThreads, kLargeSmem, s>>>(
             w.large_list, &w.ctr->n_large, &w.ctr->sched_large, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
+        count_launches(1);
+    }
+    if (Pcap > kSmallCap) {
+        int mb = num_sms * 2 < T ? num_sms * 2 : T;
+        seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2><<<mb, kMediumThreads, kMediumSmem, s>>>(
+            w.medium_list, &w.ctr->n_medium, &w.ctr->sched_medium, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
         count_launches(1);
     }
     int sb = num_sms * 6 < T ? num_sms * 6 : T;
