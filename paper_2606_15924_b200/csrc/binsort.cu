@@ -50,7 +50,7 @@ constexpr int kSmemTilesMax = 12288;     // top-left histogram kept in shared me
 constexpr int kRegroupBlocksMax = 160;   // blocks of K0 / K2 (one per SM)
 constexpr int kSmallW = 4, kSmallH = 4;  // rects up to this size go through the ballot window
 constexpr int kRounds = 1;               // write-then-check rounds before the atomic fallback
-constexpr uint32_t kMaxOcc = 64;         // bucket occupancy above which a segment takes the radix fallback
+constexpr uint32_t kMaxOcc = 512;        // bucket occupancy above which a segment takes the radix fallback
 constexpr int kFbBits = 8;               // digit width of the fallback radix sort
 constexpr uint32_t kSubTarget = 2048;    // expected sub-segment size of a giant split
 constexpr int kCoarseMax = 1024;         // sub-segments per giant tile (one per thread of giant_split)
@@ -448,6 +448,7 @@ __global__ void __launch_bounds__(kCoarseMax)
 giant_split_kernel(const Seg* __restrict__ giant_list, Seg* __restrict__ large_list, Counters* __restrict__ ctr,
                    const uint2* __restrict__ pairs, uint2* __restrict__ tmp, const int64_t* __restrict__ P_dev) {
     __shared__ uint32_t hist[kCoarseMax];
+    __shared__ uint32_t gstart[kCoarseMax];
     __shared__ uint32_t ws[66];
     __shared__ uint32_t s_ticket;
     if (P_dev[1]) return;
@@ -467,7 +468,9 @@ giant_split_kernel(const Seg* __restrict__ giant_list, Seg* __restrict__ large_l
             hi = max(hi, k);
         }
         block_minmax(lo, hi, ws);
-        const uint32_t nb = min((uint32_t)kCoarseMax, (sg.len + kSubTarget - 1u) / kSubTarget);
+        // always kCoarseMax fine buckets; runs of consecutive buckets are then merged into sub-segments
+        // of about S elements, so a depth cluster is cut as finely as the bucket map allows
+        const uint32_t nb = (uint32_t)kCoarseMax;
         const float scale = bucket_scale(lo, hi, nb);
         hist[threadIdx.x] = 0u;
         __syncthreads();
@@ -476,11 +479,24 @@ giant_split_kernel(const Seg* __restrict__ giant_list, Seg* __restrict__ large_l
         const uint32_t c = hist[threadIdx.x];
         uint32_t tot;
         const uint32_t off = block_excl_scan(c, ws, tot);
+        __syncthreads();
         hist[threadIdx.x] = off;  // becomes the bucket's cursor
-        if (c > 0u) {
-            Seg sub;
-            sub.start = sg.start + off; sub.len = c; sub.tile = sg.tile; sub.in_tmp = 1u;
-            large_list[atomicAdd(&ctr->n_large, 1u)] = sub;
+        // bucket b opens a sub-segment when its offset enters a new block of S elements (S > len / 1024)
+        const uint32_t S = max(kSubTarget, sg.len / (uint32_t)kCoarseMax + 1u);  // off / S < kCoarseMax even for off == len
+        gstart[threadIdx.x] = 0xffffffffu;
+        __syncthreads();
+        const uint32_t q = off / S;
+        const bool opens = threadIdx.x == 0 || hist[threadIdx.x - 1] / S != q;
+        if (opens) gstart[q] = off;  // q < kCoarseMax; one opener per q
+        __syncthreads();
+        const bool closes = threadIdx.x == kCoarseMax - 1 || hist[threadIdx.x + 1] / S != q;
+        if (closes) {
+            const uint32_t st = gstart[q], en = off + c;
+            if (en > st) {
+                Seg sub;
+                sub.start = sg.start + st; sub.len = en - st; sub.tile = sg.tile; sub.in_tmp = 1u;
+                large_list[atomicAdd(&ctr->n_large, 1u)] = sub;
+            }
         }
         __syncthreads();
         for (uint32_t i = threadIdx.x; i < sg.len; i += kCoarseMax) {
