@@ -207,6 +207,8 @@ def run_tgs(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    # measured FFMA-only peak (tgs_fp32_peak): the roofline denominator of the raster kernels
+    fp32_peak_measured = tg.fp32_peak(5)
     for _ in range(max(args.warmup, 3)):
         full_step()
     barrier()
@@ -280,20 +282,33 @@ def run_tgs(args):
                  "bin_sort": scene.N * 16 + P * (8 + 8 + 4) + cam.num_tiles * 12}
     kernels = {
         "raster_fwd": {"bound": "alu", "achieved": fwd_flops / (per_call_ms["raster_fwd"] * 1e-3) / 1e12,
-                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"},
+                       "peak": fp32_peak_measured, "unit": "TFLOP/s"},
         "raster_bwd": {"bound": "alu", "achieved": bwd_flops / (per_call_ms["raster_bwd"] * 1e-3) / 1e12,
-                       "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s"},
+                       "peak": fp32_peak_measured, "unit": "TFLOP/s"},
     }
     for nm in ("preprocess", "project_bwd", "bin_sort"):
         kernels[nm] = {"bound": "hbm", "achieved": hbm_bytes[nm] / (per_call_ms[nm] * 1e-3) / 1e9,
                        "peak": peaks["hbm_gbs"], "unit": "GB/s"}
+    kernels["bin_sort"]["note"] = "call of ~10 dependent kernels (launch list in profiles/), not one kernel"
     for v in kernels.values():
         v["frac"] = v["achieved"] / v["peak"]
-    dominant = max(("raster_fwd", "raster_bwd", "preprocess", "project_bwd", "bin_sort"), key=lambda k_: per_call_ms[k_])
+    # dominant KERNEL of the step (bin_sort and sample are calls of several short kernels, each shorter
+    # than these; profiles/ has the launch list that shows it)
+    dominant = max(("raster_fwd", "raster_bwd", "preprocess", "project_bwd"), key=lambda k_: per_call_ms[k_])
     roof = dict(kernels[dominant])
-    roof.update({"kernel": dominant, "traffic": None, "ms": per_call_ms[dominant],
-                 "peak_source": ("nominal fp32: 148 SM x 128 lanes x 2 flop x 1.965 GHz" if roof["bound"] == "alu"
-                                 else f"MEASURED_PEAKS.json hbm_gbs ({peak_src})")})
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu --set full capture
+    if os.path.exists(tp):
+        with open(tp) as f:
+            traffic = json.load(f).get(f"config{args.config}", {}).get(dominant)
+    roof.update({"kernel": dominant + "_kernel", "traffic": traffic, "ms": per_call_ms[dominant],
+                 "peak_nominal": FP32_PEAK_TFLOPS if roof["bound"] == "alu" else None,
+                 "peak_source": ("measured: tgs_fp32_peak (FFMA-only kernel, best of 5, CUDA events); nominal = 148 SM x 128 "
+                                 "lanes x 2 flop x 1.965 GHz" if roof["bound"] == "alu"
+                                 else f"MEASURED_PEAKS.json hbm_gbs ({peak_src})"),
+                 "algorithmic_work": ("flops = 15 x walked + 10 x blended (fwd) / 15 x replayed + 64 x blended (bwd) "
+                                      "(pixel, Gaussian) evaluations, DESIGN.md 'Roofline accounting'"
+                                      if roof["bound"] == "alu" else "bytes per Gaussian, DESIGN.md 'Kernels'")})
 
     # ---- end to end: host buffers in, host gradients out, copies inside the timed region ----
     Hout = {k_: torch.empty(v.shape, dtype=v.dtype).pin_memory() for k_, v in
@@ -345,7 +360,7 @@ def run_tgs(args):
                      "raster_px_per_s": n / ((per_call_ms["raster_fwd"] + per_call_ms["raster_bwd"]) * 1e-3)}}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        reps = 3 if scene.N <= 200_000 else 1
+        reps = 10 if scene.N <= 200_000 else 1  # ~10 s of CPU work on configs[1]
         n_o, times, _ = time_oracle(scene, reps, 0)
         line["cpu_baseline"] = {"value": n_o * len(times) / sum(times), "unit": UNIT, "cores": 1, "kind": "oracle",
                                 "sample": f"{len(times)} full step(s) of the same workload, single thread, "

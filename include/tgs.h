@@ -75,6 +75,11 @@ const char* tgs_version(void);
 /* Number of CUDA kernels this library has launched in this process (all contexts); bench.py
  * reports the difference over its timed region as gpu_launches. */
 uint64_t tgs_launch_count(void);
+/* Measured FP32 peak of the device, the roofline denominator of the ALU-bound raster kernels
+ * (SURVEY.md 8d): runs an FFMA-only kernel (8 independent chains per thread, every SM full) `reps`
+ * times on `stream`, synchronises, and writes the best rate in TFLOP/s (2 flop per FMA) to
+ * *tflops (host pointer).  Diagnostic; not on the hot path. */
+int tgs_fp32_peak(tgs_ctx* ctx, int reps, double* tflops, void* stream);
 
 /* ---- a1: projection -------------------------------------------------------
  * in : means3D[N,3] scales[N,3] quats[N,4] opacities[N] sh[N,K,3], K=(sh_degree+1)^2 (coefficient

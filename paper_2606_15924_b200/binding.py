@@ -23,7 +23,7 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
              4: "TGS_ERR_UNSUPPORTED"}
 
 # every symbol include/tgs.h declares (tests check the library exports them all)
-SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_preprocess",
+SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
            "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse"]
 
@@ -77,6 +77,7 @@ def load_library() -> C.CDLL:
     lib.tgs_last_error.restype = C.c_char_p
     lib.tgs_version.restype = C.c_char_p
     lib.tgs_launch_count.restype = C.c_uint64
+    lib.tgs_fp32_peak.argtypes = [vp, i32, C.POINTER(C.c_double), vp]
     cam = C.POINTER(Camera)
     lib.tgs_preprocess.argtypes = [vp, cam, i32, i32] + [vp] * 5 + [vp] * 3 + [vp]
     lib.tgs_bin_sort_workspace_bytes.argtypes = [i32, i64, i32, C.POINTER(C.c_size_t)]
@@ -127,6 +128,12 @@ class TGS:
 
     def launch_count(self) -> int:
         return int(self.lib.tgs_launch_count())
+
+    def fp32_peak(self, reps: int = 10, stream=None) -> float:
+        """Measured FFMA-only peak in TFLOP/s (tgs_fp32_peak)."""
+        v = C.c_double()
+        self._check(self.lib.tgs_fp32_peak(self._h, reps, C.byref(v), _stream(stream)))
+        return float(v.value)
 
     def _check(self, rc):
         if rc != 0:

@@ -81,6 +81,52 @@ int tgs_destroy(tgs_ctx* ctx) {
 
 const char* tgs_last_error(const tgs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
 
+// ---- diagnostic: FFMA-only micro-benchmark (roofline denominator of the ALU-bound kernels) ----
+namespace {
+__global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, float a, float b, int iters) {
+    float x0 = threadIdx.x, x1 = x0 + 1.f, x2 = x0 + 2.f, x3 = x0 + 3.f, x4 = x0 + 4.f, x5 = x0 + 5.f, x6 = x0 + 6.f, x7 = x0 + 7.f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            x0 = fmaf(x0, a, b); x1 = fmaf(x1, a, b); x2 = fmaf(x2, a, b); x3 = fmaf(x3, a, b);
+            x4 = fmaf(x4, a, b); x5 = fmaf(x5, a, b); x6 = fmaf(x6, a, b); x7 = fmaf(x7, a, b);
+        }
+    }
+    const float r = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (r == 123.456f) out[0] = r;  // keeps the chains alive
+}
+}  // namespace
+
+int tgs_fp32_peak(tgs_ctx* ctx, int reps, double* tflops, void* stream) {
+    if (!ctx || !tflops || reps < 1) return TGS_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    float* d = nullptr;
+    cudaEvent_t e0, e1;
+    cudaError_t e = cudaMalloc(&d, 256);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_fp32_peak", e);
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int blocks = ctx->num_sms * 8, iters = 4096;
+    const double flop = 2.0 * 8 * 16 * (double)iters * 256.0 * blocks;
+    double best = 0.0;
+    for (int r = 0; r < reps + 2; ++r) {  // two warm-up launches
+        cudaEventRecord(e0, s);
+        ffma_peak_kernel<<<blocks, 256, 0, s>>>(d, 0.999f, 0.001f, iters);
+        cudaEventRecord(e1, s);
+        e = cudaEventSynchronize(e1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r >= 2 && ms > 0.f) best = fmax(best, flop / (ms * 1e-3) / 1e12);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_fp32_peak", e);
+    *tflops = best;
+    return TGS_OK;
+}
+
 int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree, const float* means3D,
                    const float* scales, const float* quats, const float* opacities, const float* sh,
                    float* splats, int32_t* radii, uint8_t* clamped, void* stream) {
