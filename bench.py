@@ -297,10 +297,13 @@ def run_tgs(args):
     dominant = max(("raster_fwd", "raster_bwd", "preprocess", "project_bwd"), key=lambda k_: per_call_ms[k_])
     roof = dict(kernels[dominant])
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")  # dram bytes per launch from the committed ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "r1c_traffic.csv")  # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
         with open(tp) as f:
-            traffic = json.load(f).get(f"config{args.config}", {}).get(dominant)
+            for ln in f.read().splitlines()[1:]:
+                c_, k_, b_ = ln.split(",")
+                if int(c_) == args.config and k_ == dominant:
+                    traffic = float(b_)
     roof.update({"kernel": dominant + "_kernel", "traffic": traffic, "ms": per_call_ms[dominant],
                  "peak_nominal": FP32_PEAK_TFLOPS if roof["bound"] == "alu" else None,
                  "peak_source": ("measured: tgs_fp32_peak (FFMA-only kernel, best of 5, CUDA events); nominal = 148 SM x 128 "
