@@ -9,27 +9,32 @@
 // atomic per pair is as expensive as all the memory traffic of the sort, so the design avoids
 // per-pair atomics altogether:
 //
-//   K0 topleft_count  one RED per visible Gaussian: histogram of the rect's top-left tile.
-//   K1 bin_scan       (one block) exclusive scan of that histogram; summed-area table of tile_select.
-//   K2 reorder        a 16-byte record {depth bits, id, rect} per visible Gaussian, grouped by
-//                     top-left tile.  Gaussians whose rect holds no selected tile get an empty rect.
-//                     From here on a warp's 32 records are neighbours on screen.
-//   K3 pair_count     per warp: the lanes that share a top-left ROW span a window of a few tiles;
-//                     for every window tile ONE ballot gives the covering lanes, so the warp
-//                     issues one RED per (warp, tile) instead of one per pair.  Rects wider than
-//                     4x4 tiles are walked by the whole warp, one atomic per pair (few Gaussians).
-//   K4 tile_scan      (one block) CSR tile_offsets[T+1], P, and the work lists of the sort by size.
+//   Ks select_sat     (one block, only with tile_select) summed-area table of the selection.
+//   K0 topleft_count  every rect is cut into pieces of at most 4x4 tiles; histogram of the pieces'
+//                     top-left tiles (pieces without a selected tile are dropped), privatised in
+//                     shared memory per block; P = sum of the pieces' selected tiles.
+//   K1 bin_scan       (one block) exclusive scan of that histogram; publishes P and the capacity flag.
+//   K2 reorder        a 16-byte record {depth bits, id, piece rect} per piece, grouped by top-left
+//                     tile (slots from the block's private cursors: no global atomic).  From here on
+//                     a warp's 32 records are neighbours on screen.
+//   K3 pair_count     per warp: the lanes that share a top ROW span a window of a few tiles; each
+//                     lane holds its coverage of the window as a 32-bit mask, ONE ballot per window
+//                     tile gives the covering lanes, so the warp issues one RED per (warp, tile)
+//                     instead of one per pair.
+//   K4 tile_scan      (one block) CSR tile_offsets[T+1] and the work lists of the sort by size.
 //   K5 pair_scatter   same walk as K3: one ATOM per (warp, tile) reserves a run of the tile's
 //                     segment, the covering lanes write (depth bits, id) at consecutive slots.
-//   K6 giant_split    segments above the shared-memory capacity are split by depth into
-//                     sub-segments (monotone interpolation between the segment's min and max key).
-//   K7 seg_sort       a block sorts a segment in shared memory in ONE distribution step: bucket =
-//                     monotone interpolation of the depth bits between the segment's min and max
-//                     (about one element per bucket); the slot inside a bucket is found WITHOUT
-//                     atomics by write-then-check rounds on a 16-bit table (the last writer of a
-//                     round wins a slot; ~6 rounds); buckets are then ordered by counting, inside
-//                     each bucket, the elements with a smaller (depth, id).  A segment whose keys
-//                     pile up (> 64 in a bucket: equal depths) falls back to a stable LSD radix
+//   K6 giant_split    segments above the shared-memory capacity are split by depth: 1024 fine
+//                     buckets (monotone interpolation between the segment's min and max key) merged
+//                     into sub-segments of ~2k elements.
+//   K7 seg_sort       (three launches: <= 2048 / 4096 / 8192 elements) a block sorts a segment in
+//                     shared memory in ONE distribution step: bucket = monotone interpolation of the
+//                     depth bits between the segment's min and max (about two buckets per element);
+//                     the slot inside a bucket comes from one write-then-check round on a 16-bit
+//                     table (the last writer wins slot 0: no atomic for ~80 % of the elements) and a
+//                     shared-memory atomic for the losers; buckets are then ordered by counting,
+//                     inside each bucket, the elements with a smaller (depth, id).  A segment whose
+//                     keys pile up (> 512 in a bucket: equal depths) falls back to a stable LSD radix
 //                     sort on (id, depth) in global memory.
 //
 // The final order is unique, so the result is deterministic although the slot assignment of K2/K5
