@@ -458,6 +458,7 @@ giant_split_kernel(const Seg* __restrict__ giant_list, Seg* __restrict__ large_l
     __shared__ uint32_t s_ticket;
     if (P_dev[1]) return;
     const uint32_t n_work = *reinterpret_cast<volatile uint32_t*>(&ctr->n_giant);
+    if (n_work == 0u) return;
     for (;;) {
         __syncthreads();
         if (threadIdx.x == 0) s_ticket = atomicAdd(&ctr->sched_giant, 1u);
@@ -606,6 +607,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
     __shared__ uint32_t s_ticket[2];
     if (P_dev[1]) return;
     const uint32_t n_work = *reinterpret_cast<const volatile uint32_t*>(n_work_ptr);
+    if (n_work == 0u) return;  // nothing of this size class: skip the ticket round trip
     const uint32_t tid = threadIdx.x;
     if (tid == 0) s_ticket[0] = atomicAdd(sched, 1u);
     __syncthreads();
