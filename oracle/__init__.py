@@ -201,6 +201,20 @@ class Oracle:
                                   _ptr(img))
         return img
 
+    # ---- O7: sparse supervision, Eq. 9-11, 472-481 Eq. 17-18 ----
+    def loss_sparse(self, cam, samp, color, target, eps_l1=1e-3, eps_ncc=1e-6, eps_lam=1e-8):
+        n, k = samp.n, samp.k
+        col = self.r(color).reshape(n, 3)
+        tg = self.r(target).reshape(cam.height, cam.width, 3)
+        o = SimpleNamespace(dL_dcolor=np.zeros((n, 3), self.real), pix_err=np.zeros(n, self.real),
+                            tile_stats=np.zeros((k, 3), self.real), loss=np.zeros(2, self.real))
+        c = self.cam(cam)
+        R = self._creal
+        self.lib.orc_loss_sparse(C.byref(c), C.c_int(k), _ptr(samp.tile_pix_offsets), _ptr(samp.pix), _ptr(col), _ptr(tg),
+                                 R(eps_l1), R(eps_ncc), R(eps_lam), _ptr(o.dL_dcolor), _ptr(o.pix_err),
+                                 _ptr(o.tile_stats), _ptr(o.loss))
+        return o
+
     # ---- small exported helpers (pinned individually) ---------------------------------------
     def quat_to_R(self, q):
         R = np.zeros(9, self.real)

@@ -691,3 +691,79 @@ void orc_render_dense(const orc_cam* cam, const uint32_t* tile_offsets, const ui
             image[3 * p + 2] = C[2] + T * cam->bg[2];
         }
 }
+
+/* O7 orc_loss_sparse: sparse supervision on the sampled pixels.
+ *   PAPER.md:168-208 Sec. 3.7 Eq. 9-11, Eq. 17-18.  Readings (R19-R23):
+ *   - pixel term: Charbonnier l1(p) = 1/3 sum_c sqrt((x_c - y_c)^2 + eps_l1^2)   (Eq. 17 left is its derivative)
+ *   - tile term (Eq. 9): per colour channel, over the tile's m sampled pixels, population statistics
+ *       NCC_c = cov_xy / sqrt(var_x var_y + eps_ncc),   L_ncc^tau = 1/3 sum_c (1 - NCC_c)
+ *     with the per-pixel gradient of Eq. 17 right (exact derivative of m L_ncc^tau, eps placed as written here):
+ *       gN_{p,c} = m dL_ncc/dx_{p,c} = -1/3 [ (y - mu_y)/sqrt(var_x var_y + eps) - NCC_c var_y (x - mu_x)/(var_x var_y + eps) ]
+ *   - Eq. 10: gbar_k = mean over the tile's pixels of the 1-norm (over channels) of the per-pixel gradient of
+ *     term k (dl1/dx and gN); lambda = clip(gbar_l1 / (gbar_ncc + eps_lam), 0, 1), a constant for the derivative
+ *   - Eq. 11 / 18: every sampled pixel carries its tile's term (the expectation over tiles is pixel weighted,
+ *     which is what makes the per-pixel gradients of Eq. 17-18, printed without 1/m, the exact derivative):
+ *       L = 1/n sum_p [ l1(p) + lambda_tau(p) L_ncc^tau(p) ],   dL/dx_{p,c} = 1/n (dl1/dx + lambda gN)
+ *     (the minus sign in front of lambda in Eq. 18 contradicts Eq. 11 and Eq. 17; Eq. 11 decides)
+ *   - pix_err(p) = sum_c |x_c - y_c|  (Eq. 2), the per-pixel error the error map is updated with
+ * tile_stats[k,3] = { sum_p l1(p), L_ncc^tau, lambda_tau };  loss[2] = { 1/n sum_p l1, 1/n sum_tau lambda m L_ncc }. */
+void orc_loss_sparse(const orc_cam* cam, int k, const uint32_t* tpo, const uint32_t* pix, const real* color,
+                     const real* target, real eps_l1, real eps_ncc, real eps_lam, real* dL_dcolor, real* pix_err,
+                     real* tile_stats, real* loss) {
+    (void)cam;
+    const uint32_t n = tpo[k];
+    real L1 = 0, LN = 0;
+    for (int it = 0; it < k; ++it) {
+        const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
+        real l1sum = 0, g1bar = 0, Lncc = 0, gNbar = 0;
+        /* pixel term and its gradient (stored unscaled in dL_dcolor for now) */
+        for (uint32_t i = 0; i < m; ++i) {
+            const uint32_t s = p0 + i, id = pix[s];
+            real e = 0, l = 0;
+            for (int c = 0; c < 3; ++c) {
+                real d = color[3 * s + c] - target[3 * (size_t)id + c];
+                real ch = rsqrt_(d * d + eps_l1 * eps_l1);
+                l += ch;
+                e += rabs(d);
+                dL_dcolor[3 * s + c] = (d / ch) / K_(3.0);
+                g1bar += rabs((d / ch) / K_(3.0));
+            }
+            l1sum += l / K_(3.0);
+            pix_err[s] = e;
+        }
+        /* tile term: statistics per channel, then the gradient; gN kept in a scratch pass */
+        real mu_x[3], mu_y[3], vx[3], vy[3], cxy[3], ncc[3], den[3];
+        for (int c = 0; c < 3; ++c) {
+            real sx = 0, sy = 0;
+            for (uint32_t i = 0; i < m; ++i) { sx += color[3 * (p0 + i) + c]; sy += target[3 * (size_t)pix[p0 + i] + c]; }
+            mu_x[c] = m ? sx / (real)m : 0; mu_y[c] = m ? sy / (real)m : 0;
+            real a = 0, b = 0, ab = 0;
+            for (uint32_t i = 0; i < m; ++i) {
+                real dx = color[3 * (p0 + i) + c] - mu_x[c], dy = target[3 * (size_t)pix[p0 + i] + c] - mu_y[c];
+                a += dx * dx; b += dy * dy; ab += dx * dy;
+            }
+            vx[c] = m ? a / (real)m : 0; vy[c] = m ? b / (real)m : 0; cxy[c] = m ? ab / (real)m : 0;
+            den[c] = vx[c] * vy[c] + eps_ncc;
+            ncc[c] = cxy[c] / rsqrt_(den[c]);
+            Lncc += (K_(1.0) - ncc[c]) / K_(3.0);
+        }
+        for (uint32_t i = 0; i < m; ++i)
+            for (int c = 0; c < 3; ++c) {
+                real dx = color[3 * (p0 + i) + c] - mu_x[c], dy = target[3 * (size_t)pix[p0 + i] + c] - mu_y[c];
+                real gN = -(dy / rsqrt_(den[c]) - ncc[c] * vy[c] * dx / den[c]) / K_(3.0);
+                gNbar += rabs(gN);
+            }
+        if (m) { g1bar /= (real)m; gNbar /= (real)m; }
+        real lam = rmin(K_(1.0), rmax(K_(0.0), g1bar / (gNbar + eps_lam)));
+        for (uint32_t i = 0; i < m; ++i)
+            for (int c = 0; c < 3; ++c) {
+                real dx = color[3 * (p0 + i) + c] - mu_x[c], dy = target[3 * (size_t)pix[p0 + i] + c] - mu_y[c];
+                real gN = -(dy / rsqrt_(den[c]) - ncc[c] * vy[c] * dx / den[c]) / K_(3.0);
+                dL_dcolor[3 * (p0 + i) + c] = (dL_dcolor[3 * (p0 + i) + c] + lam * gN) / (real)n;
+            }
+        tile_stats[3 * it] = l1sum; tile_stats[3 * it + 1] = Lncc; tile_stats[3 * it + 2] = lam;
+        L1 += l1sum; LN += lam * (real)m * Lncc;
+    }
+    loss[0] = n ? L1 / (real)n : 0;
+    loss[1] = n ? LN / (real)n : 0;
+}

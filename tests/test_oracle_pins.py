@@ -627,3 +627,124 @@ def test_f32_build_tracks_f64_build(orc32, orc64):
                   (b32.dL_dconic, b64.dL_dconic)]:
         d = np.abs(a[good] - bb[good]); ref = np.abs(bb[good])
         assert (d <= 1e-4 + 1e-3 * ref).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# O7 pins: sparse supervision (Eq. 9-11, 472-481 Eq. 17-18)
+def _loss_case(o, seed=0, W=80, H=48, pct=(60, 100), mode=1):
+    cam = cam_simple(W, H)
+    rng = np.random.default_rng(seed)
+    samp = o.sample(cam, pct, mode, (1, 2), 7, err=workloads.blob_error_map(rng, W, H, 5))
+    color = rng.random((samp.n, 3))
+    target = rng.random((H, W, 3))
+    return cam, samp, color, target
+
+
+def _tile_slices(samp):
+    off = samp.tile_pix_offsets.astype(np.int64)
+    return [slice(off[i], off[i + 1]) for i in range(samp.k)]
+
+
+def test_loss_terms_vs_numpy_definition(orc64):
+    """Charbonnier and the per-tile NCC written from Eq. 9 / 17 with numpy (corrcoef), Eq. 2 error, Eq. 11 sum."""
+    cam, samp, color, target = _loss_case(orc64)
+    e1, e2 = 1e-3, 1e-12  # a tiny eps_ncc: NCC becomes Pearson's r
+    r = orc64.loss_sparse(cam, samp, color, target, e1, e2, 1e-8)
+    y = target.reshape(-1, 3)[samp.pix]
+    d = color - y
+    assert np.allclose(r.pix_err, np.abs(d).sum(1), rtol=1e-13)
+    l1 = np.sqrt(d * d + e1 * e1).mean(1)
+    tot_ncc = 0.0
+    for i, sl in enumerate(_tile_slices(samp)):
+        m = sl.stop - sl.start
+        assert m >= 1
+        assert np.isclose(r.tile_stats[i, 0], l1[sl].sum(), rtol=1e-12)
+        if m >= 3:
+            ncc = np.mean([np.corrcoef(color[sl, c], y[sl, c])[0, 1] for c in range(3)])
+            assert np.isclose(r.tile_stats[i, 1], 1.0 - ncc, rtol=1e-7, atol=1e-9)
+        assert 0.0 <= r.tile_stats[i, 2] <= 1.0
+        tot_ncc += r.tile_stats[i, 2] * m * r.tile_stats[i, 1]
+    assert np.isclose(r.loss[0], l1.sum() / samp.n, rtol=1e-12)
+    assert np.isclose(r.loss[1], tot_ncc / samp.n, rtol=1e-12)
+
+
+def test_loss_ncc_invariances(orc64):
+    """NCC is invariant to a positive affine map of either argument and flips sign with a negative one:
+    target = a*render + b gives L_ncc = 0 (a > 0) or 2 (a < 0), and a zero NCC gradient."""
+    cam, samp, color, target = _loss_case(orc64, seed=3, mode=0)
+    for a, expect in ((0.4, 0.0), (-0.7, 2.0)):
+        tg = target.copy().reshape(-1, 3)
+        tg[samp.pix] = a * color + 0.25
+        r = orc64.loss_sparse(cam, samp, color, tg.reshape(target.shape), 1e-3, 1e-14, 1e-8)
+        assert np.allclose(r.tile_stats[:, 1], expect, atol=1e-8)
+        # at NCC = +-1 the tile term is stationary: the whole gradient is the Charbonnier one
+        d = color - tg[samp.pix]
+        g1 = d / np.sqrt(d * d + 1e-6) / 3.0 / samp.n
+        assert np.allclose(r.dL_dcolor, g1, atol=1e-9 / samp.n + 1e-12)
+    # scaling and shifting the render leaves every tile's NCC unchanged
+    r0 = orc64.loss_sparse(cam, samp, color, target, 1e-3, 1e-14, 1e-8)
+    r1 = orc64.loss_sparse(cam, samp, 0.5 * color + 0.1, target, 1e-3, 1e-14, 1e-8)
+    assert np.allclose(r0.tile_stats[:, 1], r1.tile_stats[:, 1], atol=1e-9)
+
+
+def test_loss_charbonnier_closed_form(orc64):
+    """x == y: l1 = eps and zero gradient; |x - y| >> eps: gradient -> sign(x - y) / (3 n) (Eq. 17 left)."""
+    cam, samp, color, target = _loss_case(orc64, seed=5, mode=0, pct=(100, 100))
+    tg = target.reshape(-1, 3)
+    tg[samp.pix] = color
+    r = orc64.loss_sparse(cam, samp, color, tg.reshape(target.shape), 1e-3, 1e-6, 1e-8)
+    assert np.allclose(r.tile_stats[:, 0] / np.diff(samp.tile_pix_offsets.astype(np.int64)), 1e-3, rtol=1e-12)
+    assert np.isclose(r.loss[0], 1e-3, rtol=1e-12) and np.all(r.pix_err == 0)
+    tg[samp.pix] = color - 0.5
+    r = orc64.loss_sparse(cam, samp, color, tg.reshape(target.shape), 1e-6, 1e-14, 1e-8)
+    lam = np.repeat(r.tile_stats[:, 2], np.diff(samp.tile_pix_offsets.astype(np.int64)))
+    # target is a shift of the render: NCC = 1 up to eps, its gradient vanishes, only the pixel term is left
+    assert np.allclose(r.dL_dcolor * samp.n, 1.0 / 3.0, atol=1e-4)
+    assert np.all(lam >= 0)
+
+
+def test_loss_lambda_balancing(orc64):
+    """Eq. 10 / 18: lambda = clip(gbar_l1 / gbar_ncc, 0, 1) from the per-pixel gradient 1-norms, recomputed here
+    with numpy from Eq. 17 as printed; both regimes (clipped at 1, strictly inside) must occur."""
+    cam, samp, color, target = _loss_case(orc64, seed=8)
+    y = target.reshape(-1, 3)[samp.pix]
+    seen_inside = seen_clip = False
+    for scale in (30.0, 0.02):  # high contrast: small NCC gradients, lambda clips at 1; low contrast: lambda < 1
+        col = 0.5 + scale * (color - 0.5)
+        r = orc64.loss_sparse(cam, samp, col, target, 1e-3, 1e-10, 1e-12)
+        d = col - y
+        g1 = np.abs(d / np.sqrt(d * d + 1e-6) / 3.0).sum(1)
+        for i, sl in enumerate(_tile_slices(samp)):
+            x, t = col[sl], y[sl]
+            dx, dy = x - x.mean(0), t - t.mean(0)
+            vx, vy, cxy = (dx * dx).mean(0), (dy * dy).mean(0), (dx * dy).mean(0)
+            ncc = cxy / np.sqrt(vx * vy + 1e-10)
+            gN = -((dy / np.sqrt(vx * vy + 1e-10)) - ncc * vy * dx / (vx * vy + 1e-10)) / 3.0
+            lam = min(1.0, g1[sl].mean() / (np.abs(gN).sum(1).mean() + 1e-12))
+            assert np.isclose(r.tile_stats[i, 2], lam, rtol=1e-9)
+            seen_inside |= lam < 0.999
+            seen_clip |= lam == 1.0
+    assert seen_inside and seen_clip
+
+
+def test_loss_gradient_finite_differences(orc64):
+    """dL_dcolor is the derivative of L = 1/n sum_p [l1 + lambda L_ncc] with lambda held fixed (Eq. 18)."""
+    cam, samp, color, target = _loss_case(orc64, seed=11, W=48, H=32)
+    eps = (1e-2, 1e-5, 1e-8)
+    r = orc64.loss_sparse(cam, samp, color, target, *eps)
+    lam = r.tile_stats[:, 2].copy()
+    m = np.diff(samp.tile_pix_offsets.astype(np.int64))
+
+    def frozen_loss(col):
+        q = orc64.loss_sparse(cam, samp, col, target, *eps)
+        return (q.tile_stats[:, 0].sum() + (lam * m * q.tile_stats[:, 1]).sum()) / samp.n
+
+    rng = np.random.default_rng(0)
+    h = 1e-6
+    for _ in range(40):
+        i, c = rng.integers(samp.n), rng.integers(3)
+        cp, cm = color.copy(), color.copy()
+        cp[i, c] += h
+        cm[i, c] -= h
+        fd = (frozen_loss(cp) - frozen_loss(cm)) / (2 * h)
+        assert np.isclose(r.dL_dcolor[i, c], fd, rtol=2e-5, atol=1e-9), (i, c, r.dL_dcolor[i, c], fd)
