@@ -166,6 +166,27 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
                           float* dL_dmeans3D, float* dL_dscales, float* dL_dquats,
                           float* dL_dopacities, float* dL_dsh, void* stream);
 
+/* ---- f1: sparse supervision (Sec. 3.7 Eq. 9-11, 472-481
+ * Eq. 17-18).  Sits between the forward and the backward: from the forward's colours of the n sampled
+ * pixels and the target image it writes dL_dcolor[n,3] -- the input of tgs_raster_bwd_sparse --, the
+ * per-pixel error pix_err[n] = sum_c |x_c - y_c| (Eq. 2, what the error map is updated with),
+ * tile_stats[k,3] = { sum_p l1(p), L_ncc^tau, lambda_tau } and (if loss != NULL) loss[2] =
+ * { 1/n sum_p l1(p), 1/n sum_tau lambda_tau m_tau L_ncc^tau }, all device pointers.
+ *   l1(p)      = 1/3 sum_c sqrt((x_c - y_c)^2 + eps_l1^2)                       (Charbonnier, Eq. 17 left)
+ *   L_ncc^tau  = 1/3 sum_c (1 - cov_xy / sqrt(var_x var_y + eps_ncc))           (Eq. 9; population statistics
+ *                over the tile's m sampled pixels, per colour channel)
+ *   lambda_tau = clip(gbar_l1 / (gbar_ncc + eps_lambda), 0, 1)                   (Eq. 10 / 18; gbar = mean over the
+ *                tile's pixels of the 1-norm of the per-pixel gradient; lambda is a constant for the derivative)
+ *   L          = 1/n sum_p [ l1(p) + lambda_tau(p) L_ncc^tau(p) ]                (Eq. 11, pixel weighted), and
+ *   dL_dcolor  = 1/n (dl1/dx + lambda_tau dL_ncc-per-pixel/dx)                   (Eq. 17-18) is its exact derivative.
+ * color, dL_dcolor, pix_err are indexed like the sampled-pixel list (tile order); target is [H,W,3].
+ * k = number of sampled tiles (host value, as in the raster calls); n = tile_pix_offsets[k] is read on the
+ * device.  Enqueues two kernels, no synchronisation, no workspace. */
+int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* tile_pix_offsets,
+                    const uint32_t* pix, const float* color, const float* target,
+                    float eps_l1, float eps_ncc, float eps_lambda,
+                    float* dL_dcolor, float* pix_err, float* tile_stats, float* loss, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

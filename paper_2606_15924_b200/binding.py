@@ -25,7 +25,7 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
 # every symbol include/tgs.h declares (tests check the library exports them all)
 SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
-           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse"]
+           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse"]
 
 
 class TgsError(RuntimeError):
@@ -89,6 +89,8 @@ def load_library() -> C.CDLL:
     lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
                                          [vp] + [vp] * 5 + [vp]
+    f32 = C.c_float
+    lib.tgs_loss_sparse.argtypes = [vp, cam, i32, vp, vp, vp, vp, f32, f32, f32, vp, vp, vp, vp, vp]
     return lib
 
 
@@ -237,6 +239,21 @@ class TGS:
                                                    _p(samp.tiles), _p(samp.tile_pix_offsets), _p(samp.pix),
                                                    _p(out.color), _p(out.T), _p(out.n_contrib), _p(out.n_walked),
                                                    _p(getattr(out, "n_blended", None)), _stream(stream)))
+        return out
+
+    # ---- f1: sparse supervision between the forward and the backward ----
+    def loss_sparse(self, cam, samp, color, target, eps_l1=1e-3, eps_ncc=1e-6, eps_lambda=1e-8, n_capacity=None,
+                    want_loss=True, out=None, stream=None):
+        cam = Camera.of(cam)
+        n = n_capacity if n_capacity is not None else samp.n
+        if out is None:
+            f = dict(dtype=torch.float32, device=self.device)
+            out = SimpleNamespace(dL_dcolor=torch.empty((n, 3), **f), pix_err=torch.empty(n, **f),
+                                  tile_stats=torch.empty((max(samp.k, 1), 3), **f),
+                                  loss=torch.zeros(2, **f) if want_loss else None)
+        self._check(self.lib.tgs_loss_sparse(self._h, C.byref(cam), samp.k, _p(samp.tile_pix_offsets), _p(samp.pix),
+                                             _p(color), _p(target), eps_l1, eps_ncc, eps_lambda, _p(out.dL_dcolor),
+                                             _p(out.pix_err), _p(out.tile_stats), _p(out.loss), _stream(stream)))
         return out
 
     # ---- a5 + a6 ----

@@ -25,6 +25,7 @@ SOURCES = {
     "raster_fwd.cu": [],
     "raster_bwd.cu": [],
     "project_bwd.cu": [],
+    "loss.cu": [],
 }
 
 

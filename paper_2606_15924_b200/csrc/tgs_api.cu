@@ -282,4 +282,20 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
     return TGS_OK;
 }
 
+int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* tile_pix_offsets, const uint32_t* pix,
+                    const float* color, const float* target, float eps_l1, float eps_ncc, float eps_lambda,
+                    float* dL_dcolor, float* pix_err, float* tile_stats, float* loss, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: bad camera");
+    if (k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: k = %d outside 0..T", k);
+    if (!(eps_l1 > 0.f) || !(eps_ncc > 0.f) || !(eps_lambda > 0.f))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: the three eps must be positive");
+    if (!tile_pix_offsets || !pix || !color || !target || !dL_dcolor || !pix_err || !tile_stats)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: null pointer");
+    cudaError_t e = launch_loss_sparse(k, tile_pix_offsets, pix, color, target, eps_l1, eps_ncc, eps_lambda, dL_dcolor,
+                                       pix_err, tile_stats, loss, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_loss_sparse", e);
+    return TGS_OK;
+}
+
 }  // extern "C"

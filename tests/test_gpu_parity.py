@@ -5,6 +5,8 @@ Bit exact: splat rect / depth / mean2D words, radii, clamp masks, sort keys, sor
 ranges, tile scores, sampled tiles and pixel lists.  Tolerance: forward 1e-5 rel / 1e-6 abs,
 gradients 1e-3 rel / 1e-5 abs (BASELINE.json north_star).
 """
+from types import SimpleNamespace
+
 import numpy as np
 import pytest
 
@@ -371,3 +373,87 @@ def test_bin_sort_segment_paths(case, orc32, tgs, torch):
     assert np.array_equal(u32(out.tile_offsets), rb.tile_offsets)
     assert np.array_equal(u32(out.gid_sorted)[:rb.P], rb.gid_sorted)
     assert np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:rb.P], rb.keys_sorted)
+
+
+# ---- f1: tgs_loss_sparse against the oracle's O7 (Eq. 9-11, 17-18) ---------------------------
+# Tolerance: the kernel sums <= 256 fp32 terms per tile statistic with a fixed
+# butterfly, the oracle sums in fp64; a mean / variance is then good to ~ 256 * 2^-24 = 1.5e-5 relative and the
+# gradient, a few products and one division of such statistics, to 1e-4 relative of the largest component.
+def _check_loss(out, ref, n, k, torch):
+    g = out.dL_dcolor[:n].cpu().numpy().astype(np.float64)
+    scale = np.abs(ref.dL_dcolor).max()
+    assert np.abs(g - ref.dL_dcolor).max() <= 1e-4 * scale, np.abs(g - ref.dL_dcolor).max() / scale
+    assert np.allclose(out.pix_err[:n].cpu().numpy(), ref.pix_err, rtol=1e-6, atol=1e-7)
+    st = out.tile_stats[:k].cpu().numpy().astype(np.float64)
+    assert np.allclose(st[:, 0], ref.tile_stats[:, 0], rtol=2e-5)
+    assert np.allclose(st[:, 1], ref.tile_stats[:, 1], rtol=1e-4, atol=1e-5)
+    assert np.allclose(st[:, 2], ref.tile_stats[:, 2], rtol=1e-4, atol=1e-6)
+    assert np.allclose(out.loss.cpu().numpy(), ref.loss, rtol=1e-4, atol=1e-7)
+
+
+@pytest.mark.parametrize("name", ["cfg1", "small_d1", "cfg2"])
+def test_loss_sparse_parity_on_rendered_colours(name, orc32, orc64, tgs, torch):
+    """The loss on the forward's own output (sparse pixel lists of the scene, seeded target image)."""
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    rng = np.random.default_rng(5)
+    target = np.clip(rng.normal(0.5, 0.25, (sc.cam.height, sc.cam.width, 3)), 0, 1).astype(np.float32)
+    color = r.fwd.color.astype(np.float32)
+    ref = orc64.loss_sparse(sc.cam, r.samp, color, target)
+    samp = SimpleNamespace(k=r.samp.k, n=r.samp.n, tile_pix_offsets=dev(r.samp.tile_pix_offsets.astype(np.int32), torch),
+                           pix=dev(r.samp.pix.astype(np.int32), torch))
+    out = tgs.loss_sparse(sc.cam, samp, dev(color, torch), dev(target, torch))
+    torch.cuda.synchronize()
+    _check_loss(out, ref, r.samp.n, r.samp.k, torch)
+
+
+@pytest.mark.parametrize("mode,pct,rate", [(0, (100, 100), (1, 1)), (1, (40, 100), (1, 3)), (1, (100, 100), (1, 200))])
+def test_loss_sparse_modes_and_edge_tiles(mode, pct, rate, orc32, orc64, tgs, torch):
+    """Ragged image (edge tiles), Bernoulli lists down to one pixel per tile, low-contrast renders (lambda < 1),
+    a render equal to the target (zero residual)."""
+    W, H = 203, 117
+    cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    rng = np.random.default_rng(21)
+    s = orc32.sample(cam, pct, mode, rate, 9, err=workloads.blob_error_map(rng, W, H, 6))
+    target = rng.random((H, W, 3)).astype(np.float32)
+    samp = SimpleNamespace(k=s.k, n=s.n, tile_pix_offsets=dev(s.tile_pix_offsets.astype(np.int32), torch),
+                           pix=dev(s.pix.astype(np.int32), torch))
+    cases = [rng.random((s.n, 3)).astype(np.float32),
+             (0.5 + 0.02 * (rng.random((s.n, 3)) - 0.5)).astype(np.float32),
+             target.reshape(-1, 3)[s.pix].copy()]
+    lam_inside = False
+    for color in cases:
+        ref = orc64.loss_sparse(cam, s, color, target)
+        out = tgs.loss_sparse(cam, samp, dev(color, torch), dev(target, torch))
+        torch.cuda.synchronize()
+        _check_loss(out, ref, s.n, s.k, torch)
+        lam_inside |= bool((ref.tile_stats[:, 2] < 0.999).any())
+    assert lam_inside
+
+
+def test_loss_feeds_the_backward(orc32, orc64, tgs, torch):
+    """End of the chain: forward colours -> tgs_loss_sparse -> tgs_raster_bwd_sparse, all on the GPU, against
+    the oracle run the same way."""
+    r = oracle_run("small_rot", orc32)
+    sc = r.sc
+    rng = np.random.default_rng(2)
+    target = rng.random((sc.cam.height, sc.cam.width, 3)).astype(np.float32)
+    ref_l = orc64.loss_sparse(sc.cam, r.samp, r.fwd.color, target)
+    g = ref_l.dL_dcolor.astype(np.float32)
+    rb = orc32.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, g)
+    pb = orc32.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii, r.pre.clamped,
+                           rb.dL_dmeans2D, rb.dL_dconic, rb.dL_drgb)
+    import paper_2606_15924_b200 as pk
+    d = scene_dev(sc, torch)
+    step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 8)
+    fw = step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
+                      sc.sample_seed, err=dev(sc.err, torch))
+    P, k, n = step.counts()
+    assert (k, n) == (r.samp.k, r.samp.n)
+    samp = SimpleNamespace(k=k, n=n, tile_pix_offsets=step.samp.tile_pix_offsets, pix=step.samp.pix)
+    lo = tgs.loss_sparse(sc.cam, samp, fw.color, dev(target, torch), n_capacity=sc.cam.width * sc.cam.height)
+    bw = step.backward(lo.dL_dcolor)
+    torch.cuda.synchronize()
+    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+    check_grad("dL_dmeans3D", bw.dL_dmeans3D.cpu().numpy(), pb.dL_dmeans3D, good)
+    check_grad("dL_dsh", bw.dL_dsh.cpu().numpy(), pb.dL_dsh, good)
