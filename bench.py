@@ -18,6 +18,7 @@ import statistics
 import sys
 import threading
 import time
+from types import SimpleNamespace
 
 ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
@@ -272,6 +273,22 @@ def run_tgs(args):
         acc["project_bwd"] += max(d[5] - d[4], 0.0)  # second call = raster + projection
     per_call_ms = {k_: v / args.steps for k_, v in acc.items()}
 
+    # ---- SURVEY.md 8f f1 (not part of the five-call step): the fused sparse loss between forward and backward ----
+    target_dev = torch.rand((cam.height, cam.width, 3), device=dev, generator=torch.Generator(device=dev).manual_seed(0))
+    lo = tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
+                        st.fwd.color, target_dev, n_capacity=cam.width * cam.height)
+    la, lb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    loss_ms = 0.0
+    for _ in range(args.steps):
+        flush.fill_(1.0)
+        la.record()
+        tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
+                       st.fwd.color, target_dev, out=lo)
+        lb.record()
+        torch.cuda.synchronize()
+        loss_ms += la.elapsed_time(lb)
+    loss_ms /= args.steps
+
     # ---- roofline of the dominant kernel ----
     peaks, peak_src = measured_peaks()
     fwd_flops = FWD_FLOPS_WALK * walked + FWD_FLOPS_BLEND * blended
@@ -356,6 +373,10 @@ def run_tgs(args):
             "gpu_launches": int(launches),
             "roofline": roof,
             "per_call_ms": per_call_ms,
+            "next_rows": {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
+                          "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                          "note": "tgs_loss_sparse (SURVEY.md 8f f1), timed alone, 44 algorithmic bytes per sampled pixel; "
+                                  "not inside the five-call step"},
             "kernels": kernels,
             "work": {"fwd_evals": walked, "bwd_evals": replayed, "blended": blended,
                      "fwd_evals_per_s": walked / (per_call_ms["raster_fwd"] * 1e-3),
