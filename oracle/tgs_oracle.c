@@ -24,10 +24,13 @@
  *   O4 orc_raster_fwd   Eq. 1 alpha compositing on the sampled pixels         PAPER.md:66 (Eq.1), 154-166
  *   O5 orc_raster_bwd   exact derivative of O4
  *   O6 orc_project_bwd  chain through O1 to (mu, s, q, sh)
+ *   O7 orc_loss_sparse  Charbonnier + tile-level sparse NCC + lambda_ncc      PAPER.md:168-208 (Eq.9-11),
+ *                                                                            472-481 (Eq.17-18)
  * Pins (tests/test_oracle_pins.py): closed-form isotropic render, two-Gaussian
  * compositing, partition of unity, transmittance monotonicity, SH orthonormality by
  * quadrature, brute-force binning, full mask == dense, empty mask == zero gradients,
- * colour-linearity identity, fp64 central finite differences.  No function here is
+ * colour-linearity identity, fp64 central finite differences; O7: numpy corrcoef definition,
+ * affine invariances of NCC, Charbonnier closed forms, both lambda regimes, finite differences.  No function here is
  * "parity unpinned".
  */
 #include <math.h>
