@@ -149,19 +149,17 @@ def workload_config(scene, args, P, k, n):
 
 def run_tgs(args):
     import torch
-    import torch.distributed as dist
     import paper_2606_15924_b200 as pk
     import workloads
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
+    from paper_2606_15924_b200.replicas import Replicas
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (the product has no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
+    rep = Replicas("nccl", dev)  # replicas only: barrier + max / sum over ranks, no data-path collective
+    world, rank = rep.world, rep.rank
 
     scene = load_scene(args.config, args.pct)
     cam = scene.cam
@@ -203,10 +201,7 @@ def run_tgs(args):
 
     flush = torch.empty(256 * 1024 * 1024 // 4, dtype=torch.float32, device=dev)  # 256 MiB > 126 MB L2
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+    barrier = rep.barrier
 
     # measured FFMA-only peak (tgs_fp32_peak): the roofline denominator of the raster kernels
     fp32_peak_measured = tg.fp32_peak(5)
@@ -231,15 +226,8 @@ def run_tgs(args):
     sampler.join()
     step_ms = [s.elapsed_time(e) for s, e in ev]
     total_ms = sum(step_ms)
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        nt = torch.tensor([n], device=dev, dtype=torch.float64)
-        dist.all_reduce(nt, op=dist.ReduceOp.SUM)
-        n_total = float(nt.item())
-    else:
-        n_total = float(n)
+    total_ms = rep.max_over_ranks(total_ms)
+    n_total = rep.sum_over_ranks(n)
     value = n_total * args.steps / (total_ms * 1e-3)
 
     # ---- per-call breakdown (separate pass; events between the calls) ----
@@ -357,10 +345,7 @@ def run_tgs(args):
     ee.record()
     barrier()
     e2e_ms = es.elapsed_time(ee)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = rep.max_over_ranks(e2e_ms)
     e2e_val = n_total * args.steps / (e2e_ms * 1e-3)
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -391,8 +376,7 @@ def run_tgs(args):
                                           f"{sum(times):.1f} s", "host_cores_available": os.cpu_count()}
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
-        dist.destroy_process_group()
+    rep.close()
 
 
 def main():
