@@ -200,10 +200,11 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
                         T = valid ? Tk : T;
                         Sg = valid ? fmaf(alpha, cg, om * Sg) : Sg;
                         vdst[ii * kTStride] = make_float2(dpow, w);
-                        if (lane == 0) {  // predicated single-lane stores: one wavefront each
-                            mdst[ii] = a;
-                            mdst[kSlots + ii] = make_float4(b.x, b.z, c.w, 0.f);
-                        }
+                    }
+                    if (lane < take) {  // the Gaussians' parameters for phase 2: one parallel copy per group
+                        const float4 b = sa[32 + lane];
+                        mdst[lane] = sa[lane];
+                        mdst[kSlots + lane] = make_float4(b.x, b.z, sa[64 + lane].w, 0.f);
                     }
                     e += take;
                     m += take;
