@@ -215,6 +215,17 @@ class Oracle:
                                  _ptr(o.tile_stats), _ptr(o.loss))
         return o
 
+    # ---- O8: statistics forward, Eq. 12 ----
+    def raster_stats(self, cam, binned, pre, samp, pix_err):
+        N = pre.means2D.shape[0]
+        o = SimpleNamespace(stats=np.zeros((N, 3), self.real), depth=np.zeros(samp.n, self.real))
+        c = self.cam(cam)
+        self.lib.orc_raster_stats(C.byref(c), C.c_int(N), _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
+                                  _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.depths)),
+                                  C.c_int(samp.k), _ptr(samp.tiles), _ptr(samp.tile_pix_offsets), _ptr(samp.pix),
+                                  _ptr(self.r(pix_err)), _ptr(o.stats), _ptr(o.depth))
+        return o
+
     # ---- small exported helpers (pinned individually) ---------------------------------------
     def quat_to_R(self, q):
         R = np.zeros(9, self.real)

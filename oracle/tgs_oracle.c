@@ -770,3 +770,47 @@ void orc_loss_sparse(const orc_cam* cam, int k, const uint32_t* tpo, const uint3
     loss[0] = n ? L1 / (real)n : 0;
     loss[1] = n ? LN / (real)n : 0;
 }
+
+/* O8 orc_raster_stats: statistics forward (Sec. 3.8 Eq. 12,
+ * Alg. 1 step 11 "rasterize_forward_pixels").  The same front-to-back walk as O4 (same thresholds, same
+ * stopping rule); every composited (pixel, Gaussian) pair with weight w = T alpha adds
+ *     E_i += e(p) w,   D_i += D_i(p) w,   W_i += w,
+ * where e(p) is the per-pixel error handed in (pix_err[n], sampled-pixel order) and D_i(p) = d^T Sigma'^-1 d
+ * = -2 power is the conic Mahalanobis distance between the splat centre and the pixel.
+ * stats[N,3] = {E, D, W}; accumulators are double in both builds.  out_depth[n] (nullable) = sum_i w z_i,
+ * the expected depth of the sampled pixel (the "depth output" of SURVEY.md f3). */
+void orc_raster_stats(const orc_cam* cam, int N, const uint32_t* tile_offsets, const uint32_t* gid_sorted,
+                      const real* mean2D, const real* conic_o, const real* depth, int k, const uint32_t* tiles,
+                      const uint32_t* tile_pix_offsets, const uint32_t* pix, const real* pix_err, real* stats,
+                      real* out_depth) {
+    const int W = cam->W;
+    double* acc = (double*)calloc((size_t)N * 3, sizeof(double));
+    for (int it = 0; it < k; ++it) {
+        uint32_t t = tiles[it];
+        uint32_t start = tile_offsets[t], end = tile_offsets[t + 1];
+        for (uint32_t ip = tile_pix_offsets[it]; ip < tile_pix_offsets[it + 1]; ++ip) {
+            real px = (real)(pix[ip] % (uint32_t)W), py = (real)(pix[ip] / (uint32_t)W);
+            real T = K_(1.0);
+            double z = 0;
+            for (uint32_t j = start; j < end; ++j) {
+                uint32_t g = gid_sorted[j];
+                real dx = mean2D[2 * g] - px, dy = mean2D[2 * g + 1] - py;
+                real power = splat_power(conic_o[4 * g], conic_o[4 * g + 1], conic_o[4 * g + 2], dx, dy);
+                if (power > 0) continue;
+                real alpha = rmin(ALPHA_MAX, conic_o[4 * g + 3] * rexp(power));
+                if (alpha < ALPHA_MIN) continue;
+                real Tn = T * (K_(1.0) - alpha);
+                if (Tn < T_MIN) break;
+                real w = alpha * T;
+                acc[3 * (size_t)g] += (double)(pix_err[ip] * w);
+                acc[3 * (size_t)g + 1] += (double)(K_(-2.0) * power * w);
+                acc[3 * (size_t)g + 2] += (double)w;
+                z += (double)(w * depth[g]);
+                T = Tn;
+            }
+            if (out_depth) out_depth[ip] = (real)z;
+        }
+    }
+    for (size_t i = 0; i < (size_t)N * 3; ++i) stats[i] = (real)acc[i];
+    free(acc);
+}

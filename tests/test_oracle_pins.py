@@ -748,3 +748,115 @@ def test_loss_gradient_finite_differences(orc64):
         cm[i, c] -= h
         fd = (frozen_loss(cp) - frozen_loss(cm)) / (2 * h)
         assert np.isclose(r.dL_dcolor[i, c], fd, rtol=2e-5, atol=1e-9), (i, c, r.dL_dcolor[i, c], fd)
+
+
+# ---------------------------------------------------------------------------------------------
+# O8 pins: statistics forward (Eq. 12)
+def test_stats_single_gaussian_closed_form(orc64):
+    """One isotropic Gaussian: w = alpha (T = 1), so W = sum alpha, E = sum e alpha, D = sum (d^T S^-1 d) alpha and
+    the expected depth is alpha t_z, all from the closed form of the EWA covariance."""
+    f, s, tz, o = 64.0, 0.08, 2.0, 0.8
+    cam = cam_simple(64, 64, f)
+    mu = [0.11, -0.07, tz]
+    pre = orc64.preprocess(cam, 0, [mu], [[s] * 3], [[1.0, 0.0, 0.0, 0.0]], [o], np.zeros((1, 1, 3)))
+    b = orc64.bin_sort(cam, pre)
+    samp = full_mask(orc64, cam)
+    rng = np.random.default_rng(0)
+    e = rng.random(samp.n)
+    r = orc64.raster_stats(cam, b, pre, samp, e)
+    t = np.array(mu)
+    J = np.array([[f / tz, 0, -f * t[0] / tz ** 2], [0, f / tz, -f * t[1] / tz ** 2]])
+    inv = np.linalg.inv(s * s * J @ J.T + 0.3 * np.eye(2))
+    m = np.array([f * t[0] / tz + 32 - 0.5, f * t[1] / tz + 32 - 0.5])
+    x0, y0, x1, y1 = pre.rect[0]
+    W = E = D = 0.0
+    depth = np.zeros(samp.n)
+    for ip, p in enumerate(samp.pix):
+        x, y = int(p) % 64, int(p) // 64
+        if not (x0 <= x // 16 < x1 and y0 <= y // 16 < y1):
+            continue
+        d = np.array([x, y]) - m
+        q = d @ inv @ d
+        a = min(0.99, o * math.exp(-0.5 * q))
+        if a < 1 / 255:
+            continue
+        W += a; E += e[ip] * a; D += q * a
+        depth[ip] = a * tz
+    assert W > 5.0
+    assert np.allclose(r.stats[0], [E, D, W], rtol=1e-11)
+    assert np.allclose(r.depth, depth, rtol=1e-12, atol=1e-15)
+
+
+def test_stats_identities_on_a_composite(orc64):
+    """On a real multi-layer scene: sum_i W_i = sum_p (1 - T_final(p)) (the weights of a pixel sum to its opacity),
+    e == 1 gives E == W, D >= 0, scaling e scales E, Gaussians off the sampled pixels get nothing, and the
+    expected depth lies between the nearest and the farthest contributor."""
+    sc = workloads.small_random_scene(13, 400, 96, 64, sh_degree=0, spread=1.0, log_scale=(-2.4, 0.5))
+    pre = orc64.preprocess(sc.cam, 0, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+    b = orc64.bin_sort(sc.cam, pre)
+    samp = orc64.sample(sc.cam, (50, 100), 1, (1, 2), 3, err=workloads.blob_error_map(np.random.default_rng(1), 96, 64, 4))
+    fw = orc64.raster_fwd(sc.cam, b, pre, samp)
+    rng = np.random.default_rng(2)
+    e = rng.random(samp.n)
+    r = orc64.raster_stats(sc.cam, b, pre, samp, e)
+    E, D, W = r.stats.T
+    assert np.isclose(W.sum(), (1.0 - fw.T).sum(), rtol=1e-12)
+    assert (D >= 0).all() and (W >= 0).all() and (W > 0).sum() > 50
+    r1 = orc64.raster_stats(sc.cam, b, pre, samp, np.ones(samp.n))
+    assert np.allclose(r1.stats[:, 0], r1.stats[:, 2], rtol=1e-13) and np.allclose(r1.stats[:, 2], W, rtol=1e-13)
+    r3 = orc64.raster_stats(sc.cam, b, pre, samp, 3.0 * e)
+    assert np.allclose(r3.stats[:, 0], 3.0 * E, rtol=1e-12) and np.allclose(r3.stats[:, 1], D, rtol=1e-13)
+    # E_i / W_i is a weighted mean of the errors it saw
+    seen = W > 1e-9
+    assert (E[seen] / W[seen] <= e.max() + 1e-12).all() and (E[seen] / W[seen] >= e.min() - 1e-12).all()
+    # a Gaussian that is in no sampled tile's list cannot have weight
+    sel = np.zeros(sc.cam.num_tiles, bool); sel[samp.tiles] = True
+    off = b.tile_offsets.astype(np.int64)
+    touched = np.zeros(sc.N, bool)
+    for t in np.nonzero(sel)[0]:
+        touched[b.gid_sorted[off[t]:off[t + 1]]] = True
+    assert (W[~touched] == 0).all()
+    zmin, zmax = pre.depths[pre.radii > 0].min(), pre.depths[pre.radii > 0].max()
+    op = 1.0 - fw.T
+    ok = op > 1e-6
+    assert (r.depth[ok] / op[ok] >= zmin - 1e-9).all() and (r.depth[ok] / op[ok] <= zmax + 1e-9).all()
+
+
+def test_stats_vs_brute_force_definition(orc64):
+    """Eq. 12 written out with numpy from the definition: per pixel, K(p) in (depth, id) order, w = T alpha."""
+    sc = workloads.small_random_scene(17, 50, 40, 24, sh_degree=0, spread=0.8, log_scale=(-2.0, 0.6))
+    pre = orc64.preprocess(sc.cam, 0, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+    b = orc64.bin_sort(sc.cam, pre)
+    samp = full_mask(orc64, sc.cam)
+    fw = orc64.raster_fwd(sc.cam, b, pre, samp)
+    e = np.random.default_rng(5).random(samp.n)
+    r = orc64.raster_stats(sc.cam, b, pre, samp, e)
+    N, Wd = sc.N, sc.cam.width
+    ref = np.zeros((N, 3))
+    order = np.lexsort((np.arange(N), pre.depths.astype(np.float32).view(np.uint32)))
+    for ip, p in enumerate(samp.pix):
+        if fw.margin[ip, 0] <= 1e-9:
+            continue
+        x, y = int(p) % Wd, int(p) // Wd
+        T = 1.0
+        for g in order:
+            x0, y0, x1, y1 = pre.rect[g]
+            if pre.radii[g] <= 0 or not (x0 <= x // 16 < x1 and y0 <= y // 16 < y1):
+                continue
+            A, B, Cc, o = pre.conic_opacity[g]
+            dx, dy = pre.means2D[g, 0] - x, pre.means2D[g, 1] - y
+            q = A * dx * dx + 2 * B * dx * dy + Cc * dy * dy
+            if q < 0:
+                continue
+            a = min(0.99, o * math.exp(-0.5 * q))
+            if a < 1 / 255:
+                continue
+            if T * (1 - a) < 1e-4:
+                break
+            ref[g] += np.array([e[ip] * a * T, q * a * T, a * T])
+            T *= 1 - a
+    skip = fw.margin[:, 0] <= 1e-9
+    assert skip.mean() < 0.01
+    if not skip.any():
+        assert np.allclose(r.stats, ref, rtol=1e-9, atol=1e-12)
+    assert np.allclose(r.stats[:, 2].sum(), ref[:, 2].sum(), rtol=1e-3)
