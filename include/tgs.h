@@ -187,6 +187,23 @@ int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* 
                     float eps_l1, float eps_ncc, float eps_lambda,
                     float* dL_dcolor, float* pix_err, float* tile_stats, float* loss, void* stream);
 
+/* ---- f3: statistics forward (Sec. 3.8 Eq. 12; Alg. 1 step 11
+ * "rasterize_forward_pixels") -- the forward walk of tgs_raster_fwd_sparse (same thresholds, same stopping
+ * rule) that projects per-pixel quantities back onto the Gaussians: every composited (pixel, Gaussian)
+ * pair with weight w = T alpha adds
+ *     stats[i][0] (E_i) += pix_err(p) w     stats[i][1] (D_i) += (d^T Sigma'^-1 d) w     stats[i][2] (W_i) += w
+ * where pix_err[n] is the per-pixel error in sampled-pixel order (e.g. tgs_loss_sparse's) and
+ * d^T Sigma'^-1 d the conic Mahalanobis distance between the splat centre and the pixel.
+ * stats[N,4] (16-byte aligned; word 3 unused, 0) is zeroed inside the call and accumulated with fp32
+ * atomics (order not deterministic).  out_depth[n] (nullable) = sum_i w z_i, the expected depth of each
+ * sampled pixel.  The normalisations e_i = E_i/(W_i+eps), d_i and the score of Eq. 13 belong to the
+ * density-control logic above this library. */
+int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                            const uint32_t* tile_offsets, const uint32_t* gid_sorted,
+                            int k, const uint32_t* tiles, const uint32_t* tile_pix_offsets,
+                            const uint32_t* pix, const float* pix_err,
+                            float* stats, float* out_depth, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

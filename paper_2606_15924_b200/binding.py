@@ -25,7 +25,7 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
 # every symbol include/tgs.h declares (tests check the library exports them all)
 SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
-           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse"]
+           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse"]
 
 
 class TgsError(RuntimeError):
@@ -91,6 +91,7 @@ def load_library() -> C.CDLL:
                                          [vp] + [vp] * 5 + [vp]
     f32 = C.c_float
     lib.tgs_loss_sparse.argtypes = [vp, cam, i32, vp, vp, vp, vp, f32, f32, f32, vp, vp, vp, vp, vp]
+    lib.tgs_raster_stats_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
     return lib
 
 
@@ -254,6 +255,21 @@ class TGS:
         self._check(self.lib.tgs_loss_sparse(self._h, C.byref(cam), samp.k, _p(samp.tile_pix_offsets), _p(samp.pix),
                                              _p(color), _p(target), eps_l1, eps_ncc, eps_lambda, _p(out.dL_dcolor),
                                              _p(out.pix_err), _p(out.tile_stats), _p(out.loss), _stream(stream)))
+        return out
+
+    # ---- f3: statistics forward (E_i, D_i, W_i per Gaussian, expected depth per sampled pixel) ----
+    def raster_stats_sparse(self, cam, splats, binned, samp, pix_err, n_capacity=None, want_depth=True, out=None,
+                            stream=None):
+        cam = Camera.of(cam)
+        n = n_capacity if n_capacity is not None else samp.n
+        N = splats.shape[0]
+        if out is None:
+            f = dict(dtype=torch.float32, device=self.device)
+            out = SimpleNamespace(stats=torch.empty((max(N, 1), 4), **f), depth=torch.empty(max(n, 1), **f) if want_depth else None)
+        self._check(self.lib.tgs_raster_stats_sparse(self._h, C.byref(cam), N, _p(splats), _p(binned.tile_offsets),
+                                                     _p(binned.gid_sorted), samp.k, _p(samp.tiles),
+                                                     _p(samp.tile_pix_offsets), _p(samp.pix), _p(pix_err), _p(out.stats),
+                                                     _p(out.depth), _stream(stream)))
         return out
 
     # ---- a5 + a6 ----

@@ -26,6 +26,7 @@ SOURCES = {
     "raster_bwd.cu": [],
     "project_bwd.cu": [],
     "loss.cu": [],
+    "raster_stats.cu": [],
 }
 
 

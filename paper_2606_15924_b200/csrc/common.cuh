@@ -87,6 +87,11 @@ cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, c
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
                                float* dsh, cudaStream_t s);
 
+cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
+                                const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                                const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,
+                                uint32_t* sched, int num_sms, cudaStream_t s);
+
 cudaError_t launch_loss_sparse(int k, const uint32_t* tpo, const uint32_t* pix, const float* color, const float* target,
                                float eps_l1, float eps_ncc, float eps_lam, float* dL_dcolor, float* pix_err,
                                float* tile_stats, float* loss, cudaStream_t s);

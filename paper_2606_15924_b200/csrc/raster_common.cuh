@@ -38,7 +38,7 @@ constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kLnAlphaMin = -5.541263545158426f;  // ln(1/255)
 
 // one staged record, as three float4 planes per stage:
-//   p0 = mx, my, -A/2, -B     p1 = -C/2, thr = ln(1/(255 o)) - 1e-5, opacity, red     p2 = green, blue, bits: Gaussian id, 0
+//   p0 = mx, my, -A/2, -B     p1 = -C/2, thr = ln(1/(255 o)) - 1e-5, opacity, red     p2 = green, blue, bits: Gaussian id, depth
 template <int ENTRIES>
 struct Stage {
     float4 p0[ENTRIES];
@@ -232,7 +232,7 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                 if ((uint32_t)h * 64u >= cnt) break;
                 uint32_t g[2];
                 float4 r0[2], r1[2];
-                float r2x[2];
+                float2 r2x[2];  // blue, depth
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
                     const uint32_t i = h * 64 + j * 32 + lane;
@@ -244,7 +244,7 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                     if (g[j] != 0xffffffffu) {
                         r0[j] = splats[3 * (size_t)g[j]];
                         r1[j] = splats[3 * (size_t)g[j] + 1];
-                        r2x[j] = reinterpret_cast<const float*>(splats)[(size_t)g[j] * kSplatWords + 8];
+                        r2x[j] = *reinterpret_cast<const float2*>(reinterpret_cast<const float*>(splats) + (size_t)g[j] * kSplatWords + 8);
                     }
                 }
 #pragma unroll
@@ -253,7 +253,7 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                         const int i = h * 64 + j * 32 + lane;
                         st.p0[i] = make_float4(r0[j].x, r0[j].y, -0.5f * r0[j].z, -r0[j].w);
                         st.p1[i] = make_float4(-0.5f * r1[j].x, blend_threshold(r1[j].y), r1[j].y, r1[j].z);
-                        st.p2[i] = make_float4(r1[j].w, r2x[j], __uint_as_float(g[j]), 0.f);
+                        st.p2[i] = make_float4(r1[j].w, r2x[j].x, __uint_as_float(g[j]), r2x[j].y);
                     }
                 }
             }

@@ -298,4 +298,21 @@ int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* 
     return TGS_OK;
 }
 
+int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
+                            const uint32_t* tile_offsets, const uint32_t* gid_sorted, int k, const uint32_t* tiles,
+                            const uint32_t* tile_pix_offsets, const uint32_t* pix, const float* pix_err, float* stats,
+                            float* out_depth, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: bad camera");
+    if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: bad N or k");
+    if (!stats || (N > 0 && !splats) || (k > 0 && (!tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !pix_err)))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: null pointer");
+    if (((uintptr_t)splats & 15) || ((uintptr_t)stats & 15))
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: splats and stats must be 16-byte aligned");
+    cudaError_t e = launch_raster_stats(make_camk(cam), N, splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix,
+                                        pix_err, stats, out_depth, ctx->sched, ctx->num_sms, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_stats_sparse", e);
+    return TGS_OK;
+}
+
 }  // extern "C"

@@ -457,3 +457,54 @@ def test_loss_feeds_the_backward(orc32, orc64, tgs, torch):
     good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
     check_grad("dL_dmeans3D", bw.dL_dmeans3D.cpu().numpy(), pb.dL_dmeans3D, good)
     check_grad("dL_dsh", bw.dL_dsh.cpu().numpy(), pb.dL_dsh, good)
+
+
+# ---- f3: tgs_raster_stats_sparse against the oracle's O8 (Eq. 12) ------------------------------
+# Same bar as the gradients (fp32 atomics reorder the per-Gaussian sums): 1e-3 rel / 1e-5 abs with the block rule,
+# Gaussians reachable from a threshold-fragile pixel held to the loose bound; expected depth like the forward.
+@pytest.mark.parametrize("name", SCENES)
+def test_raster_stats_parity(name, orc32, tgs, torch):
+    r = oracle_run(name, orc32)
+    sc = r.sc
+    e = np.random.default_rng(3).random(r.samp.n).astype(np.float32)
+    ref = orc32.raster_stats(sc.cam, r.binned, r.pre, r.samp, e)
+    out = tgs.raster_stats_sparse(sc.cam, dev(pack_splats(r.pre), torch), binned_dev(r.binned, torch, sc.cam.num_tiles),
+                                  samp_dev(r.samp, torch), dev(e, torch))
+    torch.cuda.synchronize()
+    st = out.stats.cpu().numpy()
+    assert (st[:, 3] == 0).all()
+    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+    rep = check_grad("stats(E,D,W)", st[:, :3], ref.stats, good)
+    assert ref.stats[:, 2].sum() > 0
+    # sum_i W_i = sum_p (1 - T_final): the statistics walk is the forward's walk
+    assert np.isclose(st[:, 2].sum(dtype=np.float64), (1.0 - r.fwd.T.astype(np.float64)).sum(), rtol=1e-4)
+    d = out.depth[:r.samp.n].cpu().numpy()
+    ok = r.fwd.margin[:, 0] > MARGIN
+    assert ok.mean() > 0.99
+    assert np.allclose(d[ok], ref.depth[ok], rtol=1e-4, atol=1e-5), np.abs(d[ok] - ref.depth[ok]).max()
+    print(name, rep)
+
+
+def test_raster_stats_partial_tiles_and_empty(orc32, tgs, torch):
+    """Bernoulli pixel lists (partial units), error == 1 gives E == W, an empty selection gives zeros."""
+    sc = workloads.small_random_scene(23, 2500, 180, 120, sh_degree=0, spread=1.2, log_scale=(-2.6, 0.6))
+    pre = orc32.preprocess(sc.cam, 0, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+    b = orc32.bin_sort(sc.cam, pre)
+    s = orc32.sample(sc.cam, (60, 100), 1, (1, 3), 4, err=workloads.blob_error_map(np.random.default_rng(3), 180, 120, 5))
+    fw = orc32.raster_fwd(sc.cam, b, pre, s)
+    ones = np.ones(s.n, np.float32)
+    ref = orc32.raster_stats(sc.cam, b, pre, s, ones)
+    splats = dev(pack_splats(pre), torch)
+    out = tgs.raster_stats_sparse(sc.cam, splats, binned_dev(b, torch, sc.cam.num_tiles), samp_dev(s, torch), dev(ones, torch))
+    torch.cuda.synchronize()
+    st = out.stats.cpu().numpy()
+    good = tainted_gaussians(sc.N, b, s, fw)
+    check_grad("stats partial", st[:, :3], ref.stats, good)
+    assert np.allclose(st[:, 0], st[:, 2], rtol=1e-5, atol=1e-6)
+    # k = 0: nothing sampled
+    empty = SimpleNamespace(k=0, n=0, tiles=torch.zeros(1, dtype=torch.int32, device="cuda"),
+                            tile_pix_offsets=torch.zeros(1, dtype=torch.int32, device="cuda"),
+                            pix=torch.zeros(1, dtype=torch.int32, device="cuda"))
+    out0 = tgs.raster_stats_sparse(sc.cam, splats, binned_dev(b, torch, sc.cam.num_tiles), empty, dev(ones[:1], torch))
+    torch.cuda.synchronize()
+    assert (out0.stats.cpu().numpy() == 0).all()
