@@ -276,6 +276,17 @@ def run_tgs(args):
         torch.cuda.synchronize()
         loss_ms += la.elapsed_time(lb)
     loss_ms /= args.steps
+    # the statistics forward (E_i, D_i, W_i, expected depth), fed with the loss kernel's per-pixel error
+    so = tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, n_capacity=cam.width * cam.height)
+    stats_ms = 0.0
+    for _ in range(args.steps):
+        flush.fill_(1.0)
+        la.record()
+        tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, out=so)
+        lb.record()
+        torch.cuda.synchronize()
+        stats_ms += la.elapsed_time(lb)
+    stats_ms /= args.steps
 
     # ---- roofline of the dominant kernel ----
     peaks, peak_src = measured_peaks()
@@ -360,7 +371,11 @@ def run_tgs(args):
             "per_call_ms": per_call_ms,
             "next_rows": {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
                           "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                          "note": "tgs_loss_sparse (SURVEY.md 8f f1), timed alone, 44 algorithmic bytes per sampled pixel; "
+                          "raster_stats_ms": stats_ms,
+                          "raster_stats_tflops": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12,
+                          "raster_stats_alu_frac": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12 / fp32_peak_measured,
+                          "note": "tgs_raster_stats_sparse (f3): 15 flop per walked + 12 per blended pair (w, 3 sums, recomputed "
+                                  "distance). tgs_loss_sparse (SURVEY.md 8f f1), timed alone, 44 algorithmic bytes per sampled pixel; "
                                   "not inside the five-call step"},
             "kernels": kernels,
             "work": {"fwd_evals": walked, "bwd_evals": replayed, "blended": blended,
