@@ -226,6 +226,38 @@ class Oracle:
                                   _ptr(self.r(pix_err)), _ptr(o.stats), _ptr(o.depth))
         return o
 
+    # ---- O9: the paper's sampler and its maps, Eq. 3-4, 128-150 Eq. 7-8 ----
+    def sample_paper(self, cam, E_half, age, n_pix, n_hard, n_stable, seed=0):
+        """E_half: uint16 [H,W] fp16 bit patterns of the error map; age: uint16 [H,W]."""
+        H, W = cam.height, cam.width
+        gx, gy = self.grid(cam)
+        T = gx * gy
+        E = np.ascontiguousarray(E_half, np.uint16).reshape(H, W)
+        A = np.ascontiguousarray(age, np.uint16).reshape(H, W)
+        tiles = np.zeros(T, np.uint32)
+        tpo = np.zeros(T + 1, np.uint32)
+        pix = np.zeros(H * W, np.uint32)
+        kn = np.zeros(2, np.int32)
+        c = self.cam(cam)
+        self.lib.orc_sample_paper(C.byref(c), _ptr(E), _ptr(A), C.c_int(n_pix), C.c_int(n_hard), C.c_int(n_stable),
+                                  C.c_uint64(seed), _ptr(tiles), _ptr(tpo), _ptr(pix), _ptr(kn))
+        k, n = int(kn[0]), int(kn[1])
+        return SimpleNamespace(k=k, n=n, tiles=tiles[:k].copy(), tile_pix_offsets=tpo[:k + 1].copy(), pix=pix[:n].copy())
+
+    def maps_update(self, cam, E_half, age, pix, pix_err, beta):
+        """Returns the updated (E_half, age) copies (Eq. 3-4)."""
+        E = np.ascontiguousarray(E_half, np.uint16).copy()
+        A = np.ascontiguousarray(age, np.uint16).copy()
+        px = np.ascontiguousarray(pix, np.uint32)
+        er = np.ascontiguousarray(pix_err, np.float32)
+        c = self.cam(cam)
+        self.lib.orc_maps_update(C.byref(c), _ptr(E), _ptr(A), C.c_int(len(px)), _ptr(px), _ptr(er), C.c_float(beta))
+        return E, A
+
+    def float_to_half(self, f):
+        self.lib.orc_float_to_half.restype = C.c_uint16
+        return int(self.lib.orc_float_to_half(C.c_float(f)))
+
     # ---- small exported helpers (pinned individually) ---------------------------------------
     def quat_to_R(self, q):
         R = np.zeros(9, self.real)

@@ -814,3 +814,89 @@ void orc_raster_stats(const orc_cam* cam, int N, const uint32_t* tile_offsets, c
     for (size_t i = 0; i < (size_t)N * 3; ++i) stats[i] = (real)acc[i];
     free(acc);
 }
+
+/* O9 orc_sample_paper / orc_maps_update: the paper's own sampler and its persistent maps (SURVEY.md 8f row
+ * f2; Eq. 3-4, Sec. 3.5 Eq. 7-8).  Every tile is sampled with
+ * N = min(n_pix, #in-image pixels) pixels: n_hard by multinomial sampling WITHOUT replacement from
+ * pi_E (Eq. 7), n_stable by TopK of the age map over the rest (Eq. 8), the remainder uniformly without
+ * replacement.  Readings (R26-R29), all integer so that both sides agree bit for bit:
+ *   - weight of a pixel: q = 1 + trunc(min(E, 15.999) * 2^16) from the fp16 error map (E <= 0 or NaN -> 1): the
+ *     "+ eps" of Eq. 7 as one fixed-point unit per pixel, so a tile of zero errors is sampled uniformly
+ *   - draw d of tile t: r = mix64(seed, t << 16 | d) mod (sum of the remaining q); the pixel whose running sum
+ *     of q in ascending local index first exceeds r is taken and removed (sequential multinomial w/o replacement)
+ *   - TopK ties: larger age first, then smaller local index
+ *   - remainder draw d: r = mix64(seed ^ 0x5bd1e995a5a5a5a5, t << 16 | d) mod (#remaining): the r-th remaining pixel
+ *   - output: tiles = 0..T-1, per tile the chosen pixels in ascending local index (row-major inside the tile). */
+static float half_bits_to_float(uint16_t h) { _Float16 x; memcpy(&x, &h, 2); return (float)x; }
+static uint16_t float_to_half_bits(float f) { _Float16 x = (_Float16)f; uint16_t h; memcpy(&h, &x, 2); return h; }
+uint16_t orc_float_to_half(float f) { return float_to_half_bits(f); }
+float orc_half_to_float(uint16_t h) { return half_bits_to_float(h); }
+
+static uint32_t half_weight(uint16_t h) {
+    float e = half_bits_to_float(h);
+    if (!(e > 0.0f)) return 1u;
+    if (e > 15.999f) e = 15.999f;
+    return 1u + (uint32_t)(e * 65536.0f);
+}
+
+void orc_sample_paper(const orc_cam* cam, const uint16_t* E_half, const uint16_t* age, int n_pix, int n_hard,
+                      int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tpo, uint32_t* pix, int32_t* kn) {
+    const int W = cam->W, H = cam->H, gx = (W + TILE - 1) / TILE, gy = (H + TILE - 1) / TILE, T = gx * gy;
+    uint32_t n = 0;
+    for (int t = 0; t < T; ++t) {
+        const int tx = t % gx, ty = t / gx;
+        uint32_t q[256], ag[256], id[256];
+        int in[256], chosen[256], cnt = 0;
+        for (int l = 0; l < 256; ++l) {
+            int x = tx * TILE + (l % TILE), y = ty * TILE + (l / TILE);
+            in[l] = x < W && y < H;
+            chosen[l] = 0;
+            if (in[l]) {
+                id[l] = (uint32_t)(y * W + x);
+                q[l] = half_weight(E_half[id[l]]);
+                ag[l] = age[id[l]];
+                ++cnt;
+            }
+        }
+        const int N = imin(n_pix, cnt), Nh = imin(n_hard, N), Ns = imin(n_stable, N - Nh), Nr = N - Nh - Ns;
+        for (int d = 0; d < Nh; ++d) {                         /* Eq. 7: hard pixels */
+            uint64_t S = 0;
+            for (int l = 0; l < 256; ++l) if (in[l] && !chosen[l]) S += q[l];
+            uint64_t r = mix64(seed, ((uint64_t)t << 16) | (uint64_t)d) % S, acc = 0;
+            for (int l = 0; l < 256; ++l) if (in[l] && !chosen[l]) { acc += q[l]; if (r < acc) { chosen[l] = 1; break; } }
+        }
+        for (int d = 0; d < Ns; ++d) {                         /* Eq. 8: the oldest of the rest */
+            int best = -1;
+            for (int l = 0; l < 256; ++l) if (in[l] && !chosen[l] && (best < 0 || ag[l] > ag[best])) best = l;
+            chosen[best] = 1;
+        }
+        for (int d = 0; d < Nr; ++d) {                         /* remainder: uniform over what is left */
+            uint64_t R = 0;
+            for (int l = 0; l < 256; ++l) if (in[l] && !chosen[l]) ++R;
+            uint64_t r = mix64(seed ^ 0x5bd1e995a5a5a5a5ull, ((uint64_t)t << 16) | (uint64_t)d) % R, acc = 0;
+            for (int l = 0; l < 256; ++l) if (in[l] && !chosen[l]) { if (acc == r) { chosen[l] = 1; break; } ++acc; }
+        }
+        tiles[t] = (uint32_t)t;
+        tpo[t] = n;
+        for (int l = 0; l < 256; ++l) if (in[l] && chosen[l]) pix[n++] = id[l];
+    }
+    tpo[T] = n;
+    kn[0] = T; kn[1] = (int32_t)n;
+}
+
+/* Eq. 4 then Eq. 3: every age + 1 (saturating at 65535), sampled pixels reset to 0; at the sampled pixels
+ * E <- fp16( (1 - beta) * E + beta * e ) with the three operations rounded in fp32 (the paper stores E in half
+ * precision; arithmetic precision is this library's: fp32, R0). */
+void orc_maps_update(const orc_cam* cam, uint16_t* E_half, uint16_t* age, int n, const uint32_t* pix,
+                     const float* pix_err, float beta) {
+    const size_t np = (size_t)cam->W * (size_t)cam->H;
+    for (size_t p = 0; p < np; ++p) if (age[p] != 0xffffu) ++age[p];
+    const float omb = 1.0f - beta;
+    for (int i = 0; i < n; ++i) {
+        const uint32_t p = pix[i];
+        const float a = omb * half_bits_to_float(E_half[p]);
+        const float b = beta * pix_err[i];
+        E_half[p] = float_to_half_bits(a + b);
+        age[p] = 0;
+    }
+}

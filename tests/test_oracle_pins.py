@@ -860,3 +860,118 @@ def test_stats_vs_brute_force_definition(orc64):
     if not skip.any():
         assert np.allclose(r.stats, ref, rtol=1e-9, atol=1e-12)
     assert np.allclose(r.stats[:, 2].sum(), ref[:, 2].sum(), rtol=1e-3)
+
+
+# ---------------------------------------------------------------------------------------------
+# O9 pins: the paper's sampler and its maps (Eq. 3-4, 128-150 Eq. 7-8)
+def _half_bits(a):
+    return np.asarray(a, np.float32).astype(np.float16).view(np.uint16)
+
+
+def test_paper_sampler_structure(orc32):
+    """Every tile gets min(N_pix, #in-image pixels) distinct pixels of its own, ascending; tiles are 0..T-1."""
+    cam = cam_simple(75, 41)
+    rng = np.random.default_rng(0)
+    E = _half_bits(rng.random((41, 75)))
+    A = rng.integers(0, 30, (41, 75)).astype(np.uint16)
+    for n_pix, n_hard, n_stable in ((25, 10, 10), (200, 120, 60), (1, 0, 1), (7, 7, 0), (256, 0, 0)):
+        s = orc32.sample_paper(cam, E, A, n_pix, n_hard, n_stable, seed=5)
+        gx, gy = cam.grid
+        assert s.k == gx * gy and np.array_equal(s.tiles, np.arange(gx * gy))
+        for t in range(s.k):
+            p = s.pix[s.tile_pix_offsets[t]:s.tile_pix_offsets[t + 1]].astype(np.int64)
+            x, y = p % 75, p // 75
+            cnt = min(16, 75 - 16 * (t % gx)) * min(16, 41 - 16 * (t // gx))
+            assert len(p) == min(n_pix, cnt) and len(np.unique(p)) == len(p)
+            assert ((x // 16) == t % gx).all() and ((y // 16) == t // gx).all()
+            local = (y % 16) * 16 + (x % 16)
+            assert (np.diff(local) > 0).all()
+
+
+def test_paper_sampler_hard_set_is_multinomial_without_replacement(orc32):
+    """Eq. 7: inclusion probabilities of 2 draws without replacement from 6 pixels against the exact values
+    sum_j p_j p_i / (1 - p_j) + p_i, over 30000 seeds (4 sigma); zero errors give the uniform N/cnt."""
+    cam = cam_simple(3, 2)
+    e = np.array([[0.5, 0.05, 1.0], [0.25, 2.0, 0.125]], np.float32)
+    E = _half_bits(e)
+    A = np.zeros((2, 3), np.uint16)
+    q = 1.0 + np.floor(e.reshape(-1).astype(np.float64) * 65536.0)
+    p = q / q.sum()
+    exact = np.array([p[i] + sum(p[j] * p[i] / (1 - p[j]) for j in range(6) if j != i) for i in range(6)])
+    hits = np.zeros(6)
+    S = 30000
+    for seed in range(S):
+        s = orc32.sample_paper(cam, E, A, 2, 2, 0, seed=seed)
+        hits[s.pix] += 1
+    sigma = np.sqrt(exact * (1 - exact) / S)
+    assert (np.abs(hits / S - exact) < 4 * sigma).all(), (hits / S, exact)
+    hits[:] = 0
+    for seed in range(6000):
+        s = orc32.sample_paper(cam, np.zeros((2, 3), np.uint16), A, 2, 2, 0, seed=seed)
+        hits[s.pix] += 1
+    assert (np.abs(hits / 6000 - 2 / 6) < 4 * np.sqrt((1 / 3) * (2 / 3) / 6000)).all()
+    hits[:] = 0
+    for seed in range(6000):  # the remainder (neither hard nor stable) is uniform too
+        s = orc32.sample_paper(cam, E, A, 3, 0, 0, seed=seed)
+        hits[s.pix] += 1
+    assert (np.abs(hits / 6000 - 0.5) < 4 * np.sqrt(0.25 / 6000)).all()
+
+
+def test_paper_sampler_stable_set_is_topk_age(orc32):
+    """Eq. 8: with no hard pixels the stable set is the K oldest pixels of the tile (ties: lower local index);
+    with hard pixels it is the K oldest of the rest, disjoint from them."""
+    cam = cam_simple(40, 24)
+    rng = np.random.default_rng(3)
+    E = _half_bits(rng.random((24, 40)))
+    A = rng.integers(0, 6, (24, 40)).astype(np.uint16)  # many ties
+    gx, gy = cam.grid
+
+    def tile_pixels(t):
+        xs, ys = np.meshgrid(np.arange(16 * (t % gx), min(40, 16 * (t % gx) + 16)),
+                             np.arange(16 * (t // gx), min(24, 16 * (t // gx) + 16)))
+        return (ys * 40 + xs).reshape(-1)  # ascending local index
+
+    s = orc32.sample_paper(cam, E, A, 20, 0, 20, seed=1)
+    for t in range(s.k):
+        tp = tile_pixels(t)
+        order = np.lexsort((np.arange(len(tp)), -A.reshape(-1)[tp].astype(np.int64)))
+        want = np.sort(tp[order[:min(20, len(tp))]])
+        got = np.sort(s.pix[s.tile_pix_offsets[t]:s.tile_pix_offsets[t + 1]])
+        assert np.array_equal(got, want)
+    h = orc32.sample_paper(cam, E, A, 8, 8, 0, seed=9)       # the hard pixels alone (same draws)
+    b = orc32.sample_paper(cam, E, A, 20, 8, 12, seed=9)
+    for t in range(b.k):
+        tp = tile_pixels(t)
+        H = set(h.pix[h.tile_pix_offsets[t]:h.tile_pix_offsets[t + 1]].tolist())
+        P = set(b.pix[b.tile_pix_offsets[t]:b.tile_pix_offsets[t + 1]].tolist())
+        assert H <= P and len(P) == min(20, len(tp))
+        rest = np.array([p for p in tp if p not in H])
+        order = np.lexsort((np.arange(len(rest)), -A.reshape(-1)[rest].astype(np.int64)))
+        assert P - H == set(rest[order[:len(P) - len(H)]].tolist())
+
+
+def test_maps_update_eq3_eq4(orc32):
+    """Eq. 4: all ages + 1 (saturating), sampled reset; Eq. 3: fp16 EMA at the sampled pixels only, against numpy's
+    float16 (round to nearest even); the float -> half conversion on its edge cases."""
+    cam = cam_simple(37, 21)
+    rng = np.random.default_rng(4)
+    E = _half_bits(rng.random((21, 37)) * 3)
+    A = rng.integers(0, 65536, (21, 37)).astype(np.uint16)
+    A.reshape(-1)[:5] = 65535
+    s = orc32.sample_paper(cam, E, A, 30, 10, 10, seed=2)
+    e = (rng.random(s.n) * 2).astype(np.float32)
+    beta = np.float32(0.3)
+    E2, A2 = orc32.maps_update(cam, E, A, s.pix, e, float(beta))
+    wantA = np.minimum(A.astype(np.int64) + 1, 65535).reshape(-1)
+    wantA[s.pix] = 0
+    assert np.array_equal(A2.reshape(-1), wantA.astype(np.uint16))
+    Ef = E.view(np.float16).astype(np.float32).reshape(-1)
+    wantE = E.reshape(-1).copy()
+    upd = ((np.float32(1) - beta) * Ef[s.pix] + beta * e).astype(np.float16).view(np.uint16)
+    wantE[s.pix] = upd
+    assert np.array_equal(E2.reshape(-1), wantE)
+    for f in (0.0, 1.0, 65504.0, 65519.9, 65520.0, 1e9, 6.1e-5, 5.96e-8, 2.98e-8, 2.981e-8, 1.0 + 2.0 ** -11,
+              1.0 + 3 * 2.0 ** -11, -0.1, 0.1):
+        with np.errstate(over="ignore"):
+            want = int(np.float32(f).astype(np.float16).view(np.uint16))
+        assert orc32.float_to_half(f) == want, f
