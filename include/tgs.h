@@ -204,6 +204,29 @@ int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const fl
                             const uint32_t* pix, const float* pix_err,
                             float* stats, float* out_depth, void* stream);
 
+/* ---- f2: the paper's own per-tile sampler (Sec. 3.5 Eq. 7-8) and its
+ * persistent maps (Eq. 3-4).  EVERY tile is sampled with N = min(n_pix, #in-image pixels)
+ * pixels: min(n_hard, N) "hard" pixels by multinomial sampling WITHOUT replacement from the error prior
+ * pi_E (Eq. 7), then min(n_stable, rest) "stable" pixels = TopK of the age map over the remaining pixels
+ * (Eq. 8), the remainder (if n_hard + n_stable < n_pix) uniformly without replacement.
+ *   E_half[H,W]  error map, IEEE fp16 bit patterns;  age[H,W] uint16.
+ *   Integer decisions, identical on any machine: weight q = 1 + trunc(min(E, 15.999) * 2^16) (E <= 0 / NaN: 1);
+ *   hard draw d of tile t: r = mix64(seed, t << 16 | d) mod (sum of the remaining q), the pixel whose running
+ *   sum of q in ascending local index first exceeds r is taken and removed; TopK ties: lower local index;
+ *   remainder draw d: the (mix64(seed ^ 0x5bd1e995a5a5a5a5, t << 16 | d) mod #remaining)-th remaining pixel.
+ * Outputs as tgs_sample: tiles[T] = 0..T-1, tile_pix_offsets[T+1], pix[n] (ascending local index inside a
+ * tile), kn_dev = {T, n}; kn_host nullable (given: one sync).  workspace: tgs_sample_workspace_bytes. */
+int tgs_sample_paper(tgs_ctx* ctx, const tgs_camera* cam, const uint16_t* E_half, const uint16_t* age,
+                     int n_pix, int n_hard, int n_stable, uint64_t seed,
+                     uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+                     int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream);
+
+/* Eq. 4 then Eq. 3: every age + 1 (saturating at 65535) and the n = kn_dev[1] sampled pixels
+ * reset to 0; at the sampled pixels E <- fp16((1 - beta) E + beta pix_err[i]) (three fp32 roundings, then
+ * round-to-nearest-even to fp16); every other pixel of E is left unchanged.  Updates both maps in place. */
+int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
+                    const uint32_t* pix, const float* pix_err, float beta, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

@@ -25,7 +25,8 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
 # every symbol include/tgs.h declares (tests check the library exports them all)
 SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
-           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse"]
+           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse", "tgs_sample_paper",
+           "tgs_maps_update"]
 
 
 class TgsError(RuntimeError):
@@ -92,6 +93,9 @@ def load_library() -> C.CDLL:
     f32 = C.c_float
     lib.tgs_loss_sparse.argtypes = [vp, cam, i32, vp, vp, vp, vp, f32, f32, f32, vp, vp, vp, vp, vp]
     lib.tgs_raster_stats_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.tgs_sample_paper.argtypes = [vp, cam, vp, vp, i32, i32, i32, u64, vp, vp, vp, vp, C.POINTER(C.c_int32), vp,
+                                     C.c_size_t, vp]
+    lib.tgs_maps_update.argtypes = [vp, cam, vp, vp, vp, vp, vp, f32, vp]
     return lib
 
 
@@ -224,6 +228,36 @@ class TGS:
             assert kn[0] == out.k
             out.n = int(kn[1])
         return out
+
+    # ---- f2: the paper's own sampler (every tile, N_pix pixels each) and its maps ----
+    def sample_paper(self, cam, E_half, age, n_pix, n_hard, n_stable, seed=0, out=None, workspace=None, sync=True,
+                     stream=None):
+        """E_half: int16/uint16 device tensor [H,W] holding fp16 bit patterns (or a float16 tensor); age: int16 [H,W]."""
+        cam = Camera.of(cam)
+        T = cam.num_tiles
+        if out is None:
+            i32t = dict(dtype=torch.int32, device=self.device)
+            out = SimpleNamespace(tiles=torch.empty(T, **i32t), tile_pix_offsets=torch.empty(T + 1, **i32t),
+                                  pix=torch.empty(cam.width * cam.height, **i32t), kn_dev=torch.zeros(2, **i32t),
+                                  k=None, n=None)
+        if workspace is None:
+            workspace = torch.empty(self.sample_workspace_bytes(cam), dtype=torch.uint8, device=self.device)
+        kn = (C.c_int32 * 2)(-1, -1)
+        self._check(self.lib.tgs_sample_paper(self._h, C.byref(cam), _p(E_half), _p(age), int(n_pix), int(n_hard),
+                                              int(n_stable), C.c_uint64(seed), _p(out.tiles), _p(out.tile_pix_offsets),
+                                              _p(out.pix), _p(out.kn_dev), kn if sync else None, _p(workspace),
+                                              workspace.numel(), _stream(stream)))
+        out.k = T
+        if sync:
+            assert kn[0] == T
+            out.n = int(kn[1])
+        return out
+
+    def maps_update(self, cam, E_half, age, samp, pix_err, beta, stream=None):
+        """In place: Eq. 4 on age, Eq. 3 on E_half at the pixels of `samp` (its kn_dev gives n)."""
+        cam = Camera.of(cam)
+        self._check(self.lib.tgs_maps_update(self._h, C.byref(cam), _p(E_half), _p(age), _p(samp.kn_dev), _p(samp.pix),
+                                             _p(pix_err), float(beta), _stream(stream)))
 
     # ---- a4 ----
     def raster_fwd_sparse(self, cam, splats, binned, samp, n_capacity=None, want_walked=False, out=None, stream=None):

@@ -87,6 +87,12 @@ cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, c
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
                                float* dsh, cudaStream_t s);
 
+cudaError_t launch_sample_paper(const CamK& cam, const uint16_t* E_half, const uint16_t* age, int n_pix, int n_hard,
+                                int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tpo, uint32_t* pix,
+                                int32_t* kn_dev, void* ws, cudaStream_t s);
+cudaError_t launch_maps_update(const CamK& cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
+                               const uint32_t* pix, const float* pix_err, float beta, int num_sms, cudaStream_t s);
+
 cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                                 const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                                 const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,

@@ -2,6 +2,8 @@
 // lists ("sampled pixels are ordered by their tile indices",
 // 93 Eq. 2, 128-150 Sec. 3.5, 156 "tile-wise pixel offsets via prefix-sum").  Selection is done in
 // integers on a fixed-point copy of the error so that it is order independent and bit exact.
+#include <cuda_fp16.h>
+
 #include "common.cuh"
 
 namespace tgs {
@@ -201,6 +203,126 @@ write_pix_kernel(const CamK cam, int k, const uint32_t* __restrict__ tiles, cons
         if (bits & (1u << j)) pix[o++] = (uint32_t)(y * cam.W + xb + j);
 }
 
+// ---- f2: the paper's own sampler (Sec. 3.5 Eq. 7-8) and its maps (Eq. 3-4) ----
+// One warp per tile, every tile sampled.  Lane l owns local pixels 8l .. 8l+7.  All decisions are integer
+// (R26-R29): weight q = 1 + trunc(min(E, 15.999) * 2^16) from the fp16 error map; hard draw d takes
+// the pixel whose running sum of q first exceeds mix64(seed, t << 16 | d) mod (sum of remaining q) and removes
+// it (sequential multinomial sampling without replacement: a warp scan per draw); the stable set is the TopK of
+// the age map over the rest (a warp max per pick; ties: lower local index); the remainder is uniform.
+__device__ __forceinline__ uint32_t half_weight(uint16_t h) {
+    float e = __half2float(__ushort_as_half(h));
+    if (!(e > 0.0f)) return 1u;  // zero, negative, NaN
+    e = fminf(e, kErrClamp);
+    return 1u + (uint32_t)(e * 65536.0f);
+}
+
+__device__ __forceinline__ uint32_t warp_incl_scan_u32(uint32_t v, int lane) {
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += y;
+    }
+    return v;
+}
+
+__global__ void __launch_bounds__(256)
+paper_tile_kernel(const CamK cam, const uint16_t* __restrict__ E_half, const uint16_t* __restrict__ age, int n_pix,
+                  int n_hard, int n_stable, uint64_t seed, TileMeta* __restrict__ meta, uint32_t* __restrict__ selected) {
+    const int T = cam.gx * cam.gy;
+    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (t >= T) return;
+    const int lane = threadIdx.x & 31;
+    const int tx = t % cam.gx, ty = t / cam.gx;
+    const int y = ty * kTile + (lane >> 1), xb = tx * kTile + (lane & 1) * 8;
+    uint32_t q[8], ag[8];
+    uint32_t avail = 0;  // bit j: pixel j of this lane is inside the image and not chosen yet
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        q[j] = 0u; ag[j] = 0u;
+        if (y < cam.H && xb + j < cam.W) {
+            const size_t p = (size_t)y * cam.W + xb + j;
+            q[j] = half_weight(E_half[p]);
+            ag[j] = age[p];
+            avail |= 1u << j;
+        }
+    }
+    uint32_t chosen = 0;
+    const int cnt = (int)__reduce_add_sync(0xffffffffu, (uint32_t)__popc(avail));
+    const int N = min(n_pix, cnt), Nh = min(n_hard, N), Ns = min(n_stable, N - Nh), Nr = N - Nh - Ns;
+    const uint64_t tkey = (uint64_t)(uint32_t)t << 16;
+    // ---- Eq. 7: hard pixels ----
+    for (int d = 0; d < Nh; ++d) {
+        uint32_t sum = 0;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) sum += ((avail >> j) & 1u) ? q[j] : 0u;
+        const uint32_t incl = warp_incl_scan_u32(sum, lane);
+        const uint32_t S = __shfl_sync(0xffffffffu, incl, 31);
+        const uint32_t r = (uint32_t)(mix64(seed, tkey | (uint64_t)d) % (uint64_t)S);
+        uint32_t acc = incl - sum;
+        if (r >= acc && r < incl) {  // exactly one lane
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if ((avail >> j) & 1u) {
+                    acc += q[j];
+                    if (r < acc) { avail &= ~(1u << j); chosen |= 1u << j; acc = 0xffffffffu; break; }
+                }
+            }
+        }
+    }
+    // ---- Eq. 8: the oldest of the rest ----
+    for (int d = 0; d < Ns; ++d) {
+        uint32_t best = 0;  // (age + 1) << 8 | 255 - local index; 0 = nothing available
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            if ((avail >> j) & 1u) best = max(best, ((ag[j] + 1u) << 8) | (uint32_t)(255 - (lane * 8 + j)));
+        const uint32_t win = __reduce_max_sync(0xffffffffu, best);
+        const int l = 255 - (int)(win & 255u);
+        if ((l >> 3) == lane) { avail &= ~(1u << (l & 7)); chosen |= 1u << (l & 7); }
+    }
+    // ---- remainder: uniform over what is left ----
+    for (int d = 0; d < Nr; ++d) {
+        const uint32_t c = (uint32_t)__popc(avail);
+        const uint32_t incl = warp_incl_scan_u32(c, lane);
+        const uint32_t R = __shfl_sync(0xffffffffu, incl, 31);
+        const uint32_t r = (uint32_t)(mix64(seed ^ 0x5bd1e995a5a5a5a5ull, tkey | (uint64_t)d) % (uint64_t)R);
+        const uint32_t excl = incl - c;
+        if (r >= excl && r < incl) {
+            const int j = __fns(avail, 0, (int)(r - excl) + 1);  // the (r - excl)-th set bit
+            avail &= ~(1u << j);
+            chosen |= 1u << j;
+        }
+    }
+    // keep mask: word w holds local indices 32w .. 32w+31 = the bytes of lanes 4w .. 4w+3
+    uint32_t v = chosen << ((lane & 3) * 8);
+    v |= __shfl_xor_sync(0xffffffffu, v, 1);
+    v |= __shfl_xor_sync(0xffffffffu, v, 2);
+    if ((lane & 3) == 0) meta[t].mask[lane >> 2] = v;
+    if (lane == 0) { meta[t].npix = (uint32_t)N; selected[t] = 1u; }
+}
+
+// Eq. 4: every age + 1 (saturating at 65535); the sampled pixels are reset by maps_sampled_kernel
+__global__ void __launch_bounds__(256) age_increment_kernel(size_t npix, uint16_t* __restrict__ age) {
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < npix; p += (size_t)gridDim.x * blockDim.x) {
+        const uint16_t a = age[p];
+        if (a != 0xffffu) age[p] = (uint16_t)(a + 1u);
+    }
+}
+
+// Eq. 3 at the sampled pixels: E <- fp16((1 - beta) E + beta e), three fp32 roundings; age <- 0
+__global__ void __launch_bounds__(256)
+maps_sampled_kernel(const int32_t* __restrict__ kn_dev, const uint32_t* __restrict__ pix, const float* __restrict__ pix_err,
+                    float beta, uint16_t* __restrict__ E_half, uint16_t* __restrict__ age) {
+    const int n = kn_dev[1];
+    const float omb = __fsub_rn(1.0f, beta);
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const uint32_t p = pix[i];
+        const float a = __fmul_rn(omb, __half2float(__ushort_as_half(E_half[p])));
+        const float b = __fmul_rn(beta, pix_err[i]);
+        E_half[p] = __half_as_ushort(__float2half_rn(__fadd_rn(a, b)));
+        age[p] = 0;
+    }
+}
+
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 }  // namespace
@@ -221,6 +343,30 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
     tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);
     write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);
     count_launches(4);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_sample_paper(const CamK& cam, const uint16_t* E_half, const uint16_t* age, int n_pix, int n_hard,
+                                int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tpo, uint32_t* pix,
+                                int32_t* kn_dev, void* ws, cudaStream_t s) {
+    const int T = cam.gx * cam.gy;
+    TileMeta* meta = (TileMeta*)ws;
+    uint32_t* selected = (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
+    paper_tile_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, E_half, age, n_pix, n_hard, n_stable, seed, meta, selected);
+    tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);
+    write_pix_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, T, tiles, tpo, meta, pix);
+    count_launches(3);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_maps_update(const CamK& cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
+                               const uint32_t* pix, const float* pix_err, float beta, int num_sms, cudaStream_t s) {
+    const size_t npix = (size_t)cam.W * (size_t)cam.H;
+    int blocks = (int)((npix + 255) / 256);
+    if (blocks > num_sms * 16) blocks = num_sms * 16;
+    age_increment_kernel<<<blocks, 256, 0, s>>>(npix, age);
+    maps_sampled_kernel<<<blocks, 256, 0, s>>>(kn_dev, pix, pix_err, beta, E_half, age);
+    count_launches(2);
     return cudaGetLastError();
 }
 

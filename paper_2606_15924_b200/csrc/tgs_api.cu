@@ -315,4 +315,42 @@ int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const fl
     return TGS_OK;
 }
 
+int tgs_sample_paper(tgs_ctx* ctx, const tgs_camera* cam, const uint16_t* E_half, const uint16_t* age, int n_pix,
+                     int n_hard, int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+                     int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample_paper: bad camera");
+    if (n_pix < 1 || n_pix > 256 || n_hard < 0 || n_stable < 0 || n_hard + n_stable > n_pix)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample_paper: need 1 <= n_pix <= 256 and n_hard + n_stable <= n_pix (got %d, %d, %d)",
+                    n_pix, n_hard, n_stable);
+    if (!E_half || !age || !tiles || !tile_pix_offsets || !pix || !kn_dev || !workspace)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample_paper: null pointer");
+    const int T = num_tiles(cam);
+    if (T > (1 << 20)) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_sample_paper: T > 2^20");
+    const size_t need = sample_workspace_bytes(T);
+    if (workspace_bytes < need)
+        return fail(ctx, TGS_ERR_CAPACITY, "tgs_sample_paper: workspace %zu B < required %zu B", workspace_bytes, need);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = launch_sample_paper(make_camk(cam), E_half, age, n_pix, n_hard, n_stable, seed, tiles, tile_pix_offsets,
+                                        pix, kn_dev, workspace, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_sample_paper", e);
+    if (kn_host) {
+        e = cudaMemcpyAsync(kn_host, kn_dev, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return cuda_fail(ctx, "tgs_sample_paper (k, n readback)", e);
+    }
+    return TGS_OK;
+}
+
+int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
+                    const uint32_t* pix, const float* pix_err, float beta, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: bad camera");
+    if (!(beta >= 0.f && beta <= 1.f)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: beta outside [0, 1]");
+    if (!E_half || !age || !kn_dev || !pix || !pix_err) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: null pointer");
+    cudaError_t e = launch_maps_update(make_camk(cam), E_half, age, kn_dev, pix, pix_err, beta, ctx->num_sms, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_maps_update", e);
+    return TGS_OK;
+}
+
 }  // extern "C"

@@ -508,3 +508,85 @@ def test_raster_stats_partial_tiles_and_empty(orc32, tgs, torch):
     out0 = tgs.raster_stats_sparse(sc.cam, splats, binned_dev(b, torch, sc.cam.num_tiles), empty, dev(ones[:1], torch))
     torch.cuda.synchronize()
     assert (out0.stats.cpu().numpy() == 0).all()
+
+
+# ---- f2: tgs_sample_paper / tgs_maps_update against the oracle's O9 (Eq. 3-4, 7-8): bit exact ----
+def _maps(rng, W, H, zero_frac=0.0):
+    e = (rng.random((H, W)) ** 3 * 4).astype(np.float32)
+    e[rng.random((H, W)) < zero_frac] = 0
+    E = e.astype(np.float16).view(np.uint16)
+    A = rng.integers(0, 40, (H, W)).astype(np.uint16)
+    return E, A
+
+
+@pytest.mark.parametrize("W,H,n_pix,n_hard,n_stable", [(128, 128, 25, 10, 10), (203, 117, 64, 40, 24), (75, 41, 256, 100, 100),
+                                                      (980, 545, 25, 12, 8), (64, 48, 1, 0, 0), (333, 77, 85, 85, 0)])
+def test_sample_paper_bit_exact(W, H, n_pix, n_hard, n_stable, orc32, tgs, torch):
+    cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    rng = np.random.default_rng(W + H)
+    E, A = _maps(rng, W, H, zero_frac=0.3)
+    ref = orc32.sample_paper(cam, E, A, n_pix, n_hard, n_stable, seed=77)
+    Ed, Ad = dev(E.view(np.int16), torch), dev(A.view(np.int16), torch)
+    out = tgs.sample_paper(cam, Ed, Ad, n_pix, n_hard, n_stable, seed=77)
+    assert (out.k, out.n) == (ref.k, ref.n)
+    assert np.array_equal(u32(out.tiles)[:ref.k], ref.tiles)
+    assert np.array_equal(u32(out.tile_pix_offsets)[:ref.k + 1], ref.tile_pix_offsets)
+    assert np.array_equal(u32(out.pix)[:ref.n], ref.pix)
+    # maps: Eq. 3-4 in place
+    e = (rng.random(ref.n) * 3).astype(np.float32)
+    E2, A2 = orc32.maps_update(cam, E, A, ref.pix, e, 0.2)
+    tgs.maps_update(cam, Ed, Ad, out, dev(e, torch), 0.2)
+    torch.cuda.synchronize()
+    assert np.array_equal(Ed.cpu().numpy().view(np.uint16), E2)
+    assert np.array_equal(Ad.cpu().numpy().view(np.uint16), A2)
+
+
+def test_sample_paper_degenerate_maps(orc32, tgs, torch):
+    """All-zero error map (uniform draws), saturated and equal ages (ties by index), NaN / inf / negative errors."""
+    W, H = 90, 50
+    cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    rng = np.random.default_rng(1)
+    cases = []
+    cases.append((np.zeros((H, W), np.uint16), np.full((H, W), 65535, np.uint16)))
+    e = rng.random((H, W)).astype(np.float32)
+    e[::3, ::2] = np.nan; e[1::4, 1::3] = np.inf; e[2::5, :] = -1.0; e[0, 0] = 65504.0
+    cases.append((e.astype(np.float16).view(np.uint16), np.zeros((H, W), np.uint16)))
+    for E, A in cases:
+        ref = orc32.sample_paper(cam, E, A, 40, 15, 15, seed=3)
+        out = tgs.sample_paper(cam, dev(E.view(np.int16), torch), dev(A.view(np.int16), torch), 40, 15, 15, seed=3)
+        assert out.n == ref.n and np.array_equal(u32(out.pix)[:ref.n], ref.pix)
+        Ed, Ad = dev(E.view(np.int16), torch), dev(A.view(np.int16), torch)
+        pe = rng.random(ref.n).astype(np.float32)
+        E2, A2 = orc32.maps_update(cam, E, A, ref.pix, pe, 0.5)
+        tgs.maps_update(cam, Ed, Ad, out, dev(pe, torch), 0.5)
+        torch.cuda.synchronize()
+        assert np.array_equal(Ad.cpu().numpy().view(np.uint16), A2)
+        got, want = Ed.cpu().numpy().view(np.uint16), E2
+        nan = lambda b: (b & 0x7c00) == 0x7c00  # NaN payloads may differ; NaN / inf class and everything else must agree
+        assert np.array_equal(nan(got), nan(want)) and np.array_equal(got[~nan(got)], want[~nan(want)])
+
+
+def test_paper_sampler_drives_the_raster(orc32, tgs, torch):
+    """The paper's pixel lists (few pixels in every tile: all units partial) through forward and backward."""
+    r = oracle_run("small_rot", orc32)
+    sc = r.sc
+    W, H = sc.cam.width, sc.cam.height
+    E, A = _maps(np.random.default_rng(8), W, H)
+    s = orc32.sample_paper(sc.cam, E, A, 25, 10, 10, seed=4)
+    b = orc32.bin_sort(sc.cam, r.pre)
+    fw = orc32.raster_fwd(sc.cam, b, r.pre, s)
+    g = workloads.dl_dcolor(3, s.n)
+    rb = orc32.raster_bwd(sc.cam, b, r.pre, s, fw, g)
+    splats = dev(pack_splats(r.pre), torch)
+    sd = tgs.sample_paper(sc.cam, dev(E.view(np.int16), torch), dev(A.view(np.int16), torch), 25, 10, 10, seed=4)
+    assert sd.n == s.n and np.array_equal(u32(sd.pix)[:s.n], s.pix)
+    bd = binned_dev(b, torch, sc.cam.num_tiles)
+    out = tgs.raster_fwd_sparse(sc.cam, splats, bd, sd)
+    torch.cuda.synchronize()
+    check_forward(out.color[:s.n].cpu().numpy(), out.T[:s.n].cpu().numpy(), u32(out.n_contrib)[:s.n], fw)
+    bw = tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, bd, sd, out, dev(g, torch), project=False)
+    torch.cuda.synchronize()
+    got = bw.dL_dsplats.cpu().numpy()  # [N,12]: 0..1 dL/dmean2D, 2..4 conic, 5 opacity, 6..8 rgb
+    good = tainted_gaussians(sc.N, b, s, fw)
+    check_grad("dL_dmean2D", got[:, 0:2], rb.dL_dmeans2D, good)
+    check_grad("dL_drgb", got[:, 6:9], rb.dL_drgb, good)
