@@ -288,6 +288,42 @@ def run_tgs(args):
         stats_ms += la.elapsed_time(lb)
     stats_ms /= args.steps
 
+    # the paper's own regime -- N_pix = 25 pixels (r = 10 %) in EVERY tile, 40 % hard,
+    # 40 % stable -- sampler, binning of all tiles, sparse forward / backward on those lists, map updates
+    paper = None
+    if world == 1:
+        gE = torch.Generator(device=dev).manual_seed(1)
+        E_half = (torch.rand((cam.height, cam.width), device=dev, generator=gE) ** 3).to(torch.float16).view(torch.int16)
+        age = torch.randint(0, 50, (cam.height, cam.width), device=dev, generator=gE, dtype=torch.int32).to(torch.int16)
+        sp = tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1)
+        bp = tg.bin_sort(cam, st.pre.splats, P_est + 1024, workspace=st.ws_sort, sync=True)
+        fp = tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp)
+        gp = torch.randn((sp.n, 3), device=dev, generator=gE) / sp.n
+        ob = SimpleNamespace(dL_dsplats=st.bwd.dL_dsplats)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+        accp = [0.0] * 5
+        for _ in range(args.steps):
+            flush.fill_(1.0)
+            ev[0].record()
+            tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1, out=sp, workspace=st.ws_sample, sync=False)
+            ev[1].record()
+            tg.bin_sort(cam, st.pre.splats, P_est + 1024, out=bp, workspace=st.ws_sort, sync=False)
+            ev[2].record()
+            tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp, out=fp)
+            ev[3].record()
+            tg.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, bp, sp, fp, gp, project=False, out=st.bwd)
+            ev[4].record()
+            tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.2)
+            ev[5].record()
+            torch.cuda.synchronize()
+            for i_ in range(5):
+                accp[i_] += ev[i_].elapsed_time(ev[i_ + 1])
+        paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 10, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
+                 "sample_paper_ms": accp[0] / args.steps, "bin_sort_all_tiles_ms": accp[1] / args.steps,
+                 "raster_fwd_ms": accp[2] / args.steps, "raster_bwd_ms": accp[3] / args.steps,
+                 "maps_update_ms": accp[4] / args.steps,
+                 "raster_px_per_s": sp.n / ((accp[2] + accp[3]) / args.steps * 1e-3)}
+
     # ---- roofline of the dominant kernel ----
     peaks, peak_src = measured_peaks()
     fwd_flops = FWD_FLOPS_WALK * walked + FWD_FLOPS_BLEND * blended
@@ -371,6 +407,7 @@ def run_tgs(args):
             "per_call_ms": per_call_ms,
             "next_rows": {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
                           "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                          "paper_regime": paper,
                           "raster_stats_ms": stats_ms,
                           "raster_stats_tflops": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12,
                           "raster_stats_alu_frac": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12 / fp32_peak_measured,
