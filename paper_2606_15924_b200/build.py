@@ -27,6 +27,7 @@ SOURCES = {
     "project_bwd.cu": [],
     "loss.cu": [],
     "raster_stats.cu": [],
+    "raster_lite.cu": [],
 }
 
 

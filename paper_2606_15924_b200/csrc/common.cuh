@@ -19,10 +19,18 @@ constexpr float kAlphaMin = 0.00392156862745098f;  // 1/255
 constexpr float kAlphaMax = 0.99f;
 constexpr float kTMin = 0.0001f;
 
+// A second stream of the context: the warp-per-tile raster kernel of a call runs on it, concurrently with the
+// block-per-tile kernel on the caller's stream (fork / join by events; capturable in a CUDA graph).
+struct SideStream {
+    cudaStream_t aux;
+    cudaEvent_t fork, join;
+};
+
 struct ctx_impl {
     int device;
     int num_sms;
     uint32_t* sched;  // device, 8 words: work-unit counters of the persistent raster kernels (self re-arming)
+    SideStream side;
     char err[512];
 };
 
@@ -75,12 +83,23 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s);
+                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s,
+                              const SideStream* side);
 
 cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
-                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s);
+                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s,
+                              const SideStream* side);
+
+cudaError_t launch_raster_fwd_lite(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
+                                   const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                                   const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
+                                   uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s);
+cudaError_t launch_raster_bwd_lite(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
+                                   const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                                   const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
+                                   const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s);
 
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                                const float* sh, const int32_t* radii, const uint8_t* clamped,

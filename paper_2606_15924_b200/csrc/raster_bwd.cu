@@ -56,7 +56,7 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ring_init(sm.ring);
     if (warp == kConsumers) {
-        producer_loop<true>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, n_contrib, sched, lane);
+        producer_loop<true>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, n_contrib, sched, lane, kLitePixels);
         return;
     }
     Ring<kBwdStageEntries>& R = sm.ring;
@@ -223,10 +223,20 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
 cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
-                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s) {
+                              const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s,
+                              const SideStream* side) {
     cudaError_t e = cudaMemsetAsync(dL_dsplats, 0, (size_t)N * kSplatWords * sizeof(float), s);
     if (e != cudaSuccess) return e;
     if (k <= 0) return cudaSuccess;
+    // fork (after the memset): the warp-per-tile kernel for tiles with <= kLitePixels sampled pixels runs on the
+    // side stream, concurrently with the block-per-tile kernel; both accumulate with atomics
+    e = cudaEventRecord(side->fork, s);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(side->aux, side->fork, 0);
+    if (e == cudaSuccess)
+        e = launch_raster_bwd_lite(cam, splats, tile_offsets, gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
+                                   dL_dsplats, sched + 2, num_sms, side->aux);
+    if (e == cudaSuccess) e = cudaEventRecord(side->join, side->aux);
+    if (e != cudaSuccess) return e;
     int blocks = num_sms * 3;
     if (blocks > k) blocks = k;
     constexpr size_t smem = sizeof(BwdShared);
@@ -240,7 +250,9 @@ cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const
                                                           gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
                                                           dL_dsplats, sched);
     count_launches(1);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return cudaStreamWaitEvent(s, side->join, 0);  // join
 }
 
 }  // namespace tgs

@@ -32,6 +32,7 @@ namespace tgs {
 constexpr int kConsumers = 8;                        // consumer warps per block = units per tile
 constexpr int kRasterThreads = (kConsumers + 1) * 32;  // + 1 producer warp
 constexpr int kStages = 4;
+constexpr uint32_t kLitePixels = 32;  // tiles with at most this many sampled pixels go to the warp-per-tile kernels (raster_lite.cu)
 constexpr uint32_t kHdrCont = 0xfffffffeu, kHdrEnd = 0xffffffffu;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
@@ -197,13 +198,14 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                                               const uint32_t* __restrict__ gid_sorted, uint32_t k,
                                               const uint32_t* __restrict__ tiles, const uint32_t* __restrict__ tpo,
                                               const uint32_t* __restrict__ n_contrib, uint32_t* __restrict__ sched,
-                                              int lane) {
+                                              int lane, uint32_t lite_max = 0u) {
     uint32_t gchunk = 0, seq = 0;
     for (;;) {
         uint32_t it = 0;
         if (lane == 0) it = atomicAdd(&sched[0], 1u);
         it = __shfl_sync(0xffffffffu, it, 0);
         if (it >= k) break;
+        if (lite_max != 0u && tpo[it + 1] - tpo[it] <= lite_max) continue;  // a warp-per-tile kernel's tile
         ++seq;
         const uint32_t t = tiles[it];
         const uint32_t start = tile_offsets[t];

@@ -33,7 +33,7 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ring_init(sm.ring);
     if (warp == kConsumers) {
-        producer_loop<false>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, nullptr, sched, lane);
+        producer_loop<false>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, nullptr, sched, lane, kLitePixels);
         return;
     }
     Ring<128>& R = sm.ring;
@@ -153,8 +153,18 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,
-                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s) {
+                              uint32_t* n_walked, uint32_t* n_blended, uint32_t* sched, int num_sms, cudaStream_t s,
+                              const SideStream* side) {
     if (k <= 0) return cudaSuccess;
+    // fork: tiles with <= kLitePixels sampled pixels go to the warp-per-tile kernel (raster_lite.cu; its own
+    // counters at sched + 2) on the context's side stream, concurrently with the block-per-tile kernel
+    cudaError_t e = cudaEventRecord(side->fork, s);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(side->aux, side->fork, 0);
+    if (e == cudaSuccess)
+        e = launch_raster_fwd_lite(cam, splats, tile_offsets, gid_sorted, k, tiles, tpo, pix, out_color, out_T, n_contrib,
+                                   n_walked, n_blended, sched + 2, num_sms, side->aux);
+    if (e == cudaSuccess) e = cudaEventRecord(side->join, side->aux);
+    if (e != cudaSuccess) return e;
     const bool count = n_walked || n_blended;
     // persistent grid: one block per sampled tile at a time
     int blocks = num_sms * 4;
@@ -167,7 +177,9 @@ cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32
         raster_fwd_kernel<false><<<blocks, kRasterThreads, 0, s>>>(cam, sp, tile_offsets, gid_sorted, k, tiles, tpo, pix,
                                                                    out_color, out_T, n_contrib, n_walked, n_blended, sched);
     count_launches(1);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return cudaStreamWaitEvent(s, side->join, 0);  // join
 }
 
 }  // namespace tgs

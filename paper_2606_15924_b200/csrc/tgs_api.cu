@@ -68,13 +68,21 @@ int tgs_create(tgs_ctx** out, int device) {
     // the only allocation the library ever makes: 32 bytes of scheduler counters, once per context
     e = cudaMalloc((void**)&c->sched, 8 * sizeof(uint32_t));
     if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 8 * sizeof(uint32_t));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side.aux, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->side.fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->side.join, cudaEventDisableTiming);
     if (e != cudaSuccess) { delete c; return TGS_ERR_CUDA; }
     *out = c;
     return TGS_OK;
 }
 
 int tgs_destroy(tgs_ctx* ctx) {
-    if (ctx && ctx->sched) cudaFree(ctx->sched);
+    if (ctx && ctx->sched) {
+        cudaFree(ctx->sched);
+        cudaEventDestroy(ctx->side.fork);
+        cudaEventDestroy(ctx->side.join);
+        cudaStreamDestroy(ctx->side.aux);
+    }
     delete ctx;
     return TGS_OK;
 }
@@ -245,7 +253,8 @@ int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const floa
     if (!splats || !tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !out_color || !out_T || !n_contrib)
         return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: null pointer");
     cudaError_t e = launch_raster_fwd(make_camk(cam), splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix,
-                                      out_color, out_T, n_contrib, n_walked, n_blended, ctx->sched, ctx->num_sms, (cudaStream_t)stream);
+                                      out_color, out_T, n_contrib, n_walked, n_blended, ctx->sched, ctx->num_sms, (cudaStream_t)stream,
+                                      &ctx->side);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_fwd_sparse", e);
     return TGS_OK;
 }
@@ -268,7 +277,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
     cudaStream_t s = (cudaStream_t)stream;
     const CamK ck = make_camk(cam);
     cudaError_t e = launch_raster_bwd(ck, N, splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix, out_T,
-                                      n_contrib, dL_dcolor, dL_dsplats, ctx->sched + 4, ctx->num_sms, s);
+                                      n_contrib, dL_dcolor, dL_dsplats, ctx->sched + 4, ctx->num_sms, s, &ctx->side);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (raster)", e);
     if (dL_dmeans3D) {
         if (!dL_dscales || !dL_dquats || !dL_dopacities || !dL_dsh || !means3D || !scales || !quats || !sh || !radii || !clamped)
