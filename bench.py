@@ -261,68 +261,82 @@ def run_tgs(args):
         acc["project_bwd"] += max(d[5] - d[4], 0.0)  # second call = raster + projection
     per_call_ms = {k_: v / args.steps for k_, v in acc.items()}
 
-    # ---- SURVEY.md 8f f1 (not part of the five-call step): the fused sparse loss between forward and backward ----
-    target_dev = torch.rand((cam.height, cam.width, 3), device=dev, generator=torch.Generator(device=dev).manual_seed(0))
-    lo = tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
-                        st.fwd.color, target_dev, n_capacity=cam.width * cam.height)
-    la, lb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    loss_ms = 0.0
-    for _ in range(args.steps):
-        flush.fill_(1.0)
-        la.record()
-        tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
-                       st.fwd.color, target_dev, out=lo)
-        lb.record()
-        torch.cuda.synchronize()
-        loss_ms += la.elapsed_time(lb)
-    loss_ms /= args.steps
-    # the statistics forward (E_i, D_i, W_i, expected depth), fed with the loss kernel's per-pixel error
-    so = tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, n_capacity=cam.width * cam.height)
-    stats_ms = 0.0
-    for _ in range(args.steps):
-        flush.fill_(1.0)
-        la.record()
-        tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, out=so)
-        lb.record()
-        torch.cuda.synchronize()
-        stats_ms += la.elapsed_time(lb)
-    stats_ms /= args.steps
-
-    # the paper's own regime -- N_pix = 25 pixels (r = 10 %) in EVERY tile, 40 % hard,
-    # 40 % stable -- sampler, binning of all tiles, sparse forward / backward on those lists, map updates
-    paper = None
-    if world == 1:
-        gE = torch.Generator(device=dev).manual_seed(1)
-        E_half = (torch.rand((cam.height, cam.width), device=dev, generator=gE) ** 3).to(torch.float16).view(torch.int16)
-        age = torch.randint(0, 50, (cam.height, cam.width), device=dev, generator=gE, dtype=torch.int32).to(torch.int16)
-        sp = tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1)
-        bp = tg.bin_sort(cam, st.pre.splats, P_est + 1024, workspace=st.ws_sort, sync=True)
-        fp = tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp)
-        gp = torch.randn((sp.n, 3), device=dev, generator=gE) / sp.n
-        ob = SimpleNamespace(dL_dsplats=st.bwd.dL_dsplats)
-        ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
-        accp = [0.0] * 5
+    peaks, peak_src = measured_peaks()
+    next_rows = None
+    if not args.step_only:
+        # ---- SURVEY.md 8f f1 (not part of the five-call step): the fused sparse loss between forward and backward ----
+        target_dev = torch.rand((cam.height, cam.width, 3), device=dev, generator=torch.Generator(device=dev).manual_seed(0))
+        lo = tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
+                            st.fwd.color, target_dev, n_capacity=cam.width * cam.height)
+        la, lb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        loss_ms = 0.0
         for _ in range(args.steps):
             flush.fill_(1.0)
-            ev[0].record()
-            tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1, out=sp, workspace=st.ws_sample, sync=False)
-            ev[1].record()
-            tg.bin_sort(cam, st.pre.splats, P_est + 1024, out=bp, workspace=st.ws_sort, sync=False)
-            ev[2].record()
-            tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp, out=fp)
-            ev[3].record()
-            tg.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, bp, sp, fp, gp, project=False, out=st.bwd)
-            ev[4].record()
-            tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.2)
-            ev[5].record()
+            la.record()
+            tg.loss_sparse(cam, SimpleNamespace(k=k, n=n, tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix),
+                           st.fwd.color, target_dev, out=lo)
+            lb.record()
             torch.cuda.synchronize()
-            for i_ in range(5):
-                accp[i_] += ev[i_].elapsed_time(ev[i_ + 1])
-        paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 10, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
-                 "sample_paper_ms": accp[0] / args.steps, "bin_sort_all_tiles_ms": accp[1] / args.steps,
-                 "raster_fwd_ms": accp[2] / args.steps, "raster_bwd_ms": accp[3] / args.steps,
-                 "maps_update_ms": accp[4] / args.steps,
-                 "raster_px_per_s": sp.n / ((accp[2] + accp[3]) / args.steps * 1e-3)}
+            loss_ms += la.elapsed_time(lb)
+        loss_ms /= args.steps
+        # the statistics forward (E_i, D_i, W_i, expected depth), fed with the loss kernel's per-pixel error
+        so = tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, n_capacity=cam.width * cam.height)
+        stats_ms = 0.0
+        for _ in range(args.steps):
+            flush.fill_(1.0)
+            la.record()
+            tg.raster_stats_sparse(cam, st.pre.splats, st.binned, st.samp, lo.pix_err, out=so)
+            lb.record()
+            torch.cuda.synchronize()
+            stats_ms += la.elapsed_time(lb)
+        stats_ms /= args.steps
+
+        # the paper's own regime -- N_pix = 25 pixels (r = 10 %) in EVERY tile, 40 % hard,
+        # 40 % stable -- sampler, binning of all tiles, sparse forward / backward on those lists, map updates
+        paper = None
+        if world == 1:
+            gE = torch.Generator(device=dev).manual_seed(1)
+            E_half = (torch.rand((cam.height, cam.width), device=dev, generator=gE) ** 3).to(torch.float16).view(torch.int16)
+            age = torch.randint(0, 50, (cam.height, cam.width), device=dev, generator=gE, dtype=torch.int32).to(torch.int16)
+            sp = tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1)
+            bp = tg.bin_sort(cam, st.pre.splats, P_est + 1024, workspace=st.ws_sort, sync=True)
+            fp = tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp)
+            gp = torch.randn((sp.n, 3), device=dev, generator=gE) / sp.n
+            ob = SimpleNamespace(dL_dsplats=st.bwd.dL_dsplats)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
+            accp = [0.0] * 5
+            for _ in range(args.steps):
+                flush.fill_(1.0)
+                ev[0].record()
+                tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1, out=sp, workspace=st.ws_sample, sync=False)
+                ev[1].record()
+                tg.bin_sort(cam, st.pre.splats, P_est + 1024, out=bp, workspace=st.ws_sort, sync=False)
+                ev[2].record()
+                tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp, out=fp)
+                ev[3].record()
+                tg.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, bp, sp, fp, gp, project=False, out=st.bwd)
+                ev[4].record()
+                tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.2)
+                ev[5].record()
+                torch.cuda.synchronize()
+                for i_ in range(5):
+                    accp[i_] += ev[i_].elapsed_time(ev[i_ + 1])
+            paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 10, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
+                     "sample_paper_ms": accp[0] / args.steps, "bin_sort_all_tiles_ms": accp[1] / args.steps,
+                     "raster_fwd_ms": accp[2] / args.steps, "raster_bwd_ms": accp[3] / args.steps,
+                     "maps_update_ms": accp[4] / args.steps,
+                     "raster_px_per_s": sp.n / ((accp[2] + accp[3]) / args.steps * 1e-3)}
+
+
+        next_rows = {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
+                     "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
+                     "paper_regime": paper,
+                     "raster_stats_ms": stats_ms,
+                     "raster_stats_tflops": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12,
+                     "raster_stats_alu_frac": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12 / fp32_peak_measured,
+                     "note": "tgs_raster_stats_sparse (f3): 15 flop per walked + 12 per blended pair (w, 3 sums, recomputed "
+                             "distance). tgs_loss_sparse (SURVEY.md 8f f1), timed alone, 44 algorithmic bytes per sampled pixel; "
+                             "not inside the five-call step"}
 
     # ---- roofline of the dominant kernel ----
     peaks, peak_src = measured_peaks()
@@ -349,7 +363,7 @@ def run_tgs(args):
     dominant = max(("raster_fwd", "raster_bwd", "preprocess", "project_bwd"), key=lambda k_: per_call_ms[k_])
     roof = dict(kernels[dominant])
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "r1c_traffic.csv")  # dram bytes per launch from the committed ncu --set full capture
+    tp = os.path.join(ROOT, "profiles", "r1d_traffic.csv")  # dram bytes per launch from the committed ncu --set full capture
     if os.path.exists(tp):
         with open(tp) as f:
             for ln in f.read().splitlines()[1:]:
@@ -405,15 +419,7 @@ def run_tgs(args):
             "gpu_launches": int(launches),
             "roofline": roof,
             "per_call_ms": per_call_ms,
-            "next_rows": {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
-                          "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
-                          "paper_regime": paper,
-                          "raster_stats_ms": stats_ms,
-                          "raster_stats_tflops": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12,
-                          "raster_stats_alu_frac": (FWD_FLOPS_WALK * walked + 12 * blended) / (stats_ms * 1e-3) / 1e12 / fp32_peak_measured,
-                          "note": "tgs_raster_stats_sparse (f3): 15 flop per walked + 12 per blended pair (w, 3 sums, recomputed "
-                                  "distance). tgs_loss_sparse (SURVEY.md 8f f1), timed alone, 44 algorithmic bytes per sampled pixel; "
-                                  "not inside the five-call step"},
+            "next_rows": next_rows,
             "kernels": kernels,
             "work": {"fwd_evals": walked, "bwd_evals": replayed, "blended": blended,
                      "fwd_evals_per_s": walked / (per_call_ms["raster_fwd"] * 1e-3),
@@ -440,6 +446,8 @@ def main():
     ap.add_argument("--pct", type=int, default=20, help="tile percentage for config 5")
     ap.add_argument("--impl", default="tgs", choices=["tgs", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--step-only", action="store_true", help="skip the SURVEY 8f extras (loss, statistics forward, paper regime): "
+                    "used for the profiler launch list of the five-call step")
     args = ap.parse_args()
     if args.impl == "reference":
         if args.config > 2:  # bigger configs: keep the whole run within a few minutes
