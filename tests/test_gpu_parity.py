@@ -590,3 +590,55 @@ def test_paper_sampler_drives_the_raster(orc32, tgs, torch):
     good = tainted_gaussians(sc.N, b, s, fw)
     check_grad("dL_dmean2D", got[:, 0:2], rb.dL_dmeans2D, good)
     check_grad("dL_drgb", got[:, 6:9], rb.dL_drgb, good)
+
+
+def test_step_replays_in_a_cuda_graph(orc32, tgs, torch):
+    """The five calls enqueue only (sizes are read on the device), including the fork / join onto the context's
+    side stream: a whole step is captured in a CUDA graph and replayed on new inputs, bit-identical lists and the
+    same gradients as the eager step."""
+    import paper_2606_15924_b200 as pk
+    r = oracle_run("small_rot", orc32)
+    sc = r.sc
+    d = scene_dev(sc, torch)
+    err = dev(sc.err, torch)
+    step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 64)
+    g = torch.zeros((sc.cam.width * sc.cam.height, 3), device="cuda")
+    g[:r.samp.n] = dev(r.g, torch)
+
+    def run():
+        step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
+                     sc.sample_seed, err=err)
+        step.backward(g)
+
+    run()  # eager: also sets the kernels' shared-memory attributes before the capture
+    torch.cuda.synchronize()
+    P, k, n = step.counts()
+    eager = {k_: getattr(step.bwd, k_).clone() for k_ in ("dL_dmeans3D", "dL_dscales", "dL_dquats", "dL_dsh")}
+    eager_pix = step.samp.pix[:n].clone()
+    eager_gid = step.binned.gid_sorted[:P].clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(s):
+        with torch.cuda.graph(graph, stream=s):
+            run()
+    for t_ in eager:
+        getattr(step.bwd, t_).zero_()
+    step.samp.pix.zero_()
+    step.binned.gid_sorted.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert step.counts() == (P, k, n)
+    assert torch.equal(step.samp.pix[:n], eager_pix) and torch.equal(step.binned.gid_sorted[:P], eager_gid)
+    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+    for t_, ref in eager.items():
+        check_grad(t_ + " (graph vs eager)", getattr(step.bwd, t_).cpu().numpy(), ref.cpu().numpy(), good)
+    check_grad("dL_dmeans3D (graph vs oracle)", step.bwd.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
+    # replay on changed inputs: move the Gaussians, the graph must follow (nothing was baked in)
+    d.means3D.add_(0.01)
+    graph.replay()
+    torch.cuda.synchronize()
+    moved = step.bwd.dL_dmeans3D.clone()
+    run()
+    torch.cuda.synchronize()
+    check_grad("dL_dmeans3D (graph vs eager, moved)", moved.cpu().numpy(), step.bwd.dL_dmeans3D.cpu().numpy())
