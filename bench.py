@@ -436,9 +436,56 @@ def run_tgs(args):
         e2e_step()
     ee.record()
     barrier()
-    e2e_ms = es.elapsed_time(ee)
-    e2e_ms = rep.max_over_ranks(e2e_ms)
+    e2e_serial_ms = rep.max_over_ranks(es.elapsed_time(ee))
+
+    # the same end-to-end step, pipelined the way a training loop would: the H2D copy of step i+1 (copy stream, second
+    # set of device inputs) and the D2H copy of step i-1 (output stream, staged gradients) overlap the compute of step i.
+    # Every step still copies all of its inputs in and all of its gradients out.
+    comp, cs, os_ = torch.cuda.current_stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    Dsets = [D, {k_: torch.empty_like(v) for k_, v in D.items()}]
+    gsets = [g_dev, torch.zeros_like(g_dev)]
+    stage = [{k_: torch.empty_like(getattr(step.bwd, k_)) for k_ in Hout} for _ in range(2)]
+    mk = lambda: [torch.cuda.Event(), torch.cuda.Event()]
+    ev_in, ev_in_free, ev_out, ev_out_free = mk(), mk(), mk(), mk()
+
+    def pipelined(nsteps):
+        for i in range(nsteps):
+            j = i & 1
+            with torch.cuda.stream(cs):
+                if i >= 2:
+                    cs.wait_event(ev_in_free[j])
+                for k_, v in H.items():
+                    Dsets[j][k_].copy_(v, non_blocking=True)
+                gsets[j][:n].copy_(g_pin[:n], non_blocking=True)
+                ev_in[j].record(cs)
+            comp.wait_event(ev_in[j])
+            Dj = Dsets[j]
+            step.forward(Dj["means3D"], Dj["scales"], Dj["quats"], Dj["opacities"], Dj["sh"], scene.tile_pct, scene.pixel_mode,
+                         scene.pix_rate, scene.sample_seed, err=Dj["err"])
+            step.backward(gsets[j])
+            ev_in_free[j].record(comp)
+            if i >= 2:
+                comp.wait_event(ev_out_free[j])
+            for k_ in Hout:
+                stage[j][k_].copy_(getattr(step.bwd, k_), non_blocking=True)
+            ev_out[j].record(comp)
+            with torch.cuda.stream(os_):
+                os_.wait_event(ev_out[j])
+                for k_, v in Hout.items():
+                    v.copy_(stage[j][k_], non_blocking=True)
+                ev_out_free[j].record(os_)
+        comp.wait_stream(os_)
+
+    pipelined(4)
+    barrier()
+    es.record()
+    pipelined(args.steps)
+    ee.record()
+    barrier()
+    e2e_ms = rep.max_over_ranks(es.elapsed_time(ee))
     e2e_val = n_total * args.steps / (e2e_ms * 1e-3)
+    # what arrived on the host is the last step's gradient (atomics reorder sums: compare with a tolerance)
+    assert torch.allclose(Hout["dL_dsh"], step.bwd.dL_dsh.cpu(), rtol=1e-3, atol=1e-6), "pipelined e2e: host gradients differ"
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -446,6 +493,9 @@ def run_tgs(args):
             "config": dict(workload_config(scene, args, P, k, n), l2="flushed between steps (256 MiB write)", launch=launch_mode),
             "clocks": sampler.summary(),
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step_serial": e2e_serial_ms / args.steps,
+                    "how": "pinned host -> device copies of all inputs and device -> pinned host copies of all gradients every step; "
+                           "copies of neighbouring steps overlap the compute (3 streams, double-buffered); serial = one stream",
                     "ms_per_step": e2e_ms / args.steps},
             "gpu_launches": int(launches),
             "roofline": roof,
