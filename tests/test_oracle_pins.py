@@ -975,3 +975,23 @@ def test_maps_update_eq3_eq4(orc32):
         with np.errstate(over="ignore"):
             want = int(np.float32(f).astype(np.float16).view(np.uint16))
         assert orc32.float_to_half(f) == want, f
+
+
+# ---------------------------------------------------------------------------------------------
+def test_golden_digest_of_the_tiny_scene():
+    """tests/golden/cfg1_oracle.txt (written by tests/golden/make_golden.py from oracle/ alone) still describes
+    the oracle: its arithmetic cannot change silently."""
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = dict(ln.split() for ln in open(os.path.join(here, "cfg1_oracle.txt")) if not ln.startswith("#"))
+    now = {k: str(v) for name in mg.SCENES for k, v in mg.digest(name)}
+    assert set(stored) == set(now)
+    for k in stored:
+        if k.split(".")[1].startswith(("sum_color", "sum_T", "l1_")):  # floating-point digests: libm may differ in the last bits
+            assert abs(float(stored[k]) - float(now[k])) <= 2e-6 * abs(float(stored[k])) + 1e-9, k
+        else:
+            assert stored[k] == now[k], k
