@@ -10,6 +10,14 @@
  *   tgs_raster_fwd_sparse  Eq. 1 alpha compositing on sampled pixels only   PAPER.md:66 (Eq. 1), 154-166 (Sec. 3.6, Fig. 6)
  *   tgs_raster_bwd_sparse  its analytic backward + the projection chain     PAPER.md:69, 75, 166, 441 (Alg. 1 step 8)
  *
+ * and, widening along SURVEY.md 8f (each to the same parity bar, tests/test_gpu_parity.py):
+ *   tgs_loss_sparse          f1  Charbonnier + tile-level sparse NCC + lambda_ncc   PAPER.md:168-208 (Eq. 9-11), 472-481 (Eq. 17-18)
+ *   tgs_sample_paper         f2  N_pix pixels in every tile: multinomial w/o         PAPER.md:128-150 (Eq. 7-8)
+ *                                replacement on the error map, TopK age, remainder
+ *   tgs_maps_update          f2  fp16 EMA error map, uint16 age map                  PAPER.md:97-109 (Eq. 3-4)
+ *   tgs_raster_stats_sparse  f3  per-Gaussian E_i, D_i, W_i and expected depth       PAPER.md:212-223 (Eq. 12), Alg. 1 step 11
+ *   tgs_fp32_peak                diagnostic: measured FFMA peak (roofline denominator)
+ *
  * Conventions (all calls)
  *   - Plain C, no C++/torch types.  Every pointer is a DEVICE pointer unless its name ends in
  *     `_host` (then it is a HOST pointer, pinned or pageable) or it is `const tgs_camera*`
