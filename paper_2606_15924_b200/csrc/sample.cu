@@ -108,65 +108,138 @@ tile_reduce_kernel(const CamK cam, const float* __restrict__ err, const float* _
     }
 }
 
-// rank by counting: tile t is selected iff fewer than k tiles precede it in the order
-// (score descending, tile id ascending).  One warp per tile, lanes stride over all T scores:
-// O(T^2) compares spread over the whole GPU, no sort needed for T of a few thousand.
-__global__ void __launch_bounds__(256)
-tile_select_kernel(int T, int k, const uint64_t* __restrict__ tile_score, uint32_t* __restrict__ selected) {
-    const int t = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (t >= T) return;
-    const int lane = threadIdx.x & 31;
-    const uint64_t mine = tile_score[t];
-    uint32_t rank = 0;
-    for (int j = lane; j < T; j += 32) {
-        const uint64_t o = __ldg(tile_score + j);
-        rank += (o > mine || (o == mine && j < t)) ? 1u : 0u;
-    }
-    rank = __reduce_add_sync(0xffffffffu, rank);
-    if (lane == 0) selected[t] = rank < (uint32_t)k ? 1u : 0u;
-}
-
-// single block: compaction of the selected tiles (ascending id) and exclusive prefix sum of their
-// pixel counts.  A 64-bit scan carries both: count << 40 | pixels.
-__global__ void __launch_bounds__(1024)
-tile_compact_kernel(int T, const uint32_t* __restrict__ selected, const TileMeta* __restrict__ meta,
-                    uint32_t* __restrict__ tiles, uint32_t* __restrict__ tpo, int32_t* __restrict__ kn_dev) {
-    __shared__ uint64_t wsum[33];
-    __shared__ uint64_t carry_s;
+// Block-wide exclusive scan of one 64-bit value per thread (1024 threads); wsum holds 33 words.  Ends with a barrier.
+__device__ __forceinline__ uint64_t block_excl_scan_u64(uint64_t v, uint64_t* wsum, uint64_t& total) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
+    uint64_t x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint64_t yv = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += yv;
+    }
+    if (lane == 31) wsum[warp] = x;
     __syncthreads();
-    for (int b0 = 0; b0 < T; b0 += 1024) {
-        const int t = b0 + threadIdx.x;
-        const bool sel = t < T && selected[t];
-        const uint64_t v = sel ? ((1ull << 40) | (uint64_t)meta[t].npix) : 0ull;
-        uint64_t x = v;
+    if (warp == 0) {
+        const uint64_t w = wsum[lane];
+        uint64_t xs = w;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            uint64_t yv = __shfl_up_sync(0xffffffffu, x, o);
-            if (lane >= o) x += yv;
+            const uint64_t yv = __shfl_up_sync(0xffffffffu, xs, o);
+            if (lane >= o) xs += yv;
         }
-        if (lane == 31) wsum[warp] = x;
+        wsum[lane] = xs - w;
+        if (lane == 31) wsum[32] = xs;
+    }
+    __syncthreads();
+    const uint64_t r = wsum[warp] + (x - v);
+    total = wsum[32];
+    __syncthreads();
+    return r;
+}
+
+// single block: top-k selection, compaction of the selected tiles (ascending id) and exclusive prefix sum of
+// their pixel counts.
+//   Selection: tile t is selected iff fewer than k tiles precede it in the order (score descending, tile id
+//   ascending).  The k-th largest score s* is found by an MSD radix select on the 64-bit scores (5 passes of
+//   8 bits over the 40 significant bits, a 256-bin shared histogram over the tiles that still match the prefix): O(T) work for any T (the
+//   first version ranked every tile against every other, O(T^2)).  Tiles with score > s* are selected, and of
+//   those with score == s* the first (k - #greater) in tile order.
+//   Compaction: a 64-bit scan carries both results: count << 40 | pixels.
+__global__ void __launch_bounds__(1024)
+tile_select_compact_kernel(int T, int k, const uint64_t* __restrict__ tile_score, const TileMeta* __restrict__ meta,
+                           uint32_t* __restrict__ selected, uint32_t* __restrict__ tiles, uint32_t* __restrict__ tpo,
+                           int32_t* __restrict__ kn_dev) {
+    __shared__ uint64_t wsum[33];
+    __shared__ uint64_t carry_s, s_prefix;
+    __shared__ uint32_t hist[256], wtot[8];
+    __shared__ uint32_t s_kk, carry_eq;
+    if (threadIdx.x == 0) { carry_s = 0; carry_eq = 0; s_prefix = 0; s_kk = (uint32_t)k; }
+    __syncthreads();
+    // ---- the k-th largest score ----
+    // scores are (sum of <= 256 fixed-point errors < 2^24, << 8) / count < 2^40 (R11): bytes 7..5 are zero
+    constexpr int kTopByte = 4;
+    for (int p = kTopByte; p >= 0; --p) {
+        if (threadIdx.x < 256) hist[threadIdx.x] = 0u;
         __syncthreads();
-        if (warp == 0) {
-            uint64_t w = wsum[lane], xs = w;
+        const uint64_t prefix = s_prefix;
+        for (int t = threadIdx.x; t < T; t += 1024) {
+            const uint64_t sc = tile_score[t];
+            if ((sc >> (8 * (p + 1))) == prefix) atomicAdd(&hist[(uint32_t)(sc >> (8 * p)) & 255u], 1u);
+        }
+        __syncthreads();
+        // the digit d with  #(digits > d) < kk <= #(digits >= d): a scan over the bins from the top (threads 0..255)
+        const uint32_t kk = s_kk;
+        uint32_t h = 0, incl = 0;
+        if (threadIdx.x < 256) {
+            h = hist[255 - threadIdx.x];
+            incl = h;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                uint64_t yv = __shfl_up_sync(0xffffffffu, xs, o);
-                if (lane >= o) xs += yv;
+                const uint32_t yv = __shfl_up_sync(0xffffffffu, incl, o);
+                if ((threadIdx.x & 31) >= o) incl += yv;
             }
-            wsum[lane] = xs - w;
-            if (lane == 31) wsum[32] = xs;
+            if ((threadIdx.x & 31) == 31) wtot[threadIdx.x >> 5] = incl;
         }
         __syncthreads();
-        const uint64_t excl = carry_s + wsum[warp] + (x - v);
+        if (threadIdx.x < 256) {
+            for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) incl += wtot[w];
+            const uint32_t excl = incl - h;
+            if (excl < kk && kk <= incl) { s_prefix = (prefix << 8) | (uint64_t)(255 - threadIdx.x); s_kk = kk - excl; }
+        }
+        __syncthreads();
+    }
+    const uint64_t sstar = s_prefix;
+    const uint32_t need_eq = s_kk;  // how many of the tiles with score == s* are selected (the first ones in tile order)
+    // ---- selection flags and compaction, 1024 tiles at a time ----
+    for (int b0 = 0; b0 < T; b0 += 1024) {
+        const int t = b0 + threadIdx.x;
+        const uint64_t sc = t < T ? tile_score[t] : 0ull;
+        const bool gt = t < T && sc > sstar, eq = t < T && sc == sstar;
+        uint64_t tot_eq;
+        const uint64_t eq_rank = (uint64_t)carry_eq + block_excl_scan_u64(eq ? 1ull : 0ull, wsum, tot_eq);
+        const bool sel = gt || (eq && eq_rank < (uint64_t)need_eq);
+        if (t < T) selected[t] = sel ? 1u : 0u;
+        const uint64_t v = sel ? ((1ull << 40) | (uint64_t)meta[t].npix) : 0ull;
+        uint64_t tot;
+        const uint64_t excl = carry_s + block_excl_scan_u64(v, wsum, tot);
         if (sel) {
             const uint32_t pos = (uint32_t)(excl >> 40);
             tiles[pos] = (uint32_t)t;
             tpo[pos] = (uint32_t)(excl & ((1ull << 40) - 1));
         }
         __syncthreads();
-        if (threadIdx.x == 0) carry_s += wsum[32];
+        if (threadIdx.x == 0) { carry_s += tot; carry_eq += (uint32_t)tot_eq; }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const uint32_t kk = (uint32_t)(carry_s >> 40), nn = (uint32_t)(carry_s & ((1ull << 40) - 1));
+        tpo[kk] = nn;
+        kn_dev[0] = (int32_t)kk;
+        kn_dev[1] = (int32_t)nn;
+    }
+}
+
+// compaction alone (every tile selected): the paper's sampler
+__global__ void __launch_bounds__(1024)
+tile_compact_kernel(int T, const uint32_t* __restrict__ selected, const TileMeta* __restrict__ meta,
+                    uint32_t* __restrict__ tiles, uint32_t* __restrict__ tpo, int32_t* __restrict__ kn_dev) {
+    __shared__ uint64_t wsum[33];
+    __shared__ uint64_t carry_s;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int b0 = 0; b0 < T; b0 += 1024) {
+        const int t = b0 + threadIdx.x;
+        const bool sel = t < T && selected[t];
+        const uint64_t v = sel ? ((1ull << 40) | (uint64_t)meta[t].npix) : 0ull;
+        uint64_t tot;
+        const uint64_t excl = carry_s + block_excl_scan_u64(v, wsum, tot);
+        if (sel) {
+            const uint32_t pos = (uint32_t)(excl >> 40);
+            tiles[pos] = (uint32_t)t;
+            tpo[pos] = (uint32_t)(excl & ((1ull << 40) - 1));
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) carry_s += tot;
         __syncthreads();
     }
     if (threadIdx.x == 0) {
@@ -339,10 +412,9 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
     TileMeta* meta = (TileMeta*)ws;
     uint32_t* selected = tile_select ? tile_select : (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
     tile_reduce_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, err, render, target, mode, rnum, rden, seed, tile_score, meta);
-    tile_select_kernel<<<(T + 7) / 8, 256, 0, s>>>(T, k, tile_score, selected);
-    tile_compact_kernel<<<1, 1024, 0, s>>>(T, selected, meta, tiles, tpo, kn_dev);
+    tile_select_compact_kernel<<<1, 1024, 0, s>>>(T, k, tile_score, meta, selected, tiles, tpo, kn_dev);
     write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);
-    count_launches(4);
+    count_launches(3);
     return cudaGetLastError();
 }
 
