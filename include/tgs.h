@@ -26,6 +26,10 @@
  *   - `stream` is a cudaStream_t passed as void*.  Calls only enqueue work; they do not
  *     synchronise, EXCEPT when a non-NULL `*_host` output is given (one cudaStreamSynchronize).
  *     All calls are CUDA-graph capturable when the `_host` outputs are NULL.
+ *   - A context owns 32 bytes of device scheduler counters and one side stream (+ two events): the raster calls
+ *     fork their warp-per-tile kernel onto it and join before returning to `stream` (also under graph capture).
+ *     The raster calls of ONE context must therefore be ordered with respect to each other (same stream, or
+ *     stream-ordered by the caller); use one context per concurrently working stream.
  *   - fp32 only, 16x16 tiles only, sh_degree in {0,1,2,3}.  Anything else returns
  *     TGS_ERR_UNSUPPORTED.  There is no CPU fallback.
  *   - Return value: TGS_OK or an error code; tgs_last_error(ctx) holds a message.
