@@ -1,0 +1,76 @@
+"""Randomised bit-exact parity of the integer stages (tgs_bin_sort, tgs_sample, tgs_sample_paper) against the oracle:
+random image sizes, Gaussian counts, rect shapes (small, wide, whole-grid, one hot spot), depth distributions (spread,
+many ties, one tight cluster), random tile selections, random sampler parameters.  (1000 + 500 such cases were run
+once during development; this keeps a seeded subset in the suite.)"""
+from types import SimpleNamespace
+
+import numpy as np
+import pytest
+
+import workloads
+from helpers import dev, pack_splats, u32
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def tgs(torch):
+    import paper_2606_15924_b200 as pk
+    return pk.TGS(0)
+
+
+@pytest.mark.parametrize("seed", [1, 2, 3])
+def test_fuzz_bin_sort(seed, orc32, tgs, torch):
+    o, tg = orc32, tgs
+    rng = np.random.default_rng(seed)
+    for c in range(25):
+        W=int(rng.integers(17,1500)); H=int(rng.integers(17,900)); N=int(rng.integers(1,60000))
+        cam=workloads.Camera(W,H,100.,100.,W/2,H/2,np.eye(3,dtype=np.float32),np.zeros(3,np.float32)); gx,gy=cam.grid
+        mode=rng.integers(0,4)
+        x0=rng.integers(0,gx,N); y0=rng.integers(0,gy,N)
+        if mode==0: w=rng.integers(1,4,N); h=rng.integers(1,4,N)
+        elif mode==1: w=rng.integers(1,9,N); h=rng.integers(1,9,N)
+        elif mode==2: w=np.where(rng.random(N)<0.02, rng.integers(1,gx+1,N), rng.integers(1,3,N)); h=np.where(rng.random(N)<0.02, rng.integers(1,gy+1,N), rng.integers(1,3,N))
+        else:
+            x0=np.minimum(gx-1,(rng.normal(gx/2,1.0,N)).astype(int).clip(0)); y0=np.minimum(gy-1,(rng.normal(gy/2,1.0,N)).astype(int).clip(0)); w=rng.integers(1,5,N); h=rng.integers(1,5,N)
+        rect=np.zeros((N,4),np.int32); rect[:,0]=x0; rect[:,1]=y0; rect[:,2]=np.minimum(x0+w,gx); rect[:,3]=np.minimum(y0+h,gy)
+        vis=rng.random(N)<0.9; rect[~vis]=0
+        touched=((rect[:,2]-rect[:,0])*(rect[:,3]-rect[:,1])).astype(np.uint32)
+        dm=rng.integers(0,3)
+        depth=(rng.uniform(0.3,40,N) if dm==0 else np.round(rng.uniform(1,3,N),1) if dm==1 else 5+0.001*rng.normal(size=N)).astype(np.float32)
+        pre=SimpleNamespace(means2D=np.zeros((N,2),np.float32),conic_opacity=np.ones((N,4),np.float32),rgb=np.zeros((N,3),np.float32),depths=depth,rect=rect,tiles_touched=touched,radii=(touched>0).astype(np.int32))
+        sel=None
+        if rng.random()<0.6: sel=(rng.random(gx*gy)<rng.uniform(0.02,0.9)).astype(np.uint32)
+        b=o.bin_sort(cam,pre,tile_select=sel)
+        out=tg.bin_sort(cam,dev(pack_splats(pre),torch),b.P+int(rng.integers(0,5)),want_keys=True,tile_select=None if sel is None else dev(sel.astype(np.int32),torch))
+        ok=out.P==b.P and np.array_equal(u32(out.tile_offsets),b.tile_offsets) and np.array_equal(u32(out.gid_sorted)[:b.P],b.gid_sorted) and np.array_equal(out.keys_sorted.cpu().numpy().view(np.uint64)[:b.P],b.keys_sorted)
+        assert ok, (seed, c, W, H, N, int(mode), int(dm), sel is not None, out.P, b.P)
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_fuzz_samplers(seed, orc32, tgs, torch):
+    o, tg = orc32, tgs
+    rng = np.random.default_rng(100 + seed)
+    for c in range(15):
+        W=int(rng.integers(17,700)); H=int(rng.integers(17,500))
+        cam=workloads.Camera(W,H,100.,100.,W/2,H/2,np.eye(3,dtype=np.float32),np.zeros(3,np.float32))
+        e=(rng.random((H,W))**rng.uniform(0.5,6)*rng.uniform(0.01,20)).astype(np.float32); e[rng.random((H,W))<rng.uniform(0,0.9)]=0
+        E=e.astype(np.float16).view(np.uint16); A=rng.integers(0,int(rng.integers(1,70000)),(H,W)).clip(0,65535).astype(np.uint16)
+        npx=int(rng.integers(1,257)); nh=int(rng.integers(0,npx+1)); ns=int(rng.integers(0,npx-nh+1)); seed=int(rng.integers(0,2**62))
+        r=o.sample_paper(cam,E,A,npx,nh,ns,seed)
+        g=tg.sample_paper(cam,dev(E.view(np.int16),torch),dev(A.view(np.int16),torch),npx,nh,ns,seed=seed)
+        if not (g.n==r.n and np.array_equal(u32(g.pix)[:r.n],r.pix) and np.array_equal(u32(g.tile_pix_offsets)[:r.k+1],r.tile_pix_offsets)):
+            raise AssertionError(('tgs_sample_paper', seed, c, W, H, npx, nh, ns))
+        # top-k sampler too
+        pct=int(rng.integers(1,101)); md=int(rng.integers(0,2)); rate=(int(rng.integers(1,8)),int(rng.integers(8,20)))
+        r2=o.sample(cam,(pct,100),md,rate,seed%1000,err=e)
+        g2=tg.sample(cam,(pct,100),md,rate,seed%1000,err=dev(e,torch))
+        if not (g2.n==r2.n and np.array_equal(u32(g2.tiles)[:r2.k],r2.tiles) and np.array_equal(u32(g2.pix)[:r2.n],r2.pix)):
+            raise AssertionError(('tgs_sample', seed, c, W, H, pct, md))
