@@ -74,3 +74,43 @@ def test_fuzz_samplers(seed, orc32, tgs, torch):
         g2=tg.sample(cam,(pct,100),md,rate,seed%1000,err=dev(e,torch))
         if not (g2.n==r2.n and np.array_equal(u32(g2.tiles)[:r2.k],r2.tiles) and np.array_equal(u32(g2.pix)[:r2.n],r2.pix)):
             raise AssertionError(('tgs_sample', seed, c, W, H, pct, md))
+
+
+@pytest.mark.parametrize("seed", [1, 2])
+def test_fuzz_raster_mixed_pixel_lists(seed, orc32, tgs, torch):
+    """Random scenes with hand-made sampled lists: per tile all pixels, 1..32 pixels (the warp-per-tile kernels) or
+    any number of pixels, mixed inside one call; forward, backward and the statistics forward against the oracle."""
+    from helpers import binned_dev, check_forward, check_grad, samp_dev, tainted_gaussians
+    o, tg = orc32, tgs
+    rng = np.random.default_rng(seed)
+    for c in range(5):
+        W=int(rng.integers(40,400)); H=int(rng.integers(40,300)); N=int(rng.integers(200,6000))
+        sc=workloads.small_random_scene(int(rng.integers(0,10**6)), N, W, H, sh_degree=int(rng.integers(0,4)), bg=tuple(rng.random(3).round(2)), spread=float(rng.uniform(0.8,1.6)), log_scale=(float(rng.uniform(-3.2,-2.0)),float(rng.uniform(0.3,0.9))))
+        cam=sc.cam; gx,gy=cam.grid
+        pre=o.preprocess(cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
+        b=o.bin_sort(cam,pre)
+        tiles=np.nonzero(rng.random(gx*gy)<rng.uniform(0.2,1.0))[0].astype(np.uint32)
+        if len(tiles)==0: tiles=np.array([0],np.uint32)
+        pix=[]; tpo=[0]
+        for t in tiles:
+            tx,ty=int(t)%gx,int(t)//gx
+            xs,ys=np.meshgrid(np.arange(tx*16,min(W,tx*16+16)),np.arange(ty*16,min(H,ty*16+16)))
+            allp=(ys*W+xs).reshape(-1)
+            kind=rng.integers(0,4)
+            m=len(allp) if kind==0 else int(rng.integers(1,min(33,len(allp)+1))) if kind==1 else int(rng.integers(1,len(allp)+1))
+            ch=np.sort(rng.choice(len(allp),m,replace=False)); pix.append(allp[ch]); tpo.append(tpo[-1]+m)
+        s=SimpleNamespace(k=len(tiles),n=tpo[-1],tiles=tiles,tile_pix_offsets=np.array(tpo,np.uint32),pix=np.concatenate(pix).astype(np.uint32))
+        fw=o.raster_fwd(cam,b,pre,s)
+        g=workloads.dl_dcolor(c,s.n)
+        rb=o.raster_bwd(cam,b,pre,s,fw,g)
+        e=rng.random(s.n).astype(np.float32)
+        rs=o.raster_stats(cam,b,pre,s,e)
+        splats=dev(pack_splats(pre),torch); bd=binned_dev(b,torch,gx*gy); sd=samp_dev(s,torch)
+        out=tg.raster_fwd_sparse(cam,splats,bd,sd); torch.cuda.synchronize()
+        rep=check_forward(out.color[:s.n].cpu().numpy(),out.T[:s.n].cpu().numpy(),u32(out.n_contrib)[:s.n],fw,max_fragile_frac=5e-3)
+        bw=tg.raster_bwd_sparse(cam,sc.sh_degree,splats,bd,sd,out,dev(g,torch),project=False); torch.cuda.synchronize()
+        good=tainted_gaussians(sc.N,b,s,fw); ds=bw.dL_dsplats.cpu().numpy()
+        check_grad("m2d",ds[:,0:2],rb.dL_dmeans2D,good); check_grad("conic",ds[:,2:5],rb.dL_dconic,good); check_grad("op",ds[:,5:6],rb.dL_dopacity.reshape(-1,1),good); check_grad("rgb",ds[:,6:9],rb.dL_drgb,good)
+        st=tg.raster_stats_sparse(cam,splats,bd,sd,dev(e,torch)); torch.cuda.synchronize()
+        check_grad("stats",st.stats.cpu().numpy()[:,:3],rs.stats,good)
+        assert (np.diff(tpo) <= 32).any() and (np.diff(tpo) > 32).any()  # both kernel families ran
