@@ -262,7 +262,7 @@ class TGS:
     # ---- a4 ----
     def raster_fwd_sparse(self, cam, splats, binned, samp, n_capacity=None, want_walked=False, out=None, stream=None):
         cam = Camera.of(cam)
-        n = n_capacity if n_capacity is not None else samp.n
+        n = n_capacity if n_capacity is not None else (samp.n if samp.n is not None else samp.pix.numel())
         if out is None:
             out = SimpleNamespace(color=torch.empty((n, 3), dtype=torch.float32, device=self.device),
                                   T=torch.empty(n, dtype=torch.float32, device=self.device),
@@ -280,7 +280,7 @@ class TGS:
     def loss_sparse(self, cam, samp, color, target, eps_l1=1e-3, eps_ncc=1e-6, eps_lambda=1e-8, n_capacity=None,
                     want_loss=True, out=None, stream=None):
         cam = Camera.of(cam)
-        n = n_capacity if n_capacity is not None else samp.n
+        n = n_capacity if n_capacity is not None else (samp.n if samp.n is not None else samp.pix.numel())
         if out is None:
             f = dict(dtype=torch.float32, device=self.device)
             out = SimpleNamespace(dL_dcolor=torch.empty((n, 3), **f), pix_err=torch.empty(n, **f),
@@ -295,7 +295,7 @@ class TGS:
     def raster_stats_sparse(self, cam, splats, binned, samp, pix_err, n_capacity=None, want_depth=True, out=None,
                             stream=None):
         cam = Camera.of(cam)
-        n = n_capacity if n_capacity is not None else samp.n
+        n = n_capacity if n_capacity is not None else (samp.n if samp.n is not None else samp.pix.numel())
         N = splats.shape[0]
         if out is None:
             f = dict(dtype=torch.float32, device=self.device)
