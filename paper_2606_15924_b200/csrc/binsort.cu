@@ -830,7 +830,7 @@ size_t binsort_workspace_bytes(int N, int64_t Pcap, int T) { return carve(nullpt
 
 cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const uint32_t* tile_select, int64_t Pcap,
                             uint64_t* keys_sorted, uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev,
-                            void* ws, size_t ws_bytes, int num_sms, cudaStream_t s) {
+                            void* ws, size_t ws_bytes, int num_sms, cudaStream_t s, const SideStream* side) {
     (void)ws_bytes;
     const int gx = cam.gx, gy = cam.gy, T = gx * gy;
     const Workspace w = carve(ws, N, T, Pcap);
@@ -889,31 +889,43 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
                                                          P_dev, w.pairs);
     count_launches(6);
 
-    // K6-K7: sort the segments; the large ones (and the pieces of the giant ones) first
+    // K6-K7: sort the segments.  The three classes write disjoint ranges: the long ones (giant split, large,
+    // medium) run on the context's side stream, concurrently with the short ones on the caller's stream (when a class
+    // is empty its launch hides behind the others instead of adding to the call)
     int gid_bits = 1;
     while (gid_bits < 30 && (1ll << gid_bits) < (long long)N) ++gid_bits;
-    if (Pcap > kMediumCap) {  // otherwise no segment is that long
-        if (Pcap > kLargeCap) {
-            int gb = num_sms < T ? num_sms : T;
-            giant_split_kernel<<<gb, kCoarseMax, 0, s>>>(w.giant_list, w.large_list, w.ctr, w.pairs, w.tmp, P_dev);
+    const bool long_classes = Pcap > kSmallCap;
+    if (long_classes) {
+        e = cudaEventRecord(side->fork, s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(side->aux, side->fork, 0);
+        if (e != cudaSuccess) return e;
+        cudaStream_t a = side->aux;
+        if (Pcap > kMediumCap) {  // otherwise no segment is that long
+            if (Pcap > kLargeCap) {
+                int gb = num_sms < T ? num_sms : T;
+                giant_split_kernel<<<gb, kCoarseMax, 0, a>>>(w.giant_list, w.large_list, w.ctr, w.pairs, w.tmp, P_dev);
+                count_launches(1);
+            }
+            int lb = num_sms < T ? num_sms : T;
+            seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1><<<lb, kLargeThreads, kLargeSmem, a>>>(
+                w.large_list, &w.ctr->n_large, &w.ctr->sched_large, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
             count_launches(1);
         }
-        int lb = num_sms < T ? num_sms : T;
-        seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1><<<lb, kLargeThreads, kLargeSmem, s>>>(
-            w.large_list, &w.ctr->n_large, &w.ctr->sched_large, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
-        count_launches(1);
-    }
-    if (Pcap > kSmallCap) {
         int mb = num_sms * 2 < T ? num_sms * 2 : T;
-        seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2><<<mb, kMediumThreads, kMediumSmem, s>>>(
+        seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2><<<mb, kMediumThreads, kMediumSmem, a>>>(
             w.medium_list, &w.ctr->n_medium, &w.ctr->sched_medium, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
         count_launches(1);
+        e = cudaEventRecord(side->join, a);
+        if (e != cudaSuccess) return e;
     }
     int sb = num_sms * 6 < T ? num_sms * 6 : T;
     seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4><<<sb, kSmallThreads, kSmallSmem, s>>>(
         w.small_list, &w.ctr->n_small, &w.ctr->sched_small, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
     count_launches(1);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if (long_classes) e = cudaStreamWaitEvent(s, side->join, 0);
+    return e;
 }
 
 }  // namespace tgs

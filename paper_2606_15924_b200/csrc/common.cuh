@@ -72,7 +72,7 @@ size_t binsort_workspace_bytes(int N, int64_t Pcap, int T);
 cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats, const uint32_t* tile_select, int64_t Pcap,
                             uint64_t* keys_sorted,
                             uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev, void* ws,
-                            size_t ws_bytes, int num_sms, cudaStream_t s);
+                            size_t ws_bytes, int num_sms, cudaStream_t s, const SideStream* side);
 
 size_t sample_workspace_bytes(int T);
 cudaError_t launch_sample(const CamK& cam, const float* err, const float* render, const float* target, int k,

@@ -179,7 +179,7 @@ int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats
         return fail(ctx, TGS_ERR_CAPACITY, "tgs_bin_sort: workspace %zu B < required %zu B", workspace_bytes, need);
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e = launch_bin_sort(make_camk(cam), N, splats, tile_select, P_capacity, keys_sorted, gid_sorted, tile_offsets,
-                                    P_dev, workspace, workspace_bytes, ctx->num_sms, s);
+                                    P_dev, workspace, workspace_bytes, ctx->num_sms, s, &ctx->side);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_bin_sort", e);
     if (P_host) {
         int64_t h[2];
