@@ -38,19 +38,29 @@ class SparseRasterStep:
                                    dL_dsh=e((N, K, 3), f32))
         self.ws_sort = e(tgs.bin_sort_workspace_bytes(N, P_capacity, T), u8)
         self.ws_sample = e(tgs.sample_workspace_bytes(self.cam), u8)
+        self._side = torch.cuda.Stream(device=dev)
+        self._ev_fork, self._ev_join = torch.cuda.Event(), torch.cuda.Event()
 
     def forward(self, means3D, scales, quats, opacities, sh, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0,
                 err=None, render=None, target=None, stream=None, restrict=True):
         """restrict=True: sample first and bin only the selected tiles (tgs_bin_sort's tile_select;
         DESIGN.md R14).  restrict=False: bin every tile, then sample (the call order of north_star)."""
         t = self.tgs
-        t.preprocess(self.cam, self.D, means3D, scales, quats, opacities, sh, out=self.pre, stream=stream)
         if restrict:
+            # projection and sampling do not depend on each other: the sampler runs on a side stream (fork / join by
+            # events, also under graph capture) while the projection runs on the caller's stream
+            main = stream if stream is not None else torch.cuda.current_stream()
+            self._ev_fork.record(main)
+            self._side.wait_event(self._ev_fork)
             t.sample(self.cam, tile_pct, pixel_mode, pix_rate, seed, err=err, render=render, target=target,
-                     out=self.samp, workspace=self.ws_sample, sync=False, stream=stream)
+                     out=self.samp, workspace=self.ws_sample, sync=False, stream=self._side)
+            self._ev_join.record(self._side)
+            t.preprocess(self.cam, self.D, means3D, scales, quats, opacities, sh, out=self.pre, stream=stream)
+            main.wait_event(self._ev_join)
             t.bin_sort(self.cam, self.pre.splats, self.P_capacity, out=self.binned, workspace=self.ws_sort, sync=False,
                        stream=stream, tile_select=self.samp.tile_select)
         else:
+            t.preprocess(self.cam, self.D, means3D, scales, quats, opacities, sh, out=self.pre, stream=stream)
             t.bin_sort(self.cam, self.pre.splats, self.P_capacity, out=self.binned, workspace=self.ws_sort, sync=False,
                        stream=stream)
             t.sample(self.cam, tile_pct, pixel_mode, pix_rate, seed, err=err, render=render, target=target,
