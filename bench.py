@@ -334,8 +334,9 @@ def run_tgs(args):
             fp = tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp)
             gp = torch.randn((sp.n, 3), device=dev, generator=gE) / sp.n
             ob = SimpleNamespace(dL_dsplats=st.bwd.dL_dsplats)
-            ev = [torch.cuda.Event(enable_timing=True) for _ in range(6)]
-            accp = [0.0] * 5
+            sop = tg.raster_stats_sparse(cam, st.pre.splats, bp, sp, lo.pix_err)
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+            accp = [0.0] * 6
             for _ in range(args.steps):
                 flush.fill_(1.0)
                 ev[0].record()
@@ -349,13 +350,15 @@ def run_tgs(args):
                 ev[4].record()
                 tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.2)
                 ev[5].record()
+                tg.raster_stats_sparse(cam, st.pre.splats, bp, sp, lo.pix_err, out=sop)
+                ev[6].record()
                 torch.cuda.synchronize()
-                for i_ in range(5):
+                for i_ in range(6):
                     accp[i_] += ev[i_].elapsed_time(ev[i_ + 1])
             paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 10, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
                      "sample_paper_ms": accp[0] / args.steps, "bin_sort_all_tiles_ms": accp[1] / args.steps,
                      "raster_fwd_ms": accp[2] / args.steps, "raster_bwd_ms": accp[3] / args.steps,
-                     "maps_update_ms": accp[4] / args.steps,
+                     "maps_update_ms": accp[4] / args.steps, "raster_stats_ms": accp[5] / args.steps,
                      "raster_px_per_s": sp.n / ((accp[2] + accp[3]) / args.steps * 1e-3)}
 
 

@@ -101,6 +101,11 @@ cudaError_t launch_raster_bwd_lite(const CamK& cam, const float* splats, const u
                                    const uint32_t* pix, const float* out_T, const uint32_t* n_contrib,
                                    const float* dL_dcolor, float* dL_dsplats, uint32_t* sched, int num_sms, cudaStream_t s);
 
+cudaError_t launch_raster_stats_lite(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
+                                     const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                                     const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,
+                                     uint32_t* sched, int num_sms, cudaStream_t s);
+
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                                const float* sh, const int32_t* radii, const uint8_t* clamped,
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
@@ -115,7 +120,7 @@ cudaError_t launch_maps_update(const CamK& cam, uint16_t* E_half, uint16_t* age,
 cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                                 const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                                 const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,
-                                uint32_t* sched, int num_sms, cudaStream_t s);
+                                uint32_t* sched, int num_sms, cudaStream_t s, const SideStream* side);
 
 cudaError_t launch_loss_sparse(int k, const uint32_t* tpo, const uint32_t* pix, const float* color, const float* target,
                                float eps_l1, float eps_ncc, float eps_lam, float* dL_dcolor, float* pix_err,

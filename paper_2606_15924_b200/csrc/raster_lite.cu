@@ -319,7 +319,152 @@ raster_bwd_lite_kernel(const CamK cam, const float4* __restrict__ splats, const 
     lite_leave(sched, lane);
 }
 
+// ---- statistics forward (tgs_raster_stats_sparse) -----------------------------------------------------
+struct LiteStatXpose {
+    float v[kSlots * kTStride];  // [slot][pixel] = w  (row stride 33)
+    float4 ma[kSlots];           // mx, my, -A/2, -B
+    float2 mb[kSlots];           // -C/2, bits: Gaussian id
+    float4 pa[32];               // per pixel: px, py, e(p), unused
+};
+struct LiteStatShared {
+    WarpBatch batch[kLiteWarps];
+    LiteStatXpose xpose[kLiteWarps];
+};
+
+__global__ void __launch_bounds__(kLiteWarps * 32)
+raster_stats_lite_kernel(const CamK cam, const float4* __restrict__ splats, const uint32_t* __restrict__ tile_offsets,
+                         const uint32_t* __restrict__ gid_sorted, int k, const uint32_t* __restrict__ tiles,
+                         const uint32_t* __restrict__ tpo, const uint32_t* __restrict__ pix,
+                         const float* __restrict__ pix_err, float* __restrict__ stats, float* __restrict__ out_depth,
+                         uint32_t* __restrict__ sched) {
+    __shared__ __align__(16) LiteStatShared sm;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpBatch& sb = sm.batch[warp];
+    LiteStatXpose& sx = sm.xpose[warp];
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    const float kNaN = __int_as_float(0x7fc00000);
+    const int slot2 = lane & (kSlots - 1), half = lane >> 4;
+    int m = 0;
+
+    auto flush = [&]() {
+        __syncwarp();
+        const float4 ga = sx.ma[slot2];
+        const float2 gb = sx.mb[slot2];
+        float E = 0.f, D = 0.f, Wt = 0.f;
+        const float* vrow = sx.v + slot2 * kTStride + half * 16;
+        const float4* prow = sx.pa + half * 16;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const float w = vrow[i];
+            const float4 q = prow[i];
+            const float pw = splat_power(ga.z, ga.w, gb.x, ga.x - q.x, ga.y - q.y);
+            Wt += w;
+            E = fmaf(w, q.z, E);
+            D = fmaf(w, -2.0f * pw, D);
+        }
+        E += __shfl_xor_sync(0xffffffffu, E, 16);
+        D += __shfl_xor_sync(0xffffffffu, D, 16);
+        Wt += __shfl_xor_sync(0xffffffffu, Wt, 16);
+        if (slot2 < m && half == 0) red_add_v4(reinterpret_cast<float4*>(stats) + __float_as_uint(gb.y), E, D, Wt, 0.f);
+        m = 0;
+        __syncwarp();
+    };
+
+    for (;;) {
+        const uint32_t it = lite_next(sched, lane);
+        if (it >= (uint32_t)k) break;
+        const uint32_t p0 = tpo[it], np = tpo[it + 1] - p0;
+        if (np == 0u || np > kLitePixels) continue;  // the block kernel's tile
+        const uint32_t t = tiles[it];
+        const uint32_t start = tile_offsets[t], len = tile_offsets[t + 1] - start;
+        const bool active = (uint32_t)lane < np;
+        const uint32_t slot = p0 + (uint32_t)lane;
+        int ipx = 0, ipy = 0;
+        float e_p = 0.f;
+        if (active) {
+            const uint32_t id = pix[slot];
+            ipx = (int)(id % (uint32_t)cam.W);
+            ipy = (int)(id / (uint32_t)cam.W);
+            e_p = pix_err[slot];
+        }
+        const PixelBox box = warp_pixel_box(active, ipx, ipy);
+        float px = active ? (float)ipx : kNaN;
+        const float py = (float)ipy;
+        float T = 1.0f, zacc = 0.f;
+        __syncwarp();
+        sx.pa[lane] = make_float4((float)ipx, (float)ipy, e_p, 0.f);
+
+        auto gid_at = [&](uint32_t pos) { return pos < len ? gid_sorted[start + pos] : 0xffffffffu; };
+        uint32_t g_next = gid_at((uint32_t)lane + 32u);
+        LiteRec cur = lite_load(splats, gid_at((uint32_t)lane));
+        for (uint32_t b0 = 0; b0 < len; b0 += 32) {
+            const LiteRec nxt = lite_load(splats, g_next);
+            g_next = gid_at(b0 + 64u + (uint32_t)lane);
+            const bool have = b0 + (uint32_t)lane < len;
+            const bool pass = have && splat_may_touch(cur.p0.x, cur.p0.y, cur.p0.z, cur.p0.w, cur.p1.x, cur.p1.y, box);
+            const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
+            const int cnt = __popc(ballot);
+            __syncwarp();
+            if (pass) {
+                const int s = __popc(ballot & lt_mask);
+                sb.a[s] = cur.p0;
+                sb.b[s] = make_float4(cur.p1.x, cur.p1.y, cur.p1.z, 0.f);
+                sb.c[s] = make_float4(cur.p2.w, cur.p2.z, 0.f, 0.f);  // depth, bits: Gaussian id
+            }
+            __syncwarp();
+            int e = 0;
+            while (e < cnt) {
+                const int take = min(cnt - e, kSlots - m);
+                const float4* sa = sb.a + e;
+                float* vdst = sx.v + m * kTStride + lane;
+#pragma unroll 2
+                for (int ii = 0; ii < take; ++ii) {
+                    const float4 a = sa[ii];
+                    const float4 b = sa[32 + ii];
+                    const float dx = a.x - px, dy = a.y - py;
+                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                    const float alpha = fminf(kAlphaMax, __fmul_rn(b.z, ex2_approx(power * kLog2e)));
+                    const bool blend = (power <= 0.0f) && !(alpha < kAlphaMin);
+                    const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
+                    const bool term = blend && (Tn < kTMin);
+                    const bool upd = blend && !term;
+                    const float w = upd ? alpha * T : 0.0f;
+                    zacc = fmaf(w, sa[64 + ii].x, zacc);
+                    T = upd ? Tn : T;
+                    px = term ? kNaN : px;
+                    vdst[ii * kTStride] = w;
+                }
+                if (lane < take) {
+                    sx.ma[m + lane] = sa[lane];
+                    sx.mb[m + lane] = make_float2(sa[32 + lane].x, sa[64 + lane].y);
+                }
+                e += take;
+                m += take;
+                if (m == kSlots) flush();
+            }
+            if (__all_sync(0xffffffffu, px != px)) break;
+            cur = nxt;
+        }
+        if (m > 0) flush();  // before the per-pixel array changes
+        if (active && out_depth) out_depth[slot] = zacc;
+    }
+    lite_leave(sched, lane);
+}
+
 }  // namespace
+
+cudaError_t launch_raster_stats_lite(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
+                                     const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
+                                     const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,
+                                     uint32_t* sched, int num_sms, cudaStream_t s) {
+    if (k <= 0) return cudaSuccess;
+    int blocks = num_sms * 5;
+    if (blocks > (k + kLiteWarps - 1) / kLiteWarps) blocks = (k + kLiteWarps - 1) / kLiteWarps;
+    raster_stats_lite_kernel<<<blocks, kLiteWarps * 32, 0, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
+                                                               gid_sorted, k, tiles, tpo, pix, pix_err, stats, out_depth, sched);
+    count_launches(1);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_raster_fwd_lite(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                                    const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,

@@ -48,7 +48,7 @@ raster_stats_kernel(const CamK cam, const float4* __restrict__ splats, const uin
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ring_init(sm.ring);
     if (warp == kConsumers) {
-        producer_loop<false>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, nullptr, sched, lane);
+        producer_loop<false>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, nullptr, sched, lane, kLitePixels);
         return;
     }
     Ring<128>& R = sm.ring;
@@ -194,10 +194,18 @@ raster_stats_kernel(const CamK cam, const float4* __restrict__ splats, const uin
 cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, const uint32_t* tile_offsets,
                                 const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                                 const uint32_t* pix, const float* pix_err, float* stats, float* out_depth,
-                                uint32_t* sched, int num_sms, cudaStream_t s) {
+                                uint32_t* sched, int num_sms, cudaStream_t s, const SideStream* side) {
     cudaError_t e = cudaMemsetAsync(stats, 0, (size_t)N * 4 * sizeof(float), s);
     if (e != cudaSuccess) return e;
     if (k <= 0) return cudaSuccess;
+    // fork (after the memset): tiles with <= kLitePixels sampled pixels go to the warp-per-tile kernel on the side stream
+    e = cudaEventRecord(side->fork, s);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(side->aux, side->fork, 0);
+    if (e == cudaSuccess)
+        e = launch_raster_stats_lite(cam, splats, tile_offsets, gid_sorted, k, tiles, tpo, pix, pix_err, stats, out_depth,
+                                     sched + 2, num_sms, side->aux);
+    if (e == cudaSuccess) e = cudaEventRecord(side->join, side->aux);
+    if (e != cudaSuccess) return e;
     int blocks = num_sms * 3;
     if (blocks > k) blocks = k;
     constexpr size_t smem = sizeof(StatShared);
@@ -210,7 +218,9 @@ cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, con
     raster_stats_kernel<<<blocks, kRasterThreads, smem, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                             gid_sorted, k, tiles, tpo, pix, pix_err, stats, out_depth, sched);
     count_launches(1);
-    return cudaGetLastError();
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return cudaStreamWaitEvent(s, side->join, 0);  // join
 }
 
 }  // namespace tgs

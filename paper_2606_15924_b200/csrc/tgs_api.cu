@@ -319,7 +319,7 @@ int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const fl
     if (((uintptr_t)splats & 15) || ((uintptr_t)stats & 15))
         return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: splats and stats must be 16-byte aligned");
     cudaError_t e = launch_raster_stats(make_camk(cam), N, splats, tile_offsets, gid_sorted, k, tiles, tile_pix_offsets, pix,
-                                        pix_err, stats, out_depth, ctx->sched, ctx->num_sms, (cudaStream_t)stream);
+                                        pix_err, stats, out_depth, ctx->sched, ctx->num_sms, (cudaStream_t)stream, &ctx->side);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_stats_sparse", e);
     return TGS_OK;
 }
