@@ -322,14 +322,15 @@ def run_tgs(args):
             stats_ms += la.elapsed_time(lb)
         stats_ms /= args.steps
 
-        # the paper's own regime -- N_pix = 25 pixels (r = 10 %) in EVERY tile, 40 % hard,
-        # 40 % stable -- sampler, binning of all tiles, sparse forward / backward on those lists, map updates
+        # the paper's own regime -- N_pix = 25 pixels (r = 10 %) in EVERY tile with the
+        # settings of its Tab. 6: r_hard = 0.4, r_stable = 0.3, 0.3 "mixed" remainder, beta = 0.4 --
+        # sampler, binning of all tiles, sparse forward / backward / statistics on those lists, map updates
         paper = None
         if world == 1:
             gE = torch.Generator(device=dev).manual_seed(1)
             E_half = (torch.rand((cam.height, cam.width), device=dev, generator=gE) ** 3).to(torch.float16).view(torch.int16)
             age = torch.randint(0, 50, (cam.height, cam.width), device=dev, generator=gE, dtype=torch.int32).to(torch.int16)
-            sp = tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1)
+            sp = tg.sample_paper(cam, E_half, age, 25, 10, 8, seed=1)
             bp = tg.bin_sort(cam, st.pre.splats, P_est + 1024, workspace=st.ws_sort, sync=True)
             fp = tg.raster_fwd_sparse(cam, st.pre.splats, bp, sp)
             gp = torch.randn((sp.n, 3), device=dev, generator=gE) / sp.n
@@ -340,7 +341,7 @@ def run_tgs(args):
             for _ in range(args.steps):
                 flush.fill_(1.0)
                 ev[0].record()
-                tg.sample_paper(cam, E_half, age, 25, 10, 10, seed=1, out=sp, workspace=st.ws_sample, sync=False)
+                tg.sample_paper(cam, E_half, age, 25, 10, 8, seed=1, out=sp, workspace=st.ws_sample, sync=False)
                 ev[1].record()
                 tg.bin_sort(cam, st.pre.splats, P_est + 1024, out=bp, workspace=st.ws_sort, sync=False)
                 ev[2].record()
@@ -348,14 +349,14 @@ def run_tgs(args):
                 ev[3].record()
                 tg.raster_bwd_sparse(cam, scene.sh_degree, st.pre.splats, bp, sp, fp, gp, project=False, out=st.bwd)
                 ev[4].record()
-                tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.2)
+                tg.maps_update(cam, E_half, age, sp, lo.pix_err, 0.4)
                 ev[5].record()
                 tg.raster_stats_sparse(cam, st.pre.splats, bp, sp, lo.pix_err, out=sop)
                 ev[6].record()
                 torch.cuda.synchronize()
                 for i_ in range(6):
                     accp[i_] += ev[i_].elapsed_time(ev[i_ + 1])
-            paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 10, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
+            paper = {"n_pix_per_tile": 25, "n_hard": 10, "n_stable": 8, "beta": 0.4, "sampled_pixels_n": int(sp.n), "pairs_P_all_tiles": int(bp.P),
                      "sample_paper_ms": accp[0] / args.steps, "bin_sort_all_tiles_ms": accp[1] / args.steps,
                      "raster_fwd_ms": accp[2] / args.steps, "raster_bwd_ms": accp[3] / args.steps,
                      "maps_update_ms": accp[4] / args.steps, "raster_stats_ms": accp[5] / args.steps,
