@@ -151,30 +151,38 @@ class Oracle:
                                tile_pix_offsets=tpo[:k + 1].copy(), pix=pix[:n].copy())
 
     # ---- O4 ------------------------------------------------------------------------------
-    def raster_fwd(self, cam, binned, pre, samp):
+    def raster_fwd(self, cam, binned, pre, samp, margin_thr=2e-6):
+        """margin[n,2]: smallest relative distance of a tested quantity to its threshold along the walk (forward
+        decisions; forward + the 0.99 clamp that only the derivative sees).  flip_w[n]: the compositing weight that
+        moves if every decision closer than margin_thr to its threshold is taken the other way."""
         n = samp.n
         o = SimpleNamespace(color=np.zeros((n, 3), self.real), T=np.zeros(n, self.real),
                             n_contrib=np.zeros(n, np.uint32), n_walked=np.zeros(n, np.uint32),
-                            margin=np.ones((n, 2), self.real))
+                            margin=np.ones((n, 2), self.real), flip_w=np.zeros(n, self.real))
         c = self.cam(cam)
         self.lib.orc_raster_fwd(C.byref(c), _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
                                 _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.rgb)),
                                 samp.k, _ptr(samp.tiles), _ptr(samp.tile_pix_offsets), _ptr(samp.pix),
-                                _ptr(o.color), _ptr(o.T), _ptr(o.n_contrib), _ptr(o.n_walked), _ptr(o.margin))
+                                _ptr(o.color), _ptr(o.T), _ptr(o.n_contrib), _ptr(o.n_walked), _ptr(o.margin),
+                                self._creal(margin_thr), _ptr(o.flip_w))
         return o
 
     # ---- O5 ------------------------------------------------------------------------------
-    def raster_bwd(self, cam, binned, pre, samp, fwd, dL_dcolor):
+    def raster_bwd(self, cam, binned, pre, samp, fwd, dL_dcolor, want_abs=False):
+        """want_abs: also return sum_abs[N,9] (fp64), the sum of |term| behind every gradient element in the
+        order mean2D[2], conic[3], opacity, rgb[3]."""
         N = pre.means2D.shape[0]
         g = self.r(dL_dcolor).reshape(samp.n, 3)
         o = SimpleNamespace(dL_dmeans2D=np.zeros((N, 2), self.real), dL_dconic=np.zeros((N, 3), self.real),
-                            dL_dopacity=np.zeros(N, self.real), dL_drgb=np.zeros((N, 3), self.real))
+                            dL_dopacity=np.zeros(N, self.real), dL_drgb=np.zeros((N, 3), self.real),
+                            sum_abs=np.zeros((N, 9), np.float64) if want_abs else None)
         c = self.cam(cam)
         self.lib.orc_raster_bwd(C.byref(c), N, _ptr(binned.tile_offsets), _ptr(binned.gid_sorted),
                                 _ptr(self.r(pre.means2D)), _ptr(self.r(pre.conic_opacity)), _ptr(self.r(pre.rgb)),
                                 samp.k, _ptr(samp.tiles), _ptr(samp.tile_pix_offsets), _ptr(samp.pix),
                                 _ptr(self.r(fwd.T)), _ptr(fwd.n_contrib), _ptr(g),
-                                _ptr(o.dL_dmeans2D), _ptr(o.dL_dconic), _ptr(o.dL_dopacity), _ptr(o.dL_drgb))
+                                _ptr(o.dL_dmeans2D), _ptr(o.dL_dconic), _ptr(o.dL_dopacity), _ptr(o.dL_drgb),
+                                _ptr(o.sum_abs))
         return o
 
     # ---- O6 ------------------------------------------------------------------------------

@@ -462,7 +462,8 @@ void orc_raster_fwd(const orc_cam* cam, const uint32_t* tile_offsets, const uint
                     const real* mean2D, const real* conic_o, const real* rgb, int k,
                     const uint32_t* tiles, const uint32_t* tile_pix_offsets, const uint32_t* pix,
                     real* out_color, real* out_T, uint32_t* n_contrib, uint32_t* n_walked,
-                    real* margin /* [n,2]: forward, backward; nullable */) {
+                    real* margin /* [n,2]: forward, backward; nullable */,
+                    real margin_thr, real* flip_w /* [n]; nullable */) {
     const int W = cam->W;
     for (int it = 0; it < k; ++it) {
         uint32_t t = tiles[it];
@@ -472,6 +473,11 @@ void orc_raster_fwd(const orc_cam* cam, const uint32_t* tile_offsets, const uint
             real T = K_(1.0), C[3] = {0, 0, 0};
             uint32_t last = 0, walked = 0;
             real mg = K_(1.0), mgb = K_(1.0); /* distance to the nearest decision threshold */
+            /* flip_w: compositing weight that moves if every decision within margin_thr of its threshold is
+             * taken the other way: a skipped / kept Gaussian at alpha ~ 1/255
+             * moves alpha T of weight onto or off itself and as much off or onto everything behind it; a stop
+             * taken or not taken moves at most the transmittance T still unspent at that point. */
+            real flip = 0;
             for (uint32_t j = start; j < end; ++j) {
                 ++walked;
                 uint32_t g = gid_sorted[j];
@@ -481,10 +487,12 @@ void orc_raster_fwd(const orc_cam* cam, const uint32_t* tile_offsets, const uint
                 real oG = conic_o[4 * g + 3] * rexp(power);
                 real alpha = rmin(ALPHA_MAX, oG);
                 mg = rmin(mg, rel_margin(oG, ALPHA_MIN));
+                if (rel_margin(oG, ALPHA_MIN) < margin_thr) flip += alpha * T;
                 if (alpha < ALPHA_MIN) continue;
                 mgb = rmin(mgb, rel_margin(oG, ALPHA_MAX)); /* only the derivative jumps at the 0.99 clamp */
                 real Tn = T * (K_(1.0) - alpha);
                 mg = rmin(mg, rel_margin(Tn, T_MIN));
+                if (rel_margin(Tn, T_MIN) < margin_thr) flip += T;
                 if (Tn < T_MIN) break;
                 real w = alpha * T;
                 C[0] += rgb[3 * g] * w; C[1] += rgb[3 * g + 1] * w; C[2] += rgb[3 * g + 2] * w;
@@ -498,6 +506,7 @@ void orc_raster_fwd(const orc_cam* cam, const uint32_t* tile_offsets, const uint
             n_contrib[ip] = last;
             if (n_walked) n_walked[ip] = walked;
             if (margin) { margin[2 * ip] = mg; margin[2 * ip + 1] = rmin(mg, mgb); }
+            if (flip_w) flip_w[ip] = flip;
         }
     }
 }
@@ -507,9 +516,14 @@ void orc_raster_bwd(const orc_cam* cam, int N, const uint32_t* tile_offsets, con
                     const real* mean2D, const real* conic_o, const real* rgb, int k,
                     const uint32_t* tiles, const uint32_t* tile_pix_offsets, const uint32_t* pix,
                     const real* out_T, const uint32_t* n_contrib, const real* dL_dcolor,
-                    real* dL_dmean2D, real* dL_dconic, real* dL_dopac, real* dL_drgb) {
+                    real* dL_dmean2D, real* dL_dconic, real* dL_dopac, real* dL_drgb,
+                    double* sum_abs /* [N,9] nullable: per gradient element, the sum of |term| over the
+                                       (pixel, Gaussian) terms that were added -- the scale fp32 summation-order
+                                       noise is measured against; order mean2D[2],
+                                       conic[3], opacity, rgb[3] */) {
     const int W = cam->W;
     double* acc = (double*)calloc((size_t)N * 9, sizeof(double));
+    if (sum_abs) memset(sum_abs, 0, sizeof(double) * (size_t)N * 9);
     for (int it = 0; it < k; ++it) {
         uint32_t t = tiles[it];
         uint32_t start = tile_offsets[t];
@@ -534,10 +548,12 @@ void orc_raster_bwd(const orc_cam* cam, int N, const uint32_t* tile_offsets, con
                 T = T / om; /* T_k */
                 real w = alpha * T;
                 double* a = acc + (size_t)g * 9;
+                double* sa = sum_abs ? sum_abs + (size_t)g * 9 : NULL;
                 real dL_dalpha = 0;
                 for (int ch = 0; ch < 3; ++ch) {
                     real c = rgb[3 * g + ch];
                     a[6 + ch] += (double)(w * g3[ch]);
+                    if (sa) sa[6 + ch] += fabs((double)(w * g3[ch]));
                     dL_dalpha += ((c - S[ch]) * T - cam->bg[ch] * Tf / om) * g3[ch];
                     S[ch] = alpha * c + om * S[ch];
                 }
@@ -549,6 +565,14 @@ void orc_raster_bwd(const orc_cam* cam, int N, const uint32_t* tile_offsets, con
                     a[2] += (double)(K_(-0.5) * dx * dx * dL_dpower);
                     a[3] += (double)(-dx * dy * dL_dpower);
                     a[4] += (double)(K_(-0.5) * dy * dy * dL_dpower);
+                    if (sa) {
+                        sa[5] += fabs((double)(G * dL_dalpha));
+                        sa[0] += fabs((double)(dL_dpower * (-A * dx - B * dy)));
+                        sa[1] += fabs((double)(dL_dpower * (-Cc * dy - B * dx)));
+                        sa[2] += fabs((double)(K_(-0.5) * dx * dx * dL_dpower));
+                        sa[3] += fabs((double)(-dx * dy * dL_dpower));
+                        sa[4] += fabs((double)(K_(-0.5) * dy * dy * dL_dpower));
+                    }
                 }
             }
         }

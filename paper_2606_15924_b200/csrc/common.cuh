@@ -107,7 +107,7 @@ cudaError_t launch_raster_stats_lite(const CamK& cam, const float* splats, const
                                      uint32_t* sched, int num_sms, cudaStream_t s);
 
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
-                               const float* sh, const int32_t* radii, const uint8_t* clamped,
+                               const float* sh, const int32_t* radii, const uint8_t* clamped, const float* splats,
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
                                float* dsh, cudaStream_t s);
 

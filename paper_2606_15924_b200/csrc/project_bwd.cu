@@ -1,7 +1,7 @@
 // tgs_raster_bwd_sparse, projection half: chains dL/d(mean2D, conic, opacity, rgb) of every
 // Gaussian through the EWA projection and the SH colour to dL/d(mean3D, scale, quaternion,
 // opacity, SH) ("This pipeline is differentiable", 441).
-// One thread per Gaussian, no atomics; HBM-bound (reads 236 + 48 B, writes 236 B at degree 3).
+// One thread per Gaussian, no atomics; HBM-bound (reads 236 + 48 + 20 B, writes 236 B at degree 3).
 // The SH block (192 B in, 192 B out per Gaussian -- three quarters of the traffic) moves through
 // shared memory: the block's 128 x K x 3 coefficients are one contiguous span in HBM, copied with
 // coalesced float4 accesses into rows of odd stride (conflict-free for one-row-per-thread access),
@@ -71,7 +71,7 @@ template <int D>
 __global__ void __launch_bounds__(kPBThreads)
 project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const float* __restrict__ sc,
                    const float* __restrict__ qt, const float* __restrict__ sh, const int32_t* __restrict__ radii,
-                   const uint8_t* __restrict__ clamped, const float4* __restrict__ dsp,
+                   const uint8_t* __restrict__ clamped, const float4* __restrict__ spl, const float4* __restrict__ dsp,
                    float* __restrict__ dmu, float* __restrict__ dsc, float* __restrict__ dqt,
                    float* __restrict__ dop, float* __restrict__ dsh) {
     constexpr int K = (D + 1) * (D + 1);
@@ -113,6 +113,8 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
         for (int e = 0; e < K * 3; ++e) gsh[e] = 0.f;
     } else {
         const float4 d0 = dsp[3 * (size_t)i], d1 = dsp[3 * (size_t)i + 1], d2 = dsp[3 * (size_t)i + 2];
+        const float4 f0 = spl[3 * (size_t)i];
+        const float A = f0.z, B = f0.w, C = spl[3 * (size_t)i + 1].x;  // the forward's conic
         const float gmx = d0.x, gmy = d0.y, gA = d0.z, gB = d0.w, gC = d1.x;
         gop = d1.y;
         const float grgb[3] = {d1.z, d1.w, d2.x};
@@ -140,49 +142,34 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
         Rq[3] = 2.f * (x * y + w * z); Rq[4] = 1.f - 2.f * (x * x + z * z); Rq[5] = 2.f * (y * z - w * x);
         Rq[6] = 2.f * (x * z - w * y); Rq[7] = 2.f * (y * z + w * x); Rq[8] = 1.f - 2.f * (x * x + y * y);
         const float s[3] = {sc[3 * i], sc[3 * i + 1], sc[3 * i + 2]};
-        float M[9], Sg[9];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c) M[3 * r + c] = Rq[3 * r + c] * s[c];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-                Sg[3 * r + c] = M[3 * r] * M[3 * c] + M[3 * r + 1] * M[3 * c + 1] + M[3 * r + 2] * M[3 * c + 2];
-        float V[6];
-#pragma unroll
-        for (int r = 0; r < 2; ++r)
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-                V[3 * r + c] = Tm[3 * r] * Sg[c] + Tm[3 * r + 1] * Sg[3 + c] + Tm[3 * r + 2] * Sg[6 + c];
-        const float a = V[0] * Tm[0] + V[1] * Tm[1] + V[2] * Tm[2] + kLowpass;
-        const float b = V[0] * Tm[3] + V[1] * Tm[4] + V[2] * Tm[5];
-        const float c = V[3] * Tm[3] + V[4] * Tm[4] + V[5] * Tm[5] + kLowpass;
-        const float det = a * c - b * b;
-        const float idet = 1.0f / det;
-        const float A = c * idet, B = -b * idet, C = a * idet;
-        // ---- conic -> cov2D: H = -M Ghat M ----
+        // The conic (A, B, C) is the forward's own (splat record words 2..4).  With Sigma' = sum_k s_k^2 v_k v_k^T + 0.3 I,
+        // v_k = Tm R_k the projected k-th axis, everything downstream of dL/dSigma' = H = -M Ghat M (M = conic,
+        // Ghat = [[gA, gB/2], [gB/2, gC]]) only needs H v_k.  It is formed axis by axis as
+        //     y_k = M v_k,  w_k = Ghat y_k,  z_k = M w_k = -H v_k
+        // and H itself never: for a needle (condition number kappa of Sigma' large) the entries of H are ~kappa^2 larger
+        // than v^T H v along the long axis, so a gradient formed from H cancels kappa^2 of fp32 rounding; y_k = M v_k
+        // cancels only kappa, the sensitivity the 2x2 inverse has anyway.
+        //     dL/ds_k     = 2 s_k v_k^T H v_k            = -2 s_k (y_k . w_k)
+        //     dL/dM[:,k]  = 2 s_k Tm^T H v_k             = -2 s_k Tm^T z_k        (M = R diag(s), Sigma = M M^T)
+        //     dL/dTm      = 2 H Tm Sigma = 2 sum_k s_k^2 (H v_k) R_k^T = -2 sum_k s_k^2 z_k R_k^T
         const float hB = 0.5f * gB;
-        const float X00 = gA * A + hB * B, X01 = gA * B + hB * C, X10 = hB * A + gC * B, X11 = hB * B + gC * C;
-        const float H00 = -(A * X00 + B * X10), H01 = -(A * X01 + B * X11), H11 = -(B * X01 + C * X11);
-        float HT[6];
+        float dR[9], dTm[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-        for (int cc = 0; cc < 3; ++cc) {
-            HT[cc] = H00 * Tm[cc] + H01 * Tm[3 + cc];
-            HT[3 + cc] = H01 * Tm[cc] + H11 * Tm[3 + cc];
+        for (int k = 0; k < 3; ++k) {
+            const float v0 = Tm[0] * Rq[k] + Tm[1] * Rq[3 + k] + Tm[2] * Rq[6 + k];
+            const float v1 = Tm[3] * Rq[k] + Tm[4] * Rq[3 + k] + Tm[5] * Rq[6 + k];
+            const float y0 = A * v0 + B * v1, y1 = B * v0 + C * v1;
+            const float w0 = gA * y0 + hB * y1, w1 = hB * y0 + gC * y1;
+            const float z0 = A * w0 + B * w1, z1 = B * w0 + C * w1;
+            gs[k] = -2.f * s[k] * (y0 * w0 + y1 * w1);
+            const float m2s2 = -2.f * s[k] * s[k];
+#pragma unroll
+            for (int r = 0; r < 3; ++r) {
+                dR[3 * r + k] = m2s2 * (Tm[r] * z0 + Tm[3 + r] * z1);  // dL/dM[r][k] * s_k
+                dTm[r] = fmaf(m2s2 * z0, Rq[3 * r + k], dTm[r]);
+                dTm[3 + r] = fmaf(m2s2 * z1, Rq[3 * r + k], dTm[3 + r]);
+            }
         }
-        float dSg[9];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc) dSg[3 * r + cc] = Tm[r] * HT[cc] + Tm[3 + r] * HT[3 + cc];
-        float dTm[6];
-#pragma unroll
-        for (int r = 0; r < 2; ++r)
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc)
-                dTm[3 * r + cc] = 2.f * (HT[3 * r] * Sg[cc] + HT[3 * r + 1] * Sg[3 + cc] + HT[3 * r + 2] * Sg[6 + cc]);
         const float dJ00 = dTm[0] * W[0] + dTm[1] * W[1] + dTm[2] * W[2];
         const float dJ02 = dTm[0] * W[6] + dTm[1] * W[7] + dTm[2] * W[8];
         const float dJ11 = dTm[3] * W[3] + dTm[4] * W[4] + dTm[5] * W[5];
@@ -198,20 +185,6 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
         dt2 += -gmx * cam.fx * t0 * itz2 - gmy * cam.fy * t1 * itz2;
 #pragma unroll
         for (int cc = 0; cc < 3; ++cc) gmu[cc] = W[cc] * dt0 + W[3 + cc] * dt1 + W[6 + cc] * dt2;
-        // ---- Sigma = M M^T ----
-        float dM[9];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc)
-                dM[3 * r + cc] = 2.f * (dSg[3 * r] * M[cc] + dSg[3 * r + 1] * M[3 + cc] + dSg[3 * r + 2] * M[6 + cc]);
-#pragma unroll
-        for (int cc = 0; cc < 3; ++cc) gs[cc] = Rq[cc] * dM[cc] + Rq[3 + cc] * dM[3 + cc] + Rq[6 + cc] * dM[6 + cc];
-        float dR[9];
-#pragma unroll
-        for (int r = 0; r < 3; ++r)
-#pragma unroll
-            for (int cc = 0; cc < 3; ++cc) dR[3 * r + cc] = dM[3 * r + cc] * s[cc];
         gq[0] = 2.f * (z * (dR[3] - dR[1]) + y * (dR[2] - dR[6]) + x * (dR[7] - dR[5]));
         gq[1] = 2.f * (y * (dR[1] + dR[3]) + z * (dR[2] + dR[6]) + w * (dR[7] - dR[5])) - 4.f * x * (dR[4] + dR[8]);
         gq[2] = 2.f * (x * (dR[1] + dR[3]) + w * (dR[2] - dR[6]) + z * (dR[5] + dR[7])) - 4.f * y * (dR[0] + dR[8]);
@@ -267,12 +240,13 @@ project_bwd_kernel(const CamK cam, int N, const float* __restrict__ mu, const fl
 }  // namespace
 
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
-                               const float* sh, const int32_t* radii, const uint8_t* clamped,
+                               const float* sh, const int32_t* radii, const uint8_t* clamped, const float* splats,
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
                                float* dsh, cudaStream_t s) {
     const int threads = kPBThreads, blocks = (N + threads - 1) / threads;
     const float4* dsp = reinterpret_cast<const float4*>(dL_dsplats);
-#define TGS_PB(DD) project_bwd_kernel<DD><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, sh, radii, clamped, dsp, dmu, dsc, dqt, dop, dsh)
+    const float4* spl = reinterpret_cast<const float4*>(splats);
+#define TGS_PB(DD) project_bwd_kernel<DD><<<blocks, threads, 0, s>>>(cam, N, mu, sc, qt, sh, radii, clamped, spl, dsp, dmu, dsc, dqt, dop, dsh)
     switch (D) {
         case 0: TGS_PB(0); break;
         case 1: TGS_PB(1); break;

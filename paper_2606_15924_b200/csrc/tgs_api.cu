@@ -284,7 +284,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
             return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: null pointer (projection half)");
         if (((uintptr_t)quats & 15) || ((uintptr_t)dL_dquats & 15) || ((uintptr_t)dL_dsplats & 15))
             return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: quats, dL_dquats, dL_dsplats must be 16-byte aligned");
-        e = launch_project_bwd(ck, N, sh_degree, means3D, scales, quats, sh, radii, clamped, dL_dsplats, dL_dmeans3D,
+        e = launch_project_bwd(ck, N, sh_degree, means3D, scales, quats, sh, radii, clamped, splats, dL_dsplats, dL_dmeans3D,
                                dL_dscales, dL_dquats, dL_dopacities, dL_dsh, s);
         if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (projection)", e);
     }

@@ -3,7 +3,8 @@ element by element, on the same seeded inputs.  Run on the B200 box with ``-m gp
 
 Bit exact: splat rect / depth / mean2D words, radii, clamp masks, sort keys, sorted ids, per-tile
 ranges, tile scores, sampled tiles and pixel lists.  Tolerance: forward 1e-5 rel / 1e-6 abs,
-gradients 1e-3 rel / 1e-5 abs (BASELINE.json north_star).
+gradients 1e-3 rel / 1e-5 abs (BASELINE.json north_star) plus the summation-order term of
+tests/helpers.py on EVERY element; threshold-fragile pixels get a zero upstream gradient on both sides.
 """
 from types import SimpleNamespace
 
@@ -11,8 +12,8 @@ import numpy as np
 import pytest
 
 import workloads
-from helpers import (MARGIN, binned_dev, check_forward, check_grad, dev, pack_splats, samp_dev, scene_dev,
-                     tainted_gaussians, u32, unpack_splats)
+from helpers import (MARGIN, binned_dev, chain_scale, check_chain_grads, check_forward, check_grad, check_raster_grads,
+                     colour_max, dev, drop_pixels, pack_splats, samp_dev, scene_dev, u32, unpack_splats, zero_fragile)
 
 pytestmark = pytest.mark.gpu
 
@@ -30,9 +31,18 @@ def tgs(torch):
     return pk.TGS(0)
 
 
+def _cfg1_full():
+    """configs[0]'s Gaussians and camera under a FULL mask: the config's own top-25 % tiles are the nearly empty ones
+    (22 listed Gaussians in total), so this scene carries config 1's raster parity."""
+    sc = workloads.make(1)
+    sc.tile_pct, sc.err, sc.target, sc.name = (100, 100), np.ones((128, 128), np.float32), None, "cfg1_full"
+    return sc
+
+
 def _scenes():
     return {
         "cfg1": lambda: workloads.make(1),
+        "cfg1_full": _cfg1_full,
         "small_rot": lambda: workloads.small_random_scene(7, 3000, 200, 136, sh_degree=3, bg=(0.1, 0.3, 0.2), spread=1.3,
                                                           log_scale=(-2.8, 0.6)),
         "small_d1": lambda: workloads.small_random_scene(8, 2000, 333, 77, sh_degree=1, spread=1.5, log_scale=(-3.0, 0.8)),
@@ -45,27 +55,37 @@ def _scenes():
 _cache = {}
 
 
-def oracle_run(name, orc32):
+def oracle_backward(orc32, orc64, sc, r, g):
+    """Oracle backward with the upstream gradient zeroed at threshold-fragile pixels, its sum|terms|, and the
+    propagated scale of the projection chain (helpers.chain_scale)."""
+    r.g, r.n_fragile = zero_fragile(g, r.fwd)
+    r.rbwd = orc32.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, r.g, want_abs=True)
+    # the chain takes no discrete decision of its own (the clamp flags and the cull are inputs): its referee is the
+    # fp64 build, evaluated on the fp32 referee's raster gradients
+    r.pbwd = orc64.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii,
+                               r.pre.clamped, r.rbwd.dL_dmeans2D, r.rbwd.dL_dconic, r.rbwd.dL_drgb)
+    r.scale = chain_scale(orc64, sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre, r.rbwd.sum_abs,
+                          grads=(r.rbwd.dL_dmeans2D, r.rbwd.dL_dconic, r.rbwd.dL_drgb))
+    return r
+
+
+def oracle_run(name, orc32, orc64):
     if name not in _cache:
         sc = _scenes()[name]()
-        g = None
         r = orc32.pipeline(sc, backward=False)
-        g = workloads.dl_dcolor(SCENES.index(name), r.samp.n)
-        r.rbwd = orc32.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, g)
-        r.pbwd = orc32.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii,
-                                   r.pre.clamped, r.rbwd.dL_dmeans2D, r.rbwd.dL_dconic, r.rbwd.dL_drgb)
-        r.g = g
+        oracle_backward(orc32, orc64, sc, r, workloads.dl_dcolor(SCENES.index(name), r.samp.n))
         r.sc = sc
+        r.cmax = colour_max(r.pre, sc.cam)
         _cache[name] = r
     return _cache[name]
 
 
-SCENES = ["cfg1", "small_rot", "small_d1", "small_d2", "cfg2"]
+SCENES = ["cfg1", "small_rot", "small_d1", "small_d2", "cfg2", "cfg1_full"]
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_preprocess_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_preprocess_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     d = scene_dev(sc, torch)
     out = tgs.preprocess(sc.cam, sc.sh_degree, d.means3D, d.scales, d.quats, d.opacities, d.sh)
@@ -84,8 +104,8 @@ def test_preprocess_parity(name, orc32, tgs, torch):
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_bin_sort_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_bin_sort_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     splats = dev(pack_splats(r.pre), torch)  # stage isolated: the oracle's upstream bits
     P = r.binned.P
@@ -107,15 +127,15 @@ def test_bin_sort_parity(name, orc32, tgs, torch):
     sel[r.samp.tiles] = 1
     rb = orc32.bin_sort(sc.cam, r.pre, tile_select=sel)
     out3 = tgs.bin_sort(sc.cam, splats, rb.P + 5, want_keys=True, tile_select=dev(sel.astype(np.int32), torch))
-    assert out3.P == rb.P and rb.P < P
+    assert out3.P == rb.P and (rb.P < P or r.samp.k == sc.cam.num_tiles)
     assert np.array_equal(u32(out3.tile_offsets), rb.tile_offsets)
     assert np.array_equal(u32(out3.gid_sorted)[:rb.P], rb.gid_sorted)
     assert np.array_equal(out3.keys_sorted.cpu().numpy().view(np.uint64)[:rb.P], rb.keys_sorted)
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_sample_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_sample_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     if sc.err is not None:
         out = tgs.sample(sc.cam, sc.tile_pct, sc.pixel_mode, sc.pix_rate, sc.sample_seed, err=dev(sc.err, torch))
@@ -156,22 +176,24 @@ def test_sample_modes(mode, pct, rate, orc32, tgs, torch):
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_raster_fwd_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_raster_fwd_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     splats = dev(pack_splats(r.pre), torch)
     b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
     out = tgs.raster_fwd_sparse(sc.cam, splats, b, s, want_walked=True)
     torch.cuda.synchronize()
-    rep = check_forward(out.color.cpu().numpy(), out.T.cpu().numpy(), u32(out.n_contrib), r.fwd)
+    rep = check_forward(out.color.cpu().numpy(), out.T.cpu().numpy(), u32(out.n_contrib), r.fwd, r.cmax)
     ok = r.fwd.margin[:, 0] > MARGIN
     assert np.array_equal(u32(out.n_walked)[ok], r.fwd.n_walked[ok])
+    if name != "cfg1":
+        assert (r.fwd.n_contrib > 0).mean() > 0.3  # the comparison is about composited pixels, not background
     print(name, rep)
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_raster_bwd_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_raster_bwd_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     splats = dev(pack_splats(r.pre), torch)
     b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
@@ -182,66 +204,64 @@ def test_raster_bwd_parity(name, orc32, tgs, torch):
     out = tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, b, s, fwd, dev(r.g, torch), d.means3D, d.scales, d.quats,
                                 d.sh, dev(r.pre.radii, torch), dev(r.pre.clamped, torch))
     torch.cuda.synchronize()
-    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)  # rows held to the loose bound only
-    assert good.mean() < 0.5
-    ds = out.dL_dsplats.cpu().numpy()
-    worst = {}
-    worst["mean2D"] = check_grad("dL_dmean2D", ds[:, 0:2], r.rbwd.dL_dmeans2D, good)
-    worst["conic"] = check_grad("dL_dconic", ds[:, 2:5], r.rbwd.dL_dconic, good)
-    worst["opacity"] = check_grad("dL_dopacity", ds[:, 5], r.rbwd.dL_dopacity, good)
-    worst["rgb"] = check_grad("dL_drgb", ds[:, 6:9], r.rbwd.dL_drgb, good)
-    assert not ds[:, 9:].any()
-    worst["means3D"] = check_grad("dL_dmeans3D", out.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
-    worst["scales"] = check_grad("dL_dscales", out.dL_dscales.cpu().numpy(), r.pbwd.dL_dscales, good)
-    worst["quats"] = check_grad("dL_dquats", out.dL_dquats.cpu().numpy(), r.pbwd.dL_dquats, good)
-    worst["sh"] = check_grad("dL_dsh", out.dL_dsh.cpu().numpy(), r.pbwd.dL_dsh, good)
-    worst["opac"] = check_grad("dL_dopacities", out.dL_dopacities.cpu().numpy(), r.rbwd.dL_dopacity, good)
-    assert np.abs(r.pbwd.dL_dmeans3D).max() > 1e-3  # a real gradient, not zeros against zeros
-    print(name, worst)
+    # every element of every row, strict bar + the summation-order term (helpers.check_grad); the upstream gradient
+    # is zero at the scene's threshold-fragile pixels on both sides, so no Gaussian is excluded
+    rep = check_raster_grads(out.dL_dsplats.cpu().numpy(), r.rbwd)
+    rep.update(check_chain_grads(out, r.pbwd, r.rbwd, r.scale))
+    if name != "cfg1":
+        assert np.abs(r.pbwd.dL_dmeans3D).max() > 1e-3  # a real gradient, not zeros against zeros
+    print(name, f"fragile pixels zeroed: {r.n_fragile}", rep)
 
 
 @pytest.mark.parametrize("name", SCENES)
-def test_end_to_end_all_gpu(name, orc32, tgs, torch):
+def test_end_to_end_all_gpu(name, orc32, orc64, tgs, torch):
     """preprocess -> bin_sort -> sample -> fwd -> bwd entirely on the GPU, no oracle data in between."""
     import paper_2606_15924_b200 as pk
-    r = oracle_run(name, orc32)
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     d = scene_dev(sc, torch)
     step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 1000, want_walked=True)
-    kw = dict(err=dev(sc.err, torch)) if sc.err is not None else None
-    if kw is None:
-        # config 1: the mask comes from a dense render (full mask) and its residual to the target
+    ref = r
+    if sc.err is not None:
+        kw = dict(err=dev(sc.err, torch))
+    else:
+        # config 1: the mask comes from the residual of a dense render (full mask) against the target.  The GPU's
+        # render differs from the oracle's in the last bits, so the oracle is re-run on the GPU's OWN render: the
+        # selection is integer work on those fp32 values and must then agree bit for bit.
         step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, (100, 100), 0,
                      err=torch.ones((sc.cam.height, sc.cam.width), device="cuda"))
         P, k, n = step.counts()
         img = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
         img[step.samp.pix[:n].long()] = step.fwd.color[:n]
-        kw = dict(render=img.reshape(sc.cam.height, sc.cam.width, 3).contiguous(), target=dev(sc.target, torch))
+        img = img.reshape(sc.cam.height, sc.cam.width, 3).contiguous()
+        kw = dict(render=img, target=dev(sc.target, torch))
+        ref = SimpleNamespace(pre=r.pre, binned=r.binned, sc=sc, cmax=r.cmax)
+        ref.samp = orc32.sample(sc.cam, sc.tile_pct, sc.pixel_mode, sc.pix_rate, sc.sample_seed, render=img.cpu().numpy(),
+                                target=sc.target)
+        ref.fwd = orc32.raster_fwd(sc.cam, r.binned, r.pre, ref.samp)
+        oracle_backward(orc32, orc64, sc, ref, workloads.dl_dcolor(0, ref.samp.n))
     step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
                  sc.sample_seed, **kw)
     P, k, n = step.counts()
-    assert k == r.samp.k
-    if sc.err is not None:
-        # the step bins only the sampled tiles (restrict=True): same ranges for those tiles
-        sel = np.zeros(sc.cam.num_tiles, np.uint32)
-        sel[r.samp.tiles] = 1
-        rb = orc32.bin_sort(sc.cam, r.pre, tile_select=sel)
-        assert P == rb.P
-        assert np.array_equal(u32(step.binned.tile_offsets), rb.tile_offsets)
-        assert np.array_equal(u32(step.binned.gid_sorted)[:P], rb.gid_sorted)
-        assert n == r.samp.n and np.array_equal(u32(step.samp.pix)[:n], r.samp.pix)
-        rep = check_forward(step.fwd.color[:n].cpu().numpy(), step.fwd.T[:n].cpu().numpy(),
-                            u32(step.fwd.n_contrib)[:n], r.fwd)
-        g = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
-        g[:n] = dev(r.g, torch)
-        bw = step.backward(g)
-        torch.cuda.synchronize()
-        good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
-        check_grad("dL_dmeans3D", bw.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
-        check_grad("dL_dscales", bw.dL_dscales.cpu().numpy(), r.pbwd.dL_dscales, good)
-        check_grad("dL_dquats", bw.dL_dquats.cpu().numpy(), r.pbwd.dL_dquats, good)
-        check_grad("dL_dsh", bw.dL_dsh.cpu().numpy(), r.pbwd.dL_dsh, good)
-        check_grad("dL_dopacities", bw.dL_dopacities.cpu().numpy(), r.rbwd.dL_dopacity, good)
+    assert k == ref.samp.k
+    # the step bins only the sampled tiles (restrict=True): same ranges for those tiles
+    sel = np.zeros(sc.cam.num_tiles, np.uint32)
+    sel[ref.samp.tiles] = 1
+    rb = orc32.bin_sort(sc.cam, r.pre, tile_select=sel)
+    assert P == rb.P
+    assert np.array_equal(u32(step.binned.tile_offsets), rb.tile_offsets)
+    assert np.array_equal(u32(step.binned.gid_sorted)[:P], rb.gid_sorted)
+    assert n == ref.samp.n and np.array_equal(u32(step.samp.pix)[:n], ref.samp.pix)
+    assert np.array_equal(u32(step.samp.tiles)[:k], ref.samp.tiles)
+    rep = check_forward(step.fwd.color[:n].cpu().numpy(), step.fwd.T[:n].cpu().numpy(),
+                        u32(step.fwd.n_contrib)[:n], ref.fwd, ref.cmax)
+    g = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
+    g[:n] = dev(ref.g, torch)
+    bw = step.backward(g)
+    torch.cuda.synchronize()
+    rep.update(check_raster_grads(bw.dL_dsplats.cpu().numpy(), ref.rbwd))
+    rep.update(check_chain_grads(bw, ref.pbwd, ref.rbwd, ref.scale))
+    print(name, rep)
 
 
 def test_full_mask_equals_dense_and_empty_gradients(orc32, tgs, torch):
@@ -394,7 +414,7 @@ def _check_loss(out, ref, n, k, torch):
 @pytest.mark.parametrize("name", ["cfg1", "small_d1", "cfg2"])
 def test_loss_sparse_parity_on_rendered_colours(name, orc32, orc64, tgs, torch):
     """The loss on the forward's own output (sparse pixel lists of the scene, seeded target image)."""
-    r = oracle_run(name, orc32)
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
     rng = np.random.default_rng(5)
     target = np.clip(rng.normal(0.5, 0.25, (sc.cam.height, sc.cam.width, 3)), 0, 1).astype(np.float32)
@@ -432,17 +452,14 @@ def test_loss_sparse_modes_and_edge_tiles(mode, pct, rate, orc32, orc64, tgs, to
 
 
 def test_loss_feeds_the_backward(orc32, orc64, tgs, torch):
-    """End of the chain: forward colours -> tgs_loss_sparse -> tgs_raster_bwd_sparse, all on the GPU, against
-    the oracle run the same way."""
-    r = oracle_run("small_rot", orc32)
+    """End of the chain: forward colours -> tgs_loss_sparse -> tgs_raster_bwd_sparse, all on the GPU.  The loss
+    kernel's dL/dcolor is held to the loss test's bar against the oracle's O7; the backward is then compared with the
+    oracle's backward of that SAME upstream gradient (rows of threshold-fragile pixels zeroed on both sides)."""
+    r = oracle_run("small_rot", orc32, orc64)
     sc = r.sc
     rng = np.random.default_rng(2)
     target = rng.random((sc.cam.height, sc.cam.width, 3)).astype(np.float32)
     ref_l = orc64.loss_sparse(sc.cam, r.samp, r.fwd.color, target)
-    g = ref_l.dL_dcolor.astype(np.float32)
-    rb = orc32.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, g)
-    pb = orc32.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii, r.pre.clamped,
-                           rb.dL_dmeans2D, rb.dL_dconic, rb.dL_drgb)
     import paper_2606_15924_b200 as pk
     d = scene_dev(sc, torch)
     step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 8)
@@ -452,36 +469,44 @@ def test_loss_feeds_the_backward(orc32, orc64, tgs, torch):
     assert (k, n) == (r.samp.k, r.samp.n)
     samp = SimpleNamespace(k=k, n=n, tile_pix_offsets=step.samp.tile_pix_offsets, pix=step.samp.pix)
     lo = tgs.loss_sparse(sc.cam, samp, fw.color, dev(target, torch), n_capacity=sc.cam.width * sc.cam.height)
+    g_gpu = lo.dL_dcolor[:n].cpu().numpy()
+    ok = r.fwd.margin[:, 0] > MARGIN  # (a fragile pixel's colour, hence its loss gradient, may differ by a flipped Gaussian)
+    assert np.abs(g_gpu - ref_l.dL_dcolor)[ok].max() <= 1e-4 * np.abs(ref_l.dL_dcolor).max()
+    ref = SimpleNamespace(pre=r.pre, binned=r.binned, samp=r.samp, fwd=r.fwd)
+    oracle_backward(orc32, orc64, sc, ref, g_gpu)
+    lo.dL_dcolor[:n] = dev(ref.g, torch)  # = g_gpu with the fragile rows zeroed
     bw = step.backward(lo.dL_dcolor)
     torch.cuda.synchronize()
-    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
-    check_grad("dL_dmeans3D", bw.dL_dmeans3D.cpu().numpy(), pb.dL_dmeans3D, good)
-    check_grad("dL_dsh", bw.dL_dsh.cpu().numpy(), pb.dL_dsh, good)
+    rep = check_raster_grads(bw.dL_dsplats.cpu().numpy(), ref.rbwd)
+    rep.update(check_chain_grads(bw, ref.pbwd, ref.rbwd, ref.scale))
+    print("loss -> backward", rep)
 
 
 # ---- f3: tgs_raster_stats_sparse against the oracle's O8 (Eq. 12) ------------------------------
 # Same bar as the gradients (fp32 atomics reorder the per-Gaussian sums): 1e-3 rel / 1e-5 abs with the block rule,
 # Gaussians reachable from a threshold-fragile pixel held to the loose bound; expected depth like the forward.
 @pytest.mark.parametrize("name", SCENES)
-def test_raster_stats_parity(name, orc32, tgs, torch):
-    r = oracle_run(name, orc32)
+def test_raster_stats_parity(name, orc32, orc64, tgs, torch):
+    r = oracle_run(name, orc32, orc64)
     sc = r.sc
-    e = np.random.default_rng(3).random(r.samp.n).astype(np.float32)
-    ref = orc32.raster_stats(sc.cam, r.binned, r.pre, r.samp, e)
+    # the statistics are sums of positive terms (no cancellation): the plain 1e-3 / 1e-5 bar on every element.  The
+    # threshold-fragile pixels are taken out of the lists on both sides (their walk may differ by one Gaussian).
+    samp = drop_pixels(r.samp, ~(r.fwd.margin[:, 0] > MARGIN))
+    assert samp.n >= 0.99 * r.samp.n
+    fw = orc32.raster_fwd(sc.cam, r.binned, r.pre, samp)
+    e = np.random.default_rng(3).random(samp.n).astype(np.float32)
+    ref = orc32.raster_stats(sc.cam, r.binned, r.pre, samp, e)
     out = tgs.raster_stats_sparse(sc.cam, dev(pack_splats(r.pre), torch), binned_dev(r.binned, torch, sc.cam.num_tiles),
-                                  samp_dev(r.samp, torch), dev(e, torch))
+                                  samp_dev(samp, torch), dev(e, torch))
     torch.cuda.synchronize()
     st = out.stats.cpu().numpy()
     assert (st[:, 3] == 0).all()
-    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
-    rep = check_grad("stats(E,D,W)", st[:, :3], ref.stats, good)
+    rep = check_grad("stats(E,D,W)", st[:, :3], ref.stats)
     assert ref.stats[:, 2].sum() > 0
     # sum_i W_i = sum_p (1 - T_final): the statistics walk is the forward's walk
-    assert np.isclose(st[:, 2].sum(dtype=np.float64), (1.0 - r.fwd.T.astype(np.float64)).sum(), rtol=1e-4)
-    d = out.depth[:r.samp.n].cpu().numpy()
-    ok = r.fwd.margin[:, 0] > MARGIN
-    assert ok.mean() > 0.99
-    assert np.allclose(d[ok], ref.depth[ok], rtol=1e-4, atol=1e-5), np.abs(d[ok] - ref.depth[ok]).max()
+    assert np.isclose(st[:, 2].sum(dtype=np.float64), (1.0 - fw.T.astype(np.float64)).sum(), rtol=1e-4)
+    d = out.depth[:samp.n].cpu().numpy()
+    assert np.allclose(d, ref.depth, rtol=1e-4, atol=1e-5), np.abs(d - ref.depth).max()
     print(name, rep)
 
 
@@ -491,15 +516,14 @@ def test_raster_stats_partial_tiles_and_empty(orc32, tgs, torch):
     pre = orc32.preprocess(sc.cam, 0, sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh)
     b = orc32.bin_sort(sc.cam, pre)
     s = orc32.sample(sc.cam, (60, 100), 1, (1, 3), 4, err=workloads.blob_error_map(np.random.default_rng(3), 180, 120, 5))
-    fw = orc32.raster_fwd(sc.cam, b, pre, s)
+    s = drop_pixels(s, ~(orc32.raster_fwd(sc.cam, b, pre, s).margin[:, 0] > MARGIN))
     ones = np.ones(s.n, np.float32)
     ref = orc32.raster_stats(sc.cam, b, pre, s, ones)
     splats = dev(pack_splats(pre), torch)
     out = tgs.raster_stats_sparse(sc.cam, splats, binned_dev(b, torch, sc.cam.num_tiles), samp_dev(s, torch), dev(ones, torch))
     torch.cuda.synchronize()
     st = out.stats.cpu().numpy()
-    good = tainted_gaussians(sc.N, b, s, fw)
-    check_grad("stats partial", st[:, :3], ref.stats, good)
+    check_grad("stats partial", st[:, :3], ref.stats)
     assert np.allclose(st[:, 0], st[:, 2], rtol=1e-5, atol=1e-6)
     # k = 0: nothing sampled
     empty = SimpleNamespace(k=0, n=0, tiles=torch.zeros(1, dtype=torch.int32, device="cuda"),
@@ -566,38 +590,35 @@ def test_sample_paper_degenerate_maps(orc32, tgs, torch):
         assert np.array_equal(nan(got), nan(want)) and np.array_equal(got[~nan(got)], want[~nan(want)])
 
 
-def test_paper_sampler_drives_the_raster(orc32, tgs, torch):
+def test_paper_sampler_drives_the_raster(orc32, orc64, tgs, torch):
     """The paper's pixel lists (few pixels in every tile: all units partial) through forward and backward."""
-    r = oracle_run("small_rot", orc32)
+    r = oracle_run("small_rot", orc32, orc64)
     sc = r.sc
     W, H = sc.cam.width, sc.cam.height
     E, A = _maps(np.random.default_rng(8), W, H)
     s = orc32.sample_paper(sc.cam, E, A, 25, 10, 10, seed=4)
     b = orc32.bin_sort(sc.cam, r.pre)
     fw = orc32.raster_fwd(sc.cam, b, r.pre, s)
-    g = workloads.dl_dcolor(3, s.n)
-    rb = orc32.raster_bwd(sc.cam, b, r.pre, s, fw, g)
+    g, _ = zero_fragile(workloads.dl_dcolor(3, s.n), fw)
+    rb = orc32.raster_bwd(sc.cam, b, r.pre, s, fw, g, want_abs=True)
     splats = dev(pack_splats(r.pre), torch)
     sd = tgs.sample_paper(sc.cam, dev(E.view(np.int16), torch), dev(A.view(np.int16), torch), 25, 10, 10, seed=4)
     assert sd.n == s.n and np.array_equal(u32(sd.pix)[:s.n], s.pix)
     bd = binned_dev(b, torch, sc.cam.num_tiles)
     out = tgs.raster_fwd_sparse(sc.cam, splats, bd, sd)
     torch.cuda.synchronize()
-    check_forward(out.color[:s.n].cpu().numpy(), out.T[:s.n].cpu().numpy(), u32(out.n_contrib)[:s.n], fw)
+    check_forward(out.color[:s.n].cpu().numpy(), out.T[:s.n].cpu().numpy(), u32(out.n_contrib)[:s.n], fw, r.cmax)
     bw = tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, bd, sd, out, dev(g, torch), project=False)
     torch.cuda.synchronize()
-    got = bw.dL_dsplats.cpu().numpy()  # [N,12]: 0..1 dL/dmean2D, 2..4 conic, 5 opacity, 6..8 rgb
-    good = tainted_gaussians(sc.N, b, s, fw)
-    check_grad("dL_dmean2D", got[:, 0:2], rb.dL_dmeans2D, good)
-    check_grad("dL_drgb", got[:, 6:9], rb.dL_drgb, good)
+    print("paper lists", check_raster_grads(bw.dL_dsplats.cpu().numpy(), rb))
 
 
-def test_step_replays_in_a_cuda_graph(orc32, tgs, torch):
+def test_step_replays_in_a_cuda_graph(orc32, orc64, tgs, torch):
     """The five calls enqueue only (sizes are read on the device), including the fork / join onto the context's
     side stream: a whole step is captured in a CUDA graph and replayed on new inputs, bit-identical lists and the
     same gradients as the eager step."""
     import paper_2606_15924_b200 as pk
-    r = oracle_run("small_rot", orc32)
+    r = oracle_run("small_rot", orc32, orc64)
     sc = r.sc
     d = scene_dev(sc, torch)
     err = dev(sc.err, torch)
@@ -630,10 +651,10 @@ def test_step_replays_in_a_cuda_graph(orc32, tgs, torch):
     torch.cuda.synchronize()
     assert step.counts() == (P, k, n)
     assert torch.equal(step.samp.pix[:n], eager_pix) and torch.equal(step.binned.gid_sorted[:P], eager_gid)
-    good = tainted_gaussians(sc.N, r.binned, r.samp, r.fwd)
+    # two runs of the same step differ only by the order of the atomics: twice the summation-order allowance
     for t_, ref in eager.items():
-        check_grad(t_ + " (graph vs eager)", getattr(step.bwd, t_).cpu().numpy(), ref.cpu().numpy(), good)
-    check_grad("dL_dmeans3D (graph vs oracle)", step.bwd.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, good)
+        check_grad(t_ + " (graph vs eager)", getattr(step.bwd, t_).cpu().numpy(), ref.cpu().numpy(), r.scale[t_], c=16.0)
+    check_grad("dL_dmeans3D (graph vs oracle)", step.bwd.dL_dmeans3D.cpu().numpy(), r.pbwd.dL_dmeans3D, r.scale["dL_dmeans3D"])
     # replay on changed inputs: move the Gaussians, the graph must follow (nothing was baked in)
     d.means3D.add_(0.01)
     graph.replay()
@@ -641,4 +662,6 @@ def test_step_replays_in_a_cuda_graph(orc32, tgs, torch):
     moved = step.bwd.dL_dmeans3D.clone()
     run()
     torch.cuda.synchronize()
-    check_grad("dL_dmeans3D (graph vs eager, moved)", moved.cpu().numpy(), step.bwd.dL_dmeans3D.cpu().numpy())
+    # (moved scene: the unmoved scene's scale is the right order of magnitude for the same sums)
+    check_grad("dL_dmeans3D (graph vs eager, moved)", moved.cpu().numpy(), step.bwd.dL_dmeans3D.cpu().numpy(),
+               r.scale["dL_dmeans3D"], c=32.0)

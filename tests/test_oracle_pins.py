@@ -5,6 +5,7 @@ an invariant, a brute-force enumeration, numpy linear algebra written from the d
 (Eq. 1) or central finite differences.  SURVEY.md section 8c lists them.
 """
 import math
+from types import SimpleNamespace
 
 import numpy as np
 import pytest
@@ -128,14 +129,93 @@ def test_ewa_general_vs_numpy_definition(orc64):
     assert n_vis > 50
 
 
-def test_jacobian_clamp_and_near_cull(orc64):
+# Visible Gaussians whose centre projects outside the image far enough for the Jacobian clamp (reading R3 / R8:
+# |t_x/t_z| > 1.3 (W/2)/fx = 0.65 on a 64x64, f = 64 view) but whose footprint still reaches into it.
+_QROT = np.array([0.8, 0.3, -0.4, 0.2]) / np.linalg.norm([0.8, 0.3, -0.4, 0.2])
+CLAMP_CASES = {
+    "x+": (np.array([0.75, 0.05, 1.0]), np.array([0.25, 0.2, 0.3]), _QROT, (1, 0)),
+    "x-": (np.array([-0.80, -0.10, 1.1]), np.array([0.3, 0.15, 0.25]), _QROT[[0, 2, 1, 3]], (-1, 0)),
+    "y+": (np.array([0.05, 0.78, 1.0]), np.array([0.2, 0.3, 0.25]), _QROT[[1, 0, 3, 2]], (0, 1)),
+    "y-": (np.array([-0.12, -0.85, 1.2]), np.array([0.2, 0.35, 0.3]), _QROT, (0, -1)),
+    "xy": (np.array([0.72, 0.74, 1.0]), np.array([0.3, 0.3, 0.2]), _QROT[[3, 1, 0, 2]], (1, 1)),
+}
+
+
+@pytest.mark.parametrize("case", sorted(CLAMP_CASES))
+def test_jacobian_clamp_forward_vs_numpy_definition(case, orc64):
+    """The clamped branch of O1.3 (t~ = +-lim t_z inside J only) against numpy matrices; the Gaussian is VISIBLE."""
     cam = cam_simple(64, 64, 64.0)
-    # far off-axis Gaussian (t_x/t_z = 3 > 1.3*0.5): clamp active, still matches the numpy definition
-    mu = np.array([3.0, 0.1, 1.0]); s = np.array([0.2, 0.1, 0.3]); q = np.array([1.0, 0, 0, 0])
+    mu, s, q, side = CLAMP_CASES[case]
     pre = orc64.preprocess(cam, 0, [mu], [s], [q], [0.5], np.zeros((1, 1, 3)))
+    assert pre.radii[0] > 0 and pre.tiles_touched[0] > 0, "the pin Gaussian must be visible"
+    lim = 1.3 * 0.5
+    rx, ry = mu[0] / mu[2], mu[1] / mu[2]
+    assert (abs(rx) > lim, abs(ry) > lim) == (side[0] != 0, side[1] != 0)
+    assert (np.sign(rx) == side[0] or side[0] == 0) and (np.sign(ry) == side[1] or side[1] == 0)
     t, cov, m, rad = ewa_numpy(cam, mu, s, q)
     inv = np.linalg.inv(cov)
-    assert np.allclose(pre.conic_opacity[0, :3], [inv[0, 0], inv[0, 1], inv[1, 1]], rtol=1e-10) or pre.radii[0] == 0
+    assert np.allclose(pre.conic_opacity[0, :3], [inv[0, 0], inv[0, 1], inv[1, 1]], rtol=1e-11, atol=0)
+    assert np.allclose(pre.means2D[0], m, rtol=1e-12)           # the mean is NOT clamped
+    assert pre.radii[0] == rad
+    gx, gy = cam.grid
+    want = [int(np.clip(math.floor((m[0] - rad) / 16), 0, gx)), int(np.clip(math.floor((m[1] - rad) / 16), 0, gy)),
+            int(np.clip(math.floor((m[0] + rad + 15) / 16), 0, gx)), int(np.clip(math.floor((m[1] + rad + 15) / 16), 0, gy))]
+    assert list(pre.rect[0]) == want
+    # the branch matters: the same projection without the clamp gives a different conic
+    R = np.asarray(cam.R, np.float64)
+    tt = R @ mu + np.asarray(cam.t, np.float64)
+    w, x, y, z = q
+    Rq = orc64.quat_to_R(q)
+    J = np.array([[cam.fx / tt[2], 0, -cam.fx * tt[0] / tt[2] ** 2], [0, cam.fy / tt[2], -cam.fy * tt[1] / tt[2] ** 2]])
+    inv_free = np.linalg.inv(J @ R @ Rq @ np.diag(s ** 2) @ Rq.T @ R.T @ J.T + 0.3 * np.eye(2))
+    assert not np.allclose(pre.conic_opacity[0, :3], [inv_free[0, 0], inv_free[0, 1], inv_free[1, 1]], rtol=1e-3)
+
+
+@pytest.mark.parametrize("case", sorted(CLAMP_CASES))
+def test_jacobian_clamp_backward_finite_differences(case, orc64):
+    """The clamped branches of O6 (dJ02/dt_x = 0, dJ02/dt_z = +-fx lim / t_z^2; same for y): fp64 central
+    differences on all ten geometry parameters of a visible, clamped Gaussian composited between two others."""
+    cam = cam_simple(64, 64, 64.0, bg=(0.2, 0.5, 0.1))
+    mu0, s0, q0, _ = CLAMP_CASES[case]
+    rng = np.random.default_rng(7)
+    sc = Scene("clamp", cam, 1,
+               np.array([mu0, [0.1, -0.05, 0.8], [-0.15, 0.1, 1.6]], np.float64),
+               np.array([s0, [0.12, 0.2, 0.1], [0.35, 0.3, 0.4]], np.float64),
+               np.array([q0, [1, 0, 0, 0], _QROT], np.float64), np.array([0.8, 0.35, 0.7]),
+               rng.normal(0.2, 0.4, (3, 4, 3)), (100, 100), 0)
+    full = full_mask(orc64, cam)
+    _, pre, b, fw = _loss64(orc64, sc, full, np.zeros((full.n, 3)))
+    assert (pre.radii > 0).all()
+    # a sparse pixel set kept away from every threshold (north_star: "a tiny scene"), where the clamped Gaussian blends
+    sel = np.nonzero((fw.margin[:, 1] > 1e-3) & (fw.n_contrib > 0))[0][::9]
+    tile_of = np.searchsorted(full.tile_pix_offsets, sel, side="right") - 1
+    its = np.unique(tile_of)
+    samp = SimpleNamespace(k=len(its), n=len(sel), tiles=full.tiles[its].copy(),
+                           tile_pix_offsets=np.concatenate([[0], np.cumsum([(tile_of == i).sum() for i in its])]).astype(np.uint32),
+                           pix=full.pix[sel].copy())
+    rvec = rng.standard_normal((samp.n, 3))
+    L0, pre, b, fw = _loss64(orc64, sc, samp, rvec)
+    assert fw.margin.min() > 1e-3 and samp.n > 100
+    rb = orc64.raster_bwd(cam, b, pre, samp, fw, rvec)
+    assert np.abs(rb.dL_dconic[0]).max() > 1e-3, "the clamped Gaussian must receive a gradient"
+    pb = orc64.project_bwd(cam, 1, sc.means3D, sc.scales, sc.quats, sc.sh, pre.radii, pre.clamped,
+                           rb.dL_dmeans2D, rb.dL_dconic, rb.dL_drgb)
+    h = 1e-6
+    for name, ga in (("means3D", pb.dL_dmeans3D), ("scales", pb.dL_dscales), ("quats", pb.dL_dquats)):
+        arr = getattr(sc, name)
+        scale = np.abs(ga[0]).max()
+        for j in range(arr.shape[1]):
+            old = arr[0, j]
+            arr[0, j] = old + h; Lp, prep, _, _ = _loss64(orc64, sc, samp, rvec)
+            arr[0, j] = old - h; Lm, prem, _, _ = _loss64(orc64, sc, samp, rvec)
+            arr[0, j] = old
+            assert np.array_equal(prep.rect, pre.rect) and np.array_equal(prem.rect, pre.rect)
+            fd = (Lp - Lm) / (2 * h)
+            assert abs(fd - ga[0, j]) <= 2e-6 * max(abs(ga[0, j]), 1e-3 * scale), (name, j, fd, ga[0, j])
+
+
+def test_near_plane_cull(orc64):
+    cam = cam_simple(64, 64, 64.0)
     # behind / at the near plane
     pre = orc64.preprocess(cam, 0, [[0, 0, 0.2], [0, 0, -1.0], [0, 0, 0.2001]], [[.1, .1, .1]] * 3, [[1, 0, 0, 0]] * 3,
                            [0.5] * 3, np.zeros((3, 1, 3)))
