@@ -838,19 +838,13 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
     cudaError_t e = cudaMemsetAsync(w.ctr, 0, w.zero_bytes, s);
     if (e != cudaSuccess) return e;
 
-    static bool opted_in = false;  // function attributes, set once per process
-    if (!opted_in) {
-        e = cudaFuncSetAttribute(seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmallSmem);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kMediumSmem);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1>,
-                                 cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLargeSmem);
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static SmemOptIn opt[3];  // per device
+    e = opt[0].ensure((const void*)seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4>, kSmallSmem);
+    if (e != cudaSuccess) return e;
+    e = opt[1].ensure((const void*)seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2>, kMediumSmem);
+    if (e != cudaSuccess) return e;
+    e = opt[2].ensure((const void*)seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1>, kLargeSmem);
+    if (e != cudaSuccess) return e;
 
     // Ks, K0-K2: cut the rects into pieces and regroup them by top-left tile
     int nblk = (N + 255) / 256;

@@ -63,6 +63,25 @@ __device__ __forceinline__ void unpack_rect(uint32_t rx, uint32_t ry, int& x0, i
 // Every kernel launch of the library is counted (tgs_launch_count).
 void count_launches(int n);
 
+// Kernels with more than 48 KB of shared memory opt in through a function attribute, which is PER DEVICE: one flag
+// per (kernel, device), set on the first launch on that device (a race between threads only sets it twice).
+constexpr int kMaxDevices = 64;
+struct SmemOptIn {
+    unsigned char done[kMaxDevices] = {};
+    cudaError_t ensure(const void* fn, size_t bytes) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return e;
+        if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+        if (!done[dev]) {
+            e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+            if (e != cudaSuccess) return e;
+            done[dev] = 1;
+        }
+        return cudaSuccess;
+    }
+};
+
 // ---- launchers (one per translation unit) ---------------------------------------------------
 cudaError_t launch_preprocess(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                               const float* op, const float* sh, float* splats, int32_t* radii,

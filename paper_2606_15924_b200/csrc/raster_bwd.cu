@@ -240,12 +240,9 @@ cudaError_t launch_raster_bwd(const CamK& cam, int N, const float* splats, const
     int blocks = num_sms * 3;
     if (blocks > k) blocks = k;
     constexpr size_t smem = sizeof(BwdShared);
-    static bool opted_in = false;  // attribute of the function, set once per process
-    if (!opted_in) {
-        e = cudaFuncSetAttribute(raster_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static SmemOptIn opt;  // per device
+    e = opt.ensure((const void*)raster_bwd_kernel, smem);
+    if (e != cudaSuccess) return e;
     raster_bwd_kernel<<<blocks, kRasterThreads, smem, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                           gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
                                                           dL_dsplats, sched);

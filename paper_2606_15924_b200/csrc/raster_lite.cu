@@ -491,13 +491,9 @@ cudaError_t launch_raster_bwd_lite(const CamK& cam, const float* splats, const u
     if (k <= 0) return cudaSuccess;
     int blocks = num_sms * 4;  // 54 KB of shared memory per block
     if (blocks > (k + kLiteWarps - 1) / kLiteWarps) blocks = (k + kLiteWarps - 1) / kLiteWarps;
-    static bool opted_in = false;  // attribute of the function, set once per process
-    if (!opted_in) {
-        cudaError_t e = cudaFuncSetAttribute(raster_bwd_lite_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)sizeof(LiteBwdShared));
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static SmemOptIn opt;  // per device
+    cudaError_t e = opt.ensure((const void*)raster_bwd_lite_kernel, sizeof(LiteBwdShared));
+    if (e != cudaSuccess) return e;
     raster_bwd_lite_kernel<<<blocks, kLiteWarps * 32, sizeof(LiteBwdShared), s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                              gid_sorted, k, tiles, tpo, pix, out_T, n_contrib, dL_dcolor,
                                                              dL_dsplats, sched);

@@ -209,12 +209,9 @@ cudaError_t launch_raster_stats(const CamK& cam, int N, const float* splats, con
     int blocks = num_sms * 3;
     if (blocks > k) blocks = k;
     constexpr size_t smem = sizeof(StatShared);
-    static bool opted_in = false;  // attribute of the function, set once per process
-    if (!opted_in) {
-        e = cudaFuncSetAttribute(raster_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        opted_in = true;
-    }
+    static SmemOptIn opt;  // per device
+    e = opt.ensure((const void*)raster_stats_kernel, smem);
+    if (e != cudaSuccess) return e;
     raster_stats_kernel<<<blocks, kRasterThreads, smem, s>>>(cam, reinterpret_cast<const float4*>(splats), tile_offsets,
                                                             gid_sorted, k, tiles, tpo, pix, pix_err, stats, out_depth, sched);
     count_launches(1);

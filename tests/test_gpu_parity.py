@@ -49,6 +49,10 @@ def _scenes():
         "small_d2": lambda: workloads.small_random_scene(9, 1500, 97, 211, sh_degree=2, bg=(1.0, 1.0, 1.0), spread=1.0,
                                                          log_scale=(-2.5, 0.7)),
         "cfg2": lambda: workloads.make(2),
+        # wide, large splats: 311 of the 971 visible Gaussians project beyond the Jacobian clamp (|t_x/t_z| or |t_y/t_z|
+        # above 1.3 tan(fov/2)) and still reach into the image; 102 of them receive a gradient (reading R3 / R8)
+        "clamp_vis": lambda: workloads.small_random_scene(12, 1500, 200, 136, sh_degree=2, bg=(0.3, 0.2, 0.1), spread=3.4,
+                                                          log_scale=(-1.6, 0.6)),
     }
 
 
@@ -80,7 +84,7 @@ def oracle_run(name, orc32, orc64):
     return _cache[name]
 
 
-SCENES = ["cfg1", "small_rot", "small_d1", "small_d2", "cfg2", "cfg1_full"]
+SCENES = ["cfg1", "small_rot", "small_d1", "small_d2", "cfg2", "cfg1_full", "clamp_vis"]
 
 
 @pytest.mark.parametrize("name", SCENES)
@@ -210,6 +214,10 @@ def test_raster_bwd_parity(name, orc32, orc64, tgs, torch):
     rep.update(check_chain_grads(out, r.pbwd, r.rbwd, r.scale))
     if name != "cfg1":
         assert np.abs(r.pbwd.dL_dmeans3D).max() > 1e-3  # a real gradient, not zeros against zeros
+    if name == "clamp_vis":  # the clamped branches of preprocess.cu / project_bwd.cu are exercised, with a gradient
+        t = sc.means3D.astype(np.float64) @ np.asarray(sc.cam.R, np.float64).T + np.asarray(sc.cam.t, np.float64)
+        cl = (np.abs(t[:, 0] / t[:, 2]) > 1.3 * 0.5 * sc.cam.width / sc.cam.fx) | (np.abs(t[:, 1] / t[:, 2]) > 1.3 * 0.5 * sc.cam.height / sc.cam.fy)
+        assert (cl & (r.pre.radii > 0) & (np.abs(r.pbwd.dL_dscales).max(axis=1) > 1e-4)).sum() >= 50
     print(name, f"fragile pixels zeroed: {r.n_fragile}", rep)
 
 
