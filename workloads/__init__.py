@@ -222,3 +222,41 @@ def small_random_scene(seed: int, n: int, width: int, height: int, sh_degree: in
     return Scene(f"small_{seed}", cam, sh_degree, mu.astype(np.float32), s.astype(np.float32), q,
                  o.astype(np.float32), sh.astype(np.float32), (50, 100), PIXEL_MODE_ALL,
                  sample_seed=seed, err=err)
+
+
+# ---- inputs of the moment-damped LM solve (no method arithmetic here) --------
+LM_KEYS = ("means3D", "scales", "quats", "opacities", "sh")
+_LM_SHAPES = {"means3D": (3,), "scales": (3,), "quats": (4,), "opacities": ()}
+# typical magnitudes of one view's per-Gaussian gradients in a 3DGS run (activated parameters)
+_LM_SIGMA = {"means3D": 2e-3, "scales": 5e-3, "quats": 1e-3, "opacities": 1e-2, "sh": 3e-3}
+
+
+def lm_state(seed: int, n: int, sh_degree: int = 3, views: int = 1, p_update: float = 0.7, warm: bool = True):
+    """Seeded optimiser state for `tgs_lm_solve`: per-view gradients [V, N, ...] (heavy tailed: N(0, sigma) times a
+    per-Gaussian log-normal factor; Gaussians outside `update` have zero gradients, as the sparse raster backward
+    leaves them), Adam moments m, v in the parameter layouts (warm: as after some iterations; cold: zeros) and
+    the update mask (int32, 1 = received a gradient).  Returns (grads, m, v, update), dicts keyed by LM_KEYS."""
+    rng = np.random.default_rng(20_000 + seed)
+    K = (sh_degree + 1) ** 2
+    shapes = dict(_LM_SHAPES, sh=(K, 3))
+    update = (rng.random(n) < p_update).astype(np.int32)
+    if n > 0:
+        update[0] = 1
+    boost = np.exp(rng.normal(0.0, 1.0, size=n))
+    grads, m, v = {}, {}, {}
+    for key in LM_KEYS:
+        shp = shapes[key]
+        ex = (slice(None),) + (None,) * len(shp)
+        sig = _LM_SIGMA[key]
+        g = rng.standard_normal((views, n) + shp) * sig
+        g *= (boost * update)[(None,) + ex]
+        if key == "sh":
+            g[:, :, 0, :] *= 3.0  # the DC band carries the larger gradient
+        grads[key] = g.astype(np.float32)
+        if warm:
+            m[key] = (rng.standard_normal((n,) + shp) * 0.5 * sig * boost[ex]).astype(np.float32)
+            v[key] = ((0.05 + rng.random((n,) + shp)) * (sig * boost[ex]) ** 2).astype(np.float32)
+        else:
+            m[key] = np.zeros((n,) + shp, np.float32)
+            v[key] = np.zeros((n,) + shp, np.float32)
+    return grads, m, v, update
