@@ -16,6 +16,8 @@
  *                                replacement on the error map, TopK age, remainder
  *   tgs_maps_update          f2  fp16 EMA error map, uint16 age map                  PAPER.md:97-109 (Eq. 3-4)
  *   tgs_raster_stats_sparse  f3  per-Gaussian E_i, D_i, W_i and expected depth       PAPER.md:212-223 (Eq. 12), Alg. 1 step 11
+ *   tgs_lm_solve             f4  moment-damped LM solve (10x10 + 4x4 Cholesky per       PAPER.md:231-239 (Eq. 14), 483-490 (Eq. 19),
+ *                                Gaussian), Adam for the higher SH coefficients         Alg. 1 steps 9-10
  *   tgs_fp32_peak                diagnostic: measured FFMA peak (roofline denominator)
  *
  * Conventions (all calls)
@@ -238,6 +240,43 @@ int tgs_sample_paper(tgs_ctx* ctx, const tgs_camera* cam, const uint16_t* E_half
  * round-to-nearest-even to fp16); every other pixel of E is left unchanged.  Updates both maps in place. */
 int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
                     const uint32_t* pix, const float* pix_err, float beta, void* stream);
+
+/* ---- f4: the moment-damped Levenberg-Marquardt solve (Sec. 3.9 Eq. 14;
+ * PAPER.md:483-490 App. A Eq. 19; Alg. 1 steps 9-10).
+ * A parameter set in the layouts of tgs_preprocess / tgs_raster_bwd_sparse; five DEVICE pointers in a host struct
+ * (copied by value into the launch, not retained). */
+typedef struct tgs_params {
+    float* means3D;   /* [N,3]   */
+    float* scales;    /* [N,3]   */
+    float* quats;     /* [N,4]   */
+    float* opacities; /* [N]     */
+    float* sh;        /* [N,K,3], K = (sh_degree+1)^2; the RGB DC term is sh[:,0,:] */
+} tgs_params;
+
+/* Per Gaussian, two blocks solved independently: geometry g = (position 3, scale 3, rotation 4) in
+ * R^10 and appearance a = (RGB DC 3, opacity 1) in R^4, each by
+ *     (J^T J + diag(sqrt(v) + eps)) Delta = -m                    (Eq. 14 = Eq. 19 left; Cholesky)
+ * and every higher SH coefficient by  Delta = -eta_sh m_hat / (sqrt(v_hat) + eps)      (Eq. 19 right).
+ *   grads   the V per-view gradients of this iteration, view major: grads->means3D is [V,N,3], ... grads->sh
+ *           [V,N,K,3] (V calls of tgs_raster_bwd_sparse writing into slices of one buffer).  Read only.
+ *           J ("estimated from the accumulated gradients") is the V x d matrix of the block's per-view
+ *           gradients, J^T J = sum_i g_i g_i^T; the accumulated gradient is gbar = sum_i g_i (R31-R32).
+ *   m, v    Adam moments in the parameter layouts, updated IN PLACE before the solve:
+ *           m <- beta1 m + (1-beta1) gbar, v <- beta2 v + (1-beta2) gbar^2.  Eq. 14 takes them as printed (no bias
+ *           correction); Eq. 19 right takes m_hat = m/(1-beta1^t), v_hat = v/(1-beta2^t), t >= 1.
+ *   update  [N] int32, nullable: a Gaussian with update == 0 keeps its moments and gets Delta = 0 (it received no
+ *           gradient; the sparse-Adam convention of Tab. 5).  NULL updates every Gaussian.
+ *   delta   nullable: receives Delta in the parameter layouts.
+ *   params  nullable: Alg. 1 step 10, params <- params + Delta in place.  At least one of delta / params.
+ * Arithmetic: fp32 storage; the moment sums, J^T J and the Cholesky factorisation / substitutions run in fp64
+ * registers (the systems mix parameter groups whose gradients differ by orders of magnitude: condition numbers
+ * of 1e4-1e8 would otherwise leave 1e-3-level errors in Delta); the Adam branch divides in fp32.  The system is
+ * positive definite for any J because sqrt(v) + eps > 0; eps must be > 0.  NaN inputs give NaN outputs, no trap.
+ * One fused kernel, no workspace, no synchronisation; V <= 64.  All sh pointers 16-byte aligned. */
+int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update,
+                 float beta1, float beta2, float eps, float eta_sh, int t,
+                 const tgs_params* m, const tgs_params* v, const tgs_params* delta, const tgs_params* params,
+                 void* stream);
 
 #ifdef __cplusplus
 }

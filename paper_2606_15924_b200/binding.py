@@ -26,7 +26,8 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
 SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
            "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse", "tgs_sample_paper",
-           "tgs_maps_update"]
+           "tgs_maps_update", "tgs_lm_solve"]
+PARAM_KEYS = ("means3D", "scales", "quats", "opacities", "sh")
 
 
 class TgsError(RuntimeError):
@@ -66,6 +67,22 @@ class Camera(C.Structure):
         return gx * gy
 
 
+class Params(C.Structure):
+    """tgs_params: five device pointers in the parameter layouts."""
+    _fields_ = [(k, C.c_void_p) for k in ("means3D", "scales", "quats", "opacities", "sh")]
+
+    @staticmethod
+    def of(ps) -> "Params":
+        """From a dict (or any object) holding the five device tensors under PARAM_KEYS."""
+        get = ps.__getitem__ if isinstance(ps, dict) else (lambda k: getattr(ps, k))
+        q = Params()
+        for k in PARAM_KEYS:
+            t = get(k)
+            assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32, "device, contiguous, fp32 tensors only"
+            setattr(q, k, t.data_ptr())
+        return q
+
+
 def load_library() -> C.CDLL:
     if not os.path.exists(LIB_PATH):
         raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_15924_b200.build` "
@@ -96,6 +113,8 @@ def load_library() -> C.CDLL:
     lib.tgs_sample_paper.argtypes = [vp, cam, vp, vp, i32, i32, i32, u64, vp, vp, vp, vp, C.POINTER(C.c_int32), vp,
                                      C.c_size_t, vp]
     lib.tgs_maps_update.argtypes = [vp, cam, vp, vp, vp, vp, vp, f32, vp]
+    ps = C.POINTER(Params)
+    lib.tgs_lm_solve.argtypes = [vp, i32, i32, i32, ps, vp, f32, f32, f32, f32, i32, ps, ps, ps, ps, vp]
     return lib
 
 
@@ -305,6 +324,22 @@ class TGS:
                                                      _p(samp.tile_pix_offsets), _p(samp.pix), _p(pix_err), _p(out.stats),
                                                      _p(out.depth), _stream(stream)))
         return out
+
+    # ---- f4: moment-damped LM solve (Alg. 1 steps 9-10) ----
+    def lm_solve(self, sh_degree, grads, m, v, update=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, t=1,
+                 want_delta=True, delta=None, params=None, stream=None):
+        """grads: parameter set with a leading view axis [V,N,...]; m, v (and params, if given) are updated in place.
+        Returns the delta parameter set (allocated here unless given; None if want_delta is False)."""
+        V, N = grads["opacities"].shape
+        if delta is None and want_delta:
+            delta = {k: torch.empty_like(m[k]) for k in PARAM_KEYS}
+        pg, pm, pv = Params.of(grads), Params.of(m), Params.of(v)
+        pd = Params.of(delta) if delta is not None else None
+        pp = Params.of(params) if params is not None else None
+        self._check(self.lib.tgs_lm_solve(self._h, N, sh_degree, V, C.byref(pg), _p(update), beta1, beta2, eps, eta_sh, int(t),
+                                          C.byref(pm), C.byref(pv), C.byref(pd) if pd is not None else None,
+                                          C.byref(pp) if pp is not None else None, _stream(stream)))
+        return delta
 
     # ---- a5 + a6 ----
     def raster_bwd_sparse(self, cam, sh_degree, splats, binned, samp, fwd, dL_dcolor, means3D=None, scales=None,

@@ -28,6 +28,7 @@ SOURCES = {
     "loss.cu": [],
     "raster_stats.cu": [],
     "raster_lite.cu": [],
+    "lm.cu": [],
 }
 
 

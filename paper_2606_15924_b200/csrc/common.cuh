@@ -145,4 +145,20 @@ cudaError_t launch_loss_sparse(int k, const uint32_t* tpo, const uint32_t* pix, 
                                float eps_l1, float eps_ncc, float eps_lam, float* dL_dcolor, float* pix_err,
                                float* tile_stats, float* loss, cudaStream_t s);
 
+// f4: parameter sets of tgs_lm_solve (device pointers in the parameter layouts).
+struct LmSet {
+    float* mu; float* sc; float* qt; float* op; float* sh;
+};
+
+struct LmArgs {
+    LmSet g, m, v, d, p;   // g: [V, N, ...] read only; d / p nullable as a whole (d.mu == nullptr, p.mu == nullptr)
+    const int32_t* update; // nullable
+    int N, K, V;
+    double b1, b2, eps;    // Eq. 14
+    double inv_bc1, inv_bc2;  // 1 / (1 - beta^t), Eq. 19 right
+    float eta, epsf;
+};
+
+cudaError_t launch_lm_solve(const LmArgs& a, cudaStream_t s);
+
 }  // namespace tgs

@@ -362,4 +362,39 @@ int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint1
     return TGS_OK;
 }
 
+int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update, float beta1,
+                 float beta2, float eps, float eta_sh, int t, const tgs_params* m, const tgs_params* v,
+                 const tgs_params* delta, const tgs_params* params, void* stream) {
+    if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (N < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: N < 0");
+    if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_lm_solve: sh_degree %d not in 0..3", sh_degree);
+    if (V < 1 || V > 64) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: V = %d outside 1..64", V);
+    if (!(beta1 >= 0.f && beta1 < 1.f) || !(beta2 >= 0.f && beta2 < 1.f) || !(eps > 0.f) || t < 1)
+        return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: need 0 <= beta < 1, eps > 0, t >= 1");
+    if (!grads || !m || !v || (!delta && !params)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: null parameter set");
+    if (N == 0) return TGS_OK;
+    const tgs_params* sets[5] = {grads, m, v, delta, params};
+    LmArgs a;
+    LmSet* dst[5] = {&a.g, &a.m, &a.v, &a.d, &a.p};
+    for (int i = 0; i < 5; ++i) {
+        const tgs_params* q = sets[i];
+        if (!q) { *dst[i] = LmSet{nullptr, nullptr, nullptr, nullptr, nullptr}; continue; }
+        if (!q->means3D || !q->scales || !q->quats || !q->opacities || !q->sh)
+            return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: null pointer in parameter set %d", i);
+        if ((uintptr_t)q->sh & 15) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: sh pointers must be 16-byte aligned");
+        *dst[i] = LmSet{q->means3D, q->scales, q->quats, q->opacities, q->sh};
+    }
+    a.update = update;
+    a.N = N; a.K = (sh_degree + 1) * (sh_degree + 1); a.V = V;
+    a.b1 = (double)beta1; a.b2 = (double)beta2; a.eps = (double)eps;
+    // bias corrections of Eq. 19 (right) are scalars of the call, formed in double on the host
+    double p1 = 1.0, p2 = 1.0;
+    for (int i = 0; i < t && (p1 > 0.0 || p2 > 0.0); ++i) { p1 *= a.b1; p2 *= a.b2; }
+    a.inv_bc1 = 1.0 / (1.0 - p1); a.inv_bc2 = 1.0 / (1.0 - p2);
+    a.eta = eta_sh; a.epsf = eps;
+    cudaError_t e = launch_lm_solve(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(ctx, "tgs_lm_solve", e);
+    return TGS_OK;
+}
+
 }  // extern "C"

@@ -1,0 +1,158 @@
+"""GPU parity of tgs_lm_solve against oracle/lm.py (numpy fp64), element by element, through the C ABI.
+
+Bars (f4): the kernel forms the moment sums, J^T J and the Cholesky solve in fp64 from the
+same fp32 inputs, so every output is the oracle's value rounded to fp32 up to the conditioning of the system in
+fp64 (negligible):  Delta of the LM blocks, m, v and the applied parameters within 1e-6 relative (a few fp32 ulp);
+Delta of the Adam branch (fp32 quotient) within 1e-5 relative.  Masked Gaussians: exactly zero / exactly unchanged.
+"""
+import numpy as np
+import pytest
+
+import workloads
+from oracle import lm
+
+pytestmark = pytest.mark.gpu
+
+# scalars of the call are fp32 on the ABI: both sides get the fp32-representable values
+B1, B2, EPS, ETA = (float(np.float32(x)) for x in (0.9, 0.999, 1e-8, 1.25e-4))
+KEYS = workloads.LM_KEYS
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    assert t.cuda.is_available(), "GPU tests need a CUDA device"
+    return t
+
+
+@pytest.fixture(scope="module")
+def tgs(torch):
+    import paper_2606_15924_b200 as pk
+    return pk.TGS(0)
+
+
+def _dev(ps, torch):
+    return {k: torch.from_numpy(np.ascontiguousarray(a)).cuda() for k, a in ps.items()}
+
+
+def _close(got, ref, rtol, what, atol=0.0):
+    got = np.asarray(got, np.float64)
+    err = np.abs(got - ref)
+    bar = atol + rtol * np.abs(ref)
+    bad = err > bar
+    assert not bad.any(), f"{what}: {bad.sum()} of {bad.size} off, worst {err[bad].max():.3e} vs ref {np.abs(ref[bad]).max():.3e}"
+    with np.errstate(divide="ignore", invalid="ignore"):
+        rel = np.where(ref != 0, err / np.abs(ref), 0.0)
+    return float(rel.max()) if rel.size else 0.0
+
+
+def _run(tgs, torch, seed, n, D, V, t, use_mask, with_params, p_update=0.7, warm=True):
+    grads, m, v, upd = workloads.lm_state(seed, n, D, views=V, p_update=p_update, warm=warm)
+    rng = np.random.default_rng(777 + seed)
+    params = {k: rng.standard_normal(m[k].shape).astype(np.float32) for k in KEYS} if with_params else None
+    d_ref, m_ref, v_ref, p_ref = lm.lm_solve(grads, m, v, upd if use_mask else None, B1, B2, EPS, ETA, t=t, params=params)
+    gd, md, vd = _dev(grads, torch), _dev(m, torch), _dev(v, torch)
+    pd = _dev(params, torch) if with_params else None
+    ud = torch.from_numpy(upd).cuda() if use_mask else None
+    dd = tgs.lm_solve(D, gd, md, vd, update=ud, beta1=B1, beta2=B2, eps=EPS, eta_sh=ETA, t=t, params=pd)
+    torch.cuda.synchronize()
+    worst = {}
+    for k in KEYS:
+        got = dd[k].cpu().numpy()
+        if k == "sh":
+            worst["d_dc"] = _close(got[:, 0, :], d_ref[k][:, 0, :], 1e-6, "delta sh DC", atol=1e-30)
+            if got.shape[1] > 1:
+                worst["d_adam"] = _close(got[:, 1:, :], d_ref[k][:, 1:, :], 1e-5, "delta sh (Adam)", atol=1e-30)
+        else:
+            worst["d_" + k] = _close(got, d_ref[k], 1e-6, "delta " + k, atol=1e-30)
+        worst["m_" + k] = _close(md[k].cpu().numpy(), m_ref[k], 1e-6, "m " + k, atol=1e-37)
+        worst["v_" + k] = _close(vd[k].cpu().numpy(), v_ref[k], 1e-6, "v " + k, atol=1e-37)
+        if with_params:
+            worst["p_" + k] = _close(pd[k].cpu().numpy(), p_ref[k], 1e-6, "params " + k, atol=1e-7)
+        if use_mask:
+            off = upd == 0
+            assert not got[off].any()
+            assert np.array_equal(md[k].cpu().numpy()[off], m[k][off]) and np.array_equal(vd[k].cpu().numpy()[off], v[k][off])
+            if with_params:
+                assert np.array_equal(pd[k].cpu().numpy()[off], params[k][off])
+    return worst
+
+
+@pytest.mark.parametrize("D", [0, 1, 2, 3])
+@pytest.mark.parametrize("V", [1, 3, 7])
+def test_lm_solve_parity(tgs, torch, D, V):
+    # sizes spanning several blocks of 128 and a ragged tail
+    w = _run(tgs, torch, 10 * D + V, 1000 + 37 * D, D, V, t=5, use_mask=True, with_params=(V == 3))
+    print(f"lm parity D={D} V={V}: worst relative errors " + ", ".join(f"{k} {x:.1e}" for k, x in w.items() if x > 2e-7))
+
+
+def test_lm_solve_no_mask_first_iteration(tgs, torch):
+    """t = 1 from zero moments (cold start): v = (1 - beta2) gbar^2 is tiny, the damping nearly vanishes and the
+    systems are at their worst conditioned."""
+    _run(tgs, torch, 50, 4099, 3, 2, t=1, use_mask=False, with_params=True, warm=False, p_update=1.0)
+
+
+def test_lm_solve_large_t_and_sizes(tgs, torch):
+    _run(tgs, torch, 51, 1, 3, 1, t=1000, use_mask=False, with_params=False)
+    _run(tgs, torch, 52, 127, 3, 4, t=30000, use_mask=True, with_params=True)
+    _run(tgs, torch, 53, 129, 1, 10, t=2, use_mask=True, with_params=False, p_update=0.1)
+
+
+def test_lm_solve_params_only_and_errors(tgs, torch):
+    """delta == NULL with params given is allowed (steps 9 and 10 fused); neither is an error; so are V = 0, eps = 0."""
+    import paper_2606_15924_b200 as pk
+    grads, m, v, upd = workloads.lm_state(60, 300, 3, views=2)
+    params = {k: np.ones_like(a) for k, a in m.items()}
+    _, _, _, p_ref = lm.lm_solve(grads, m, v, upd, B1, B2, EPS, ETA, t=3, params=params)
+    gd, md, vd, pd = _dev(grads, torch), _dev(m, torch), _dev(v, torch), _dev(params, torch)
+    out = tgs.lm_solve(3, gd, md, vd, update=torch.from_numpy(upd).cuda(), beta1=B1, beta2=B2, eps=EPS, eta_sh=ETA, t=3,
+                       want_delta=False, params=pd)
+    assert out is None
+    for k in KEYS:
+        _close(pd[k].cpu().numpy(), p_ref[k], 1e-6, "params " + k, atol=1e-7)
+    with pytest.raises(pk.TgsError):
+        tgs.lm_solve(3, gd, md, vd, want_delta=False, params=None)
+    with pytest.raises(pk.TgsError):
+        tgs.lm_solve(3, gd, md, vd, eps=0.0)
+    with pytest.raises(pk.TgsError):
+        tgs.lm_solve(3, gd, md, vd, t=0)
+    with pytest.raises(pk.TgsError):
+        tgs.lm_solve(4, gd, md, vd)
+
+
+def test_lm_solve_follows_the_backward(tgs, torch):
+    """The call as the step uses it: the per-view gradients are the outputs of tgs_raster_bwd_sparse for V views of one
+    scene (written into slices of one [V, N, ...] buffer), update = Gaussians visible in any view."""
+    import oracle
+    V = 2
+    scs = [workloads.small_random_scene(7 + i, 1200, 120, 88, sh_degree=3, spread=1.3, log_scale=(-2.8, 0.6)) for i in range(V)]
+    sc0 = scs[0]
+    N, K = sc0.N, 16
+    o = oracle.Oracle("f32")
+    g_np = {k: np.zeros((V,) + s, np.float32) for k, s in
+            (("means3D", (N, 3)), ("scales", (N, 3)), ("quats", (N, 4)), ("opacities", (N,)), ("sh", (N, K, 3)))}
+    vis = np.zeros(N, bool)
+    for i, sc in enumerate(scs):
+        sc.means3D, sc.scales, sc.quats, sc.opacities, sc.sh = sc0.means3D, sc0.scales, sc0.quats, sc0.opacities, sc0.sh
+        r = o.pipeline(sc, backward=False, restrict=True)
+        g = workloads.dl_dcolor(i, r.samp.n)
+        rb = o.raster_bwd(sc.cam, r.binned, r.pre, r.samp, r.fwd, g)
+        pb = o.project_bwd(sc.cam, sc.sh_degree, sc.means3D, sc.scales, sc.quats, sc.sh, r.pre.radii, r.pre.clamped,
+                           rb.dL_dmeans2D, rb.dL_dconic, rb.dL_drgb)
+        g_np["means3D"][i], g_np["scales"][i], g_np["quats"][i] = pb.dL_dmeans3D, pb.dL_dscales, pb.dL_dquats
+        g_np["opacities"][i], g_np["sh"][i] = rb.dL_dopacity, pb.dL_dsh
+        vis |= r.pre.radii > 0
+    _, m, v, _ = workloads.lm_state(70, N, 3, views=1)
+    upd = vis.astype(np.int32)
+    d_ref, m_ref, v_ref, _ = lm.lm_solve(g_np, m, v, upd, B1, B2, EPS, ETA, t=4)
+    gd, md, vd = _dev(g_np, torch), _dev(m, torch), _dev(v, torch)
+    dd = tgs.lm_solve(3, gd, md, vd, update=torch.from_numpy(upd).cuda(), beta1=B1, beta2=B2, eps=EPS, eta_sh=ETA, t=4)
+    torch.cuda.synchronize()
+    for k in KEYS:
+        got = dd[k].cpu().numpy()
+        if k == "sh":
+            _close(got[:, 0], d_ref[k][:, 0], 1e-6, "delta DC", atol=1e-30)
+            _close(got[:, 1:], d_ref[k][:, 1:], 1e-5, "delta sh", atol=1e-30)
+        else:
+            _close(got, d_ref[k], 1e-6, "delta " + k, atol=1e-30)
+        _close(md[k].cpu().numpy(), m_ref[k], 1e-6, "m " + k, atol=1e-37)
