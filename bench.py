@@ -402,7 +402,7 @@ def run_tgs(args):
     rep = Replicas("nccl", dev)  # replicas only: barrier + max / sum over ranks, no data-path collective
     world, rank = rep.world, rep.rank
 
-    scene = load_scene(args.config, args.pct)
+    scene = workloads.orbit_view(load_scene(args.config, args.pct), rep.view_seed(0))  # one view per rank, rank 0: the config's own
     scene.extra["config"] = args.config
     cam = scene.cam
     tg = pk.TGS(local)
@@ -643,8 +643,34 @@ def measure_next_rows(tg, w, args, dev, flush, world, fp32_peak_measured, peaks)
                  "maps_update_ms": accp[4] / args.steps, "raster_stats_ms": accp[5] / args.steps,
                  "raster_px_per_s": sp.n / ((accp[2] + accp[3]) / args.steps * 1e-3)}
         del E_half, age, sp, bp, fp, gp, sop
+    # f4: the moment-damped LM solve on this scene's Gaussians, V = 3 views (the lower end of K_t in [3, 10])
+    lm = None
+    if world == 1:
+        N, K, V = scene.N, (scene.sh_degree + 1) ** 2, 3
+        shp = dict(means3D=(N, 3), scales=(N, 3), quats=(N, 4), opacities=(N,), sh=(N, K, 3))
+        gL = torch.Generator(device=dev).manual_seed(2)
+        rnd = lambda s_, sc_: torch.randn(s_, device=dev, generator=gL) * sc_
+        lg = {k_: rnd((V,) + s_, 1e-3) for k_, s_ in shp.items()}
+        lmm = {k_: rnd(s_, 1e-3) for k_, s_ in shp.items()}
+        lv = {k_: torch.rand(s_, device=dev, generator=gL) * 1e-6 for k_, s_ in shp.items()}
+        ld = {k_: torch.empty(s_, device=dev) for k_, s_ in shp.items()}
+        tg.lm_solve(scene.sh_degree, lg, lmm, lv, t=5, delta=ld)
+        lm_ms = 0.0
+        for _ in range(args.steps):
+            flush.fill_(1.0)
+            la.record()
+            tg.lm_solve(scene.sh_degree, lg, lmm, lv, t=5, delta=ld)
+            lb.record()
+            torch.cuda.synchronize()
+            lm_ms += la.elapsed_time(lb)
+        lm_ms /= args.steps
+        row = 4 * (14 + 3 * K)                         # bytes of one parameter set per Gaussian (236 at degree 3)
+        lm_bytes = N * row * ((V + 2) + 3)             # read V gradients + m + v, write m + v + Delta
+        lm = {"views": V, "ms": lm_ms, "bytes_per_gaussian": row * (V + 5), "gbs": lm_bytes / (lm_ms * 1e-3) / 1e9,
+              "hbm_frac": lm_bytes / (lm_ms * 1e-3) / 1e9 / peaks["hbm_gbs"], "kernels": ["lm_geo_kernel", "lm_app_sh_kernel"]}
+        del lg, lmm, lv, ld
     stats_flops = FWD_FLOPS_WALK * w.walked + 12 * w.blended
-    return {"loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
+    return {"lm_solve": lm, "loss_sparse_ms": loss_ms, "loss_sparse_gbs": n * 44 / (loss_ms * 1e-3) / 1e9,
             "loss_sparse_hbm_frac": n * 44 / (loss_ms * 1e-3) / 1e9 / peaks["hbm_gbs"],
             "paper_regime": paper,
             "raster_stats_ms": stats_ms,

@@ -28,7 +28,8 @@
  *   - `stream` is a cudaStream_t passed as void*.  Calls only enqueue work; they do not
  *     synchronise, EXCEPT when a non-NULL `*_host` output is given (one cudaStreamSynchronize).
  *     All calls are CUDA-graph capturable when the `_host` outputs are NULL.
- *   - A context owns 32 bytes of device scheduler counters and one side stream (+ two events): the raster calls
+ *   - Every call makes the context's device current (cudaSetDevice) before it enqueues work.
+ *   - A context owns 32 bytes of device scheduler counters (+ 256 scratch bytes for tgs_fp32_peak) and one side stream (+ two events): the raster calls
  *     fork their warp-per-tile kernel onto it and join before returning to `stream` (also under graph capture).
  *     The raster calls of ONE context must therefore be ordered with respect to each other (same stream, or
  *     stream-ordered by the caller); use one context per concurrently working stream.
@@ -117,10 +118,13 @@ int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree,
  * P = number of emitted pairs is data dependent: P_dev[0] = P, P_dev[1] = 1 if P > P_capacity (then
  * the lists are invalid and, if P_host != NULL, the call returns TGS_ERR_CAPACITY).  P_host (host,
  * nullable) receives P and forces one stream synchronisation.
- * The sort is a hand-written radix sort: a counting sort on the tile id (most significant digit)
- * followed by an LSD radix sort of every tile's segment in shared memory over the varying depth
- * bits, ties by Gaussian id.  workspace: tgs_bin_sort_workspace_bytes (16 B per pair + 12 B per
- * tile), contents undefined on return. */
+ * The sort is hand written (no library sort / scan): the most significant digit -- the tile id -- is a counting
+ * sort (regroup by piece, ballot pair walk, per-tile counts and scan); every tile's segment is then ordered in shared
+ * memory in ONE distribution step (monotone interpolation of the depth bits into ~2m buckets, members of a bucket
+ * ranked by counting), ties by Gaussian id; a segment whose keys pile up in one bucket (equal depths) falls back to
+ * a stable LSD radix sort on (id, depth bits) in global memory.  The result is unique, hence deterministic.
+ * workspace: tgs_bin_sort_workspace_bytes (16 B per pair + 16 B per piece record + 12 B per tile), contents
+ * undefined on return. */
 int tgs_bin_sort_workspace_bytes(int N, int64_t P_capacity, int num_tiles, size_t* bytes);
 int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
                  const uint32_t* tile_select,
@@ -195,7 +199,8 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
  *   dL_dcolor  = 1/n (dl1/dx + lambda_tau dL_ncc-per-pixel/dx)                   (Eq. 17-18) is its exact derivative.
  * color, dL_dcolor, pix_err are indexed like the sampled-pixel list (tile order); target is [H,W,3].
  * k = number of sampled tiles (host value, as in the raster calls); n = tile_pix_offsets[k] is read on the
- * device.  Enqueues two kernels, no synchronisation, no workspace. */
+ * device.  Every tile must list 1 <= m <= 256 pixels (what tgs_sample / tgs_sample_paper produce); a tile with
+ * m == 0 is skipped (tile_stats = {0, 0, 0}, no contribution to loss), pixels beyond the 256th are ignored.  Enqueues two kernels, no synchronisation, no workspace. */
 int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* tile_pix_offsets,
                     const uint32_t* pix, const float* color, const float* target,
                     float eps_l1, float eps_ncc, float eps_lambda,
@@ -268,11 +273,13 @@ typedef struct tgs_params {
  *           gradient; the sparse-Adam convention of Tab. 5).  NULL updates every Gaussian.
  *   delta   nullable: receives Delta in the parameter layouts.
  *   params  nullable: Alg. 1 step 10, params <- params + Delta in place.  At least one of delta / params.
- * Arithmetic: fp32 storage; the moment sums, J^T J and the Cholesky factorisation / substitutions run in fp64
- * registers (the systems mix parameter groups whose gradients differ by orders of magnitude: condition numbers
- * of 1e4-1e8 would otherwise leave 1e-3-level errors in Delta); the Adam branch divides in fp32.  The system is
- * positive definite for any J because sqrt(v) + eps > 0; eps must be > 0.  NaN inputs give NaN outputs, no trap.
- * One fused kernel, no workspace, no synchronisation; V <= 64.  All sh pointers 16-byte aligned. */
+ * Arithmetic: fp32 storage.  For the two LM blocks the moment sums, J^T J and the Cholesky factorisation /
+ * substitutions run in fp64 registers (the systems mix parameter groups whose gradients differ by orders of
+ * magnitude: condition numbers of 1e4-1e8 would otherwise leave 1e-3-level errors in Delta); the Adam branch is
+ * fp32 throughout (IEEE sqrt and division).  The system is positive definite for any J because
+ * sqrt(v) + eps > 0; eps must be > 0.  NaN inputs give NaN outputs, no trap.
+ * Two kernels (geometry arrays; sh + opacity arrays), no workspace, no synchronisation; V <= 64.  All sh pointers
+ * 16-byte aligned. */
 int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update,
                  float beta1, float beta2, float eps, float eta_sh, int t,
                  const tgs_params* m, const tgs_params* v, const tgs_params* delta, const tgs_params* params,

@@ -21,8 +21,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "tgs_oracle.c")
 
 
+# ORACLE_SANITIZE=1: a second build with -fsanitize=address,undefined; run the CPU suite as
+#   ORACLE_SANITIZE=1 LD_PRELOAD="$(gcc -print-file-name=libasan.so) $(gcc -print-file-name=libubsan.so)" \
+#   ASAN_OPTIONS=detect_leaks=0 python -m pytest tests -q -m "not gpu"
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+
+
 def _lib_path(prec: str) -> str:
-    return os.path.join(_HERE, f"liboracle_{prec}.so")
+    return os.path.join(_HERE, f"liboracle_{prec}{'_san' if _SANITIZE else ''}.so")
 
 
 def build(force: bool = False) -> None:
@@ -41,6 +47,8 @@ def build(force: bool = False) -> None:
             continue
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fPIC", "-shared",
                "-Wall", "-Wno-unused-function"] + (["-mfma"] if has_fma else []) + define + \
+              (["-g", "-fno-omit-frame-pointer", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"]
+               if _SANITIZE else []) + \
               [_SRC, "-o", out + ".tmp", "-lm"]
         subprocess.run(cmd, check=True)
         os.replace(out + ".tmp", out)

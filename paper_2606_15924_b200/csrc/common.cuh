@@ -157,6 +157,7 @@ struct LmArgs {
     double b1, b2, eps;    // Eq. 14
     double inv_bc1, inv_bc2;  // 1 / (1 - beta^t), Eq. 19 right
     float eta, epsf;
+    float b1f, b2f, omb1f, omb2f, ibc1f, ibc2f;  // fp32 copies for the Adam branch (1 - beta and 1 / (1 - beta^t) rounded once)
 };
 
 cudaError_t launch_lm_solve(const LmArgs& a, cudaStream_t s);

@@ -32,6 +32,10 @@ loss_sparse_kernel(int k, const uint32_t* __restrict__ tpo, const uint32_t* __re
     const int it = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     if (it >= k) return;
     const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0, n = tpo[k];
+    if (m == 0) {  // an empty tile (never produced by the library's samplers): no pixel, no term
+        if (lane < 3) tile_stats[3 * (size_t)it + lane] = 0.f;
+        return;
+    }
     const float inv_m = 1.0f / (float)m, inv_n = 1.0f / (float)n;
 
     float x[kPerLane][3], y[kPerLane][3];

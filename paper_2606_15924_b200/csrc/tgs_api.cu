@@ -33,6 +33,16 @@ int cuda_fail(tgs_ctx* ctx, const char* where, cudaError_t e) {
     return fail(ctx, TGS_ERR_CUDA, "%s: %s", where, cudaGetErrorString(e));
 }
 
+constexpr size_t kCtxDeviceBytes = 8 * sizeof(uint32_t) + 256;
+
+// Every entry point makes its context's device current: a process may hold contexts on several GPUs.
+bool on_device(tgs_ctx* ctx, const char* where) {
+    cudaError_t e = cudaSetDevice(ctx->device);
+    if (e == cudaSuccess) return true;
+    cuda_fail(ctx, where, e);
+    return false;
+}
+
 bool cam_ok(const tgs_camera* c) {
     return c && c->width > 0 && c->height > 0 && c->fx > 0.f && c->fy > 0.f;
 }
@@ -65,9 +75,9 @@ int tgs_create(tgs_ctx** out, int device) {
     c->num_sms = prop.multiProcessorCount;
     e = cudaSetDevice(device);
     if (e != cudaSuccess) { delete c; return TGS_ERR_CUDA; }
-    // the only allocation the library ever makes: 32 bytes of scheduler counters, once per context
-    e = cudaMalloc((void**)&c->sched, 8 * sizeof(uint32_t));
-    if (e == cudaSuccess) e = cudaMemset(c->sched, 0, 8 * sizeof(uint32_t));
+    // the only allocation the library ever makes: scheduler counters + a scratch line, once per context
+    e = cudaMalloc((void**)&c->sched, kCtxDeviceBytes);  // 8 counter words + 256 B scratch (tgs_fp32_peak)
+    if (e == cudaSuccess) e = cudaMemset(c->sched, 0, kCtxDeviceBytes);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&c->side.aux, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->side.fork, cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->side.join, cudaEventDisableTiming);
@@ -108,10 +118,10 @@ __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, float a, flo
 int tgs_fp32_peak(tgs_ctx* ctx, int reps, double* tflops, void* stream) {
     if (!ctx || !tflops || reps < 1) return TGS_ERR_INVALID_ARG;
     cudaStream_t s = (cudaStream_t)stream;
-    float* d = nullptr;
-    cudaEvent_t e0, e1;
-    cudaError_t e = cudaMalloc(&d, 256);
+    cudaError_t e = cudaSetDevice(ctx->device);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_fp32_peak", e);
+    float* d = reinterpret_cast<float*>(ctx->sched + 8);  // the context's scratch line
+    cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
     const int blocks = ctx->num_sms * 8, iters = 4096;
@@ -129,7 +139,6 @@ int tgs_fp32_peak(tgs_ctx* ctx, int reps, double* tflops, void* stream) {
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(d);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_fp32_peak", e);
     *tflops = best;
     return TGS_OK;
@@ -139,6 +148,7 @@ int tgs_preprocess(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree, co
                    const float* scales, const float* quats, const float* opacities, const float* sh,
                    float* splats, int32_t* radii, uint8_t* clamped, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_preprocess")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: bad camera");
     if (N < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_preprocess: N < 0");
     if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_preprocess: sh_degree %d not in 0..3", sh_degree);
@@ -166,6 +176,7 @@ int tgs_bin_sort(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats
                  uint64_t* keys_sorted, uint32_t* gid_sorted, uint32_t* tile_offsets, int64_t* P_dev,
                  int64_t* P_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_bin_sort")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: bad camera");
     if (N < 0 || P_capacity < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_bin_sort: negative size");
     if (P_capacity >= (1ll << 30) || (int64_t)N >= (1ll << 30))
@@ -213,6 +224,7 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const floa
                uint64_t seed, uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
                uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_sample")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: bad camera");
     if (tile_pct_den <= 0 || tile_pct_num < 0 || tile_pct_num > tile_pct_den)
         return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample: tile fraction %d/%d not in [0,1]", tile_pct_num, tile_pct_den);
@@ -247,6 +259,7 @@ int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const floa
                           const uint32_t* tile_pix_offsets, const uint32_t* pix, float* out_color, float* out_T,
                           uint32_t* n_contrib, uint32_t* n_walked, uint32_t* n_blended, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_raster_fwd_sparse")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad camera");
     if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_fwd_sparse: bad N or k");
     if (k == 0) return TGS_OK;
@@ -267,6 +280,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
                           const uint8_t* clamped, float* dL_dsplats, float* dL_dmeans3D, float* dL_dscales,
                           float* dL_dquats, float* dL_dopacities, float* dL_dsh, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_raster_bwd_sparse")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: bad camera");
     if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: bad N or k");
     if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_raster_bwd_sparse: sh_degree %d", sh_degree);
@@ -295,6 +309,7 @@ int tgs_loss_sparse(tgs_ctx* ctx, const tgs_camera* cam, int k, const uint32_t* 
                     const float* color, const float* target, float eps_l1, float eps_ncc, float eps_lambda,
                     float* dL_dcolor, float* pix_err, float* tile_stats, float* loss, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_loss_sparse")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: bad camera");
     if (k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_loss_sparse: k = %d outside 0..T", k);
     if (!(eps_l1 > 0.f) || !(eps_ncc > 0.f) || !(eps_lambda > 0.f))
@@ -312,6 +327,7 @@ int tgs_raster_stats_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const fl
                             const uint32_t* tile_pix_offsets, const uint32_t* pix, const float* pix_err, float* stats,
                             float* out_depth, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_raster_stats_sparse")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: bad camera");
     if (N < 0 || k < 0 || k > num_tiles(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_stats_sparse: bad N or k");
     if (!stats || (N > 0 && !splats) || (k > 0 && (!tile_offsets || !gid_sorted || !tiles || !tile_pix_offsets || !pix || !pix_err)))
@@ -328,6 +344,7 @@ int tgs_sample_paper(tgs_ctx* ctx, const tgs_camera* cam, const uint16_t* E_half
                      int n_hard, int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
                      int32_t* kn_dev, int32_t* kn_host, void* workspace, size_t workspace_bytes, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_sample_paper")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample_paper: bad camera");
     if (n_pix < 1 || n_pix > 256 || n_hard < 0 || n_stable < 0 || n_hard + n_stable > n_pix)
         return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_sample_paper: need 1 <= n_pix <= 256 and n_hard + n_stable <= n_pix (got %d, %d, %d)",
@@ -354,6 +371,7 @@ int tgs_sample_paper(tgs_ctx* ctx, const tgs_camera* cam, const uint16_t* E_half
 int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint16_t* age, const int32_t* kn_dev,
                     const uint32_t* pix, const float* pix_err, float beta, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_maps_update")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: bad camera");
     if (!(beta >= 0.f && beta <= 1.f)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: beta outside [0, 1]");
     if (!E_half || !age || !kn_dev || !pix || !pix_err) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_maps_update: null pointer");
@@ -366,6 +384,7 @@ int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* gr
                  float beta2, float eps, float eta_sh, int t, const tgs_params* m, const tgs_params* v,
                  const tgs_params* delta, const tgs_params* params, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
+    if (!on_device(ctx, "tgs_lm_solve")) return TGS_ERR_CUDA;
     if (N < 0) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: N < 0");
     if (sh_degree < 0 || sh_degree > 3) return fail(ctx, TGS_ERR_UNSUPPORTED, "tgs_lm_solve: sh_degree %d not in 0..3", sh_degree);
     if (V < 1 || V > 64) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_lm_solve: V = %d outside 1..64", V);
@@ -392,6 +411,8 @@ int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* gr
     for (int i = 0; i < t && (p1 > 0.0 || p2 > 0.0); ++i) { p1 *= a.b1; p2 *= a.b2; }
     a.inv_bc1 = 1.0 / (1.0 - p1); a.inv_bc2 = 1.0 / (1.0 - p2);
     a.eta = eta_sh; a.epsf = eps;
+    a.b1f = beta1; a.b2f = beta2; a.omb1f = (float)(1.0 - a.b1); a.omb2f = (float)(1.0 - a.b2);
+    a.ibc1f = (float)a.inv_bc1; a.ibc2f = (float)a.inv_bc2;
     cudaError_t e = launch_lm_solve(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(ctx, "tgs_lm_solve", e);
     return TGS_OK;

@@ -26,7 +26,8 @@ class Replicas:
             dist.init_process_group(backend, **kw)
             self._own = True
 
-    # one view per rank: the seed of rank r's view (the scene is replicated, the view differs)
+    # one view per rank: the index of rank r's view (the scene is replicated, the view differs; bench.py hands it to
+    # workloads.orbit_view, rank 0 keeps the config's own camera)
     def view_seed(self, base_seed: int) -> int:
         return int(base_seed) + self.rank
 

@@ -113,6 +113,26 @@ def _front_camera(width, height, f, dist) -> Camera:
                   np.eye(3, dtype=np.float32), np.array([0, 0, dist], dtype=np.float32))
 
 
+def orbit_view(scene: "Scene", view: int) -> "Scene":
+    """View `view` of a scene whose camera orbits the origin at the scene's distance: view 0 is the scene's own camera,
+    view r > 0 is turned by a seeded yaw in [-pi, pi) and pitch in [-0.3, 0.3] about the scene's centre (the Gaussian
+    clouds of configs 2-5 are centred there), keeping the distance.  Used by the N > 1 replicas: one view per rank
+    (PAPER.md:113).  Input generation only: no arithmetic of the method."""
+    if view == 0:
+        return scene
+    rng = np.random.default_rng(30_000 + int(view))
+    yaw, pitch = rng.uniform(-np.pi, np.pi), rng.uniform(-0.3, 0.3)
+    cy, sy, cp, sp = np.cos(yaw), np.sin(yaw), np.cos(pitch), np.sin(pitch)
+    Ry = np.array([[cy, 0, sy], [0, 1, 0], [-sy, 0, cy]])
+    Rx = np.array([[1, 0, 0], [0, cp, -sp], [0, sp, cp]])
+    c = scene.cam
+    R = (np.asarray(c.R, np.float64) @ Rx @ Ry).astype(np.float32)  # x_cam = R x_world + t with the same t: same distance
+    cam = Camera(c.width, c.height, c.fx, c.fy, c.cx, c.cy, R, c.t.copy(), c.znear, c.bg)
+    return Scene(f"{scene.name}_view{view}", cam, scene.sh_degree, scene.means3D, scene.scales, scene.quats, scene.opacities,
+                 scene.sh, scene.tile_pct, scene.pixel_mode, scene.pix_rate, scene.sample_seed + int(view), scene.err,
+                 scene.target, dict(scene.extra))
+
+
 def config1(seed: int = 0, n: int = 1024) -> Scene:
     """Tiny scene (BASELINE.json configs[0])."""
     rng = np.random.default_rng(seed)
