@@ -37,11 +37,12 @@ struct WarpXpose {
     float pb[32];                 // per pixel: g2
 };
 
-constexpr int kBwdStageEntries = 64;
+constexpr int kBwdStageEntries = 128;
+using BwdRing = Ring<kBwdStageEntries, false, 4>;
 
 struct BwdShared {
-    Ring<kBwdStageEntries> ring;
-    WarpBatch batch[kConsumers];
+    BwdRing ring;
+    WarpList<kBwdStageEntries> list[kConsumers];
     WarpXpose xpose[kConsumers];
 };
 
@@ -59,8 +60,8 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         producer_loop<true>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, n_contrib, sched, lane, kLitePixels);
         return;
     }
-    Ring<kBwdStageEntries>& R = sm.ring;
-    WarpBatch& sb = sm.batch[warp];
+    BwdRing& R = sm.ring;
+    uint32_t* const idx = sm.list[warp].idx;
     WarpXpose& sx = sm.xpose[warp];
     const uint32_t lt_mask = (1u << lane) - 1u;
     const int slot2 = lane & (kSlots - 1), half = lane >> 4;  // phase-2 role of this lane
@@ -99,8 +100,8 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         a6 += __shfl_xor_sync(0xffffffffu, a6, 16); a7 += __shfl_xor_sync(0xffffffffu, a7, 16);
         a8 += __shfl_xor_sync(0xffffffffu, a8, 16);
         // moments -> gradients:  dL/dmx = sum dpow (-A dx - B dy),  dL/dA = -1/2 sum dpow dx^2, ...
-        if (slot2 < m) {
-            const float4 gb = sx.mb[slot2];
+        const float4 gb = sx.mb[slot2];
+        if (slot2 < m && __float_as_uint(gb.z) != 0xffffffffu) {  // (a padding slot holds the stage's dummy record)
             float4* dst = reinterpret_cast<float4*>(dL_dsplats + (size_t)__float_as_uint(gb.z) * kSplatWords);
             const float dmx = fmaf(2.0f * ga.z, a0, ga.w * a1), dmy = fmaf(2.0f * gb.x, a1, ga.w * a0);
             const float dop = a5 / gb.y;  // dL/dopacity = sum G dL/dalpha = (sum dpow) / o
@@ -116,8 +117,8 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     };
 
     for (;;) {
-        const uint32_t s = gchunk % kStages;
-        mbar_wait(&R.full[s], (gchunk / kStages) & 1u);
+        const uint32_t s = gchunk % BwdRing::kStages;
+        mbar_wait(&R.full[s], (gchunk / BwdRing::kStages) & 1u);
         const StageInfo inf = R.info[s];
         if (inf.hdr != kHdrCont) {
             if (m > 0) flush();  // tail of the previous tile
@@ -148,69 +149,66 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         }
         if (wmax > 0) {
             const Stage<kBwdStageEntries>& st = R.st[s];
+            // ---- cull the stage against the pixel box; survivors' indices in range order (descending position) ----
+            uint32_t n = 0;
             for (uint32_t b0 = 0; b0 < inf.cnt; b0 += 32) {
                 // records of this batch sit at range positions base-b0 .. base-b0-31 (descending)
                 if (inf.base - b0 >= wmax + 31u && inf.base >= b0 + 31u) continue;  // all beyond this warp's deepest contributor
                 const uint32_t i = b0 + lane;
-                const bool have = i < inf.cnt;
                 const float4 q0 = st.p0[i];
-                const float4 q1 = st.p1[i];
-                const bool pass = have && splat_may_touch(q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, box);
+                const float2 c2 = st.ct[i];
+                const bool pass = i < inf.cnt && splat_may_touch(q0.x, q0.y, q0.z, q0.w, c2.x, c2.y, box);
                 const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
-                const int cnt = __popc(ballot);
-                __syncwarp();
-                if (pass) {
-                    const float4 q2 = st.p2[i];
-                    const int slot = __popc(ballot & lt_mask);
-                    sb.a[slot] = q0;
-                    sb.b[slot] = make_float4(q1.x, q1.y, q1.z, __uint_as_float(inf.base - i));
-                    sb.c[slot] = make_float4(q1.w, q2.x, q2.y, q2.z);
-                }
-                __syncwarp();
-                int e = 0;
-                while (e < cnt) {
-                    // ---- phase 1: replay the next survivors (as many as fit in the transposed tile), branch free ----
-                    const int take = min(cnt - e, kSlots - m);
-                    const float4* sa = sb.a + e;
-                    float2* vdst = sx.v + m * kTStride + lane;
-                    float4* mdst = sx.ma + m;
-#pragma unroll 2
-                    for (int ii = 0; ii < take; ++ii) {
-                        const float4 a = sa[ii];
-                        const float4 b = sa[32 + ii];
-                        const float4 c = sa[64 + ii];
-                        const float dx = a.x - px, dy = a.y - py;
-                        const float power = splat_power(a.z, a.w, b.x, dx, dy);
-                        // power is clamped for the exp only: G stays finite on lanes that fail the tests (no inf * 0)
-                        const float G = ex2_approx(fminf(power, 0.0f) * kLog2e);
-                        const float oG = __fmul_rn(b.z, G);
-                        const float alpha = fminf(kAlphaMax, oG);
-                        // (power >= thr is implied by the alpha test; thr only serves the cull)
-                        const bool valid = (__float_as_uint(b.w) < last) && (power <= 0.0f) && !(alpha < kAlphaMin);
-                        const float om = 1.0f - alpha;
-                        const float rom = rcp_approx(om);
-                        const float Tk = T * rom;  // T_k
-                        // only the projection of the colour behind onto dL/dcolor is needed: one scalar
-                        // recurrence Sg = S . g instead of three
-                        const float cg = fmaf(c.z, g2, fmaf(c.y, g1, c.x * g0));
-                        const float dL_dalpha = fmaf(cg - Sg, Tk, -bgdot * rom);
-                        // zero derivative through the active 0.99 clamp; invalid lanes contribute exact zeros
-                        const float dpow = (valid && oG < kAlphaMax) ? oG * dL_dalpha : 0.0f;  // dL/dpower
-                        const float w = valid ? alpha * Tk : 0.0f;
-                        T = valid ? Tk : T;
-                        Sg = valid ? fmaf(alpha, cg, om * Sg) : Sg;
-                        vdst[ii * kTStride] = make_float2(dpow, w);
-                    }
-                    if (lane < take) {  // the Gaussians' parameters for phase 2: one parallel copy per group
-                        const float4 b = sa[32 + lane];
-                        mdst[lane] = sa[lane];
-                        mdst[kSlots + lane] = make_float4(b.x, b.z, sa[64 + lane].w, 0.f);
-                    }
-                    e += take;
-                    m += take;
-                    if (m == kSlots) flush();
-                }
+                if (pass) idx[n + __popc(ballot & lt_mask)] = i;
+                n += __popc(ballot);
             }
+            // pad the list to a multiple of four with the stage's dummy record: groups stay aligned and m stays a
+            // multiple of four, so a group never straddles a flush
+            if (lane < 3) idx[n + lane] = (uint32_t)kBwdStageEntries;
+            n = (n + 3u) & ~3u;
+            __syncwarp();
+            for (uint32_t e = 0; e < n; e += 4) {
+                // ---- phase 1: replay four survivors in place, branch free ----
+                const uint4 j4 = *reinterpret_cast<const uint4*>(idx + e);
+                float2* vdst = sx.v + m * kTStride + lane;
+#pragma unroll
+                for (int ii = 0; ii < 4; ++ii) {
+                    const uint32_t i = ii == 0 ? j4.x : (ii == 1 ? j4.y : (ii == 2 ? j4.z : j4.w));
+                    const float4 a = st.p0[i];
+                    const float4 b = st.p1[i];  // -C/2, opacity, red, green
+                    const float blue = st.bl[i];
+                    const float dx = a.x - px, dy = a.y - py;
+                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                    const float G = ex2_approx(power * kLog2e);
+                    const float oG = __fmul_rn(b.y, G);
+                    const float alpha = fminf(kAlphaMax, oG);
+                    // (power >= thr is implied by the alpha test; thr only serves the cull); every use of a quantity
+                    // of an invalid lane below is a select, never a product: G may be inf there
+                    const bool valid = (inf.base - i < last) && (power <= 0.0f) && !(alpha < kAlphaMin);
+                    const float om = 1.0f - alpha;
+                    const float rom = rcp_approx(om);
+                    const float Tk = T * rom;  // T_k
+                    // only the projection of the colour behind onto dL/dcolor is needed: one scalar
+                    // recurrence Sg = S . g instead of three
+                    const float cg = fmaf(blue, g2, fmaf(b.w, g1, b.z * g0));
+                    const float dL_dalpha = fmaf(cg - Sg, Tk, -bgdot * rom);
+                    // zero derivative through the active 0.99 clamp; invalid lanes contribute exact zeros
+                    const float dpow = (valid && oG < kAlphaMax) ? oG * dL_dalpha : 0.0f;  // dL/dpower
+                    const float w = valid ? alpha * Tk : 0.0f;
+                    T = valid ? Tk : T;
+                    Sg = valid ? fmaf(alpha, cg, om * Sg) : Sg;
+                    vdst[ii * kTStride] = make_float2(dpow, w);
+                }
+                if (lane < 4) {  // the Gaussians' parameters for phase 2: one parallel copy per group
+                    const uint32_t i = idx[e + lane];
+                    const float4 b = st.p1[i];
+                    sx.ma[m + lane] = st.p0[i];
+                    sx.mb[m + lane] = make_float4(b.x, b.y, __uint_as_float(st.id[i]), 0.f);
+                }
+                m += 4;
+                if (m == kSlots) flush();
+            }
+            __syncwarp();  // the list is rewritten at the next stage
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&R.empty[s]);

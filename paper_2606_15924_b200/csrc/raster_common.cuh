@@ -31,37 +31,51 @@ namespace tgs {
 
 constexpr int kConsumers = 8;                        // consumer warps per block = units per tile
 constexpr int kRasterThreads = (kConsumers + 1) * 32;  // + 1 producer warp
-constexpr int kStages = 4;
 constexpr uint32_t kLitePixels = 32;  // tiles with at most this many sampled pixels go to the warp-per-tile kernels (raster_lite.cu)
 constexpr uint32_t kHdrCont = 0xfffffffeu, kHdrEnd = 0xffffffffu;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kLnAlphaMin = -5.541263545158426f;  // ln(1/255)
 
-// one staged record, as three float4 planes per stage:
-//   p0 = mx, my, -A/2, -B     p1 = -C/2, thr = ln(1/(255 o)) - 1e-5, opacity, red     p2 = green, blue, bits: Gaussian id, depth
-template <int ENTRIES>
-struct Stage {
-    float4 p0[ENTRIES];
-    float4 p1[ENTRIES];
-    float4 p2[ENTRIES];
-};
+// One staged record, split into planes so that every consumer access is as narrow as its use (profiles/r2b: both
+// raster kernels are bound by shared-memory wavefronts -- a warp-wide broadcast LDS.128 costs 2, LDS.64 / LDS.32 1):
+//   p0 = mx, my, -A/2, -B      p1 = -C/2, opacity, red, green      ct = -C/2, thr = ln(1/(255 o)) - 1e-5 (cull only)
+//   bl = blue                  id = Gaussian id                     dz = depth (statistics forward only)
+// Entry ENTRIES of every plane is a DUMMY record (opacity 0, id 0xffffffff) that never blends: lists of survivor
+// indices are padded with it to a multiple of four.
 struct StageInfo {
     uint32_t cnt;   // valid records in this stage
     uint32_t hdr;   // index into tiles[] of the sampled tile this stage STARTS, kHdrCont, or kHdrEnd
     uint32_t base;  // range position (0-based) of record 0; forward ascending, backward descending
     uint32_t pad;
 };
-template <int ENTRIES>
+template <int ENTRIES, bool DEPTH = false>
+struct Stage {
+    float4 p0[ENTRIES + 4];
+    float4 p1[ENTRIES + 4];
+    float2 ct[ENTRIES + 4];
+    float bl[ENTRIES + 4];
+    uint32_t id[ENTRIES + 4];
+    float dz[DEPTH ? ENTRIES + 4 : 4];
+};
+template <int ENTRIES, bool DEPTH = false, int STAGES = 4>
 struct Ring {
     static constexpr int kEntries = ENTRIES;
-    Stage<ENTRIES> st[kStages];
+    static constexpr bool kDepth = DEPTH;
+    static constexpr int kStages = STAGES;
+    Stage<ENTRIES, DEPTH> st[kStages];
     unsigned long long full[kStages], empty[kStages];
     StageInfo info[kStages];
     uint32_t done_seq[kConsumers];  // consumer w needs nothing more of the block's done_seq[w]-th tile
 };
 
-// a consumer's private survivors of one 32-record batch
+// a consumer's private list of the stage entries that survived its cull, in range order (block-per-tile kernels)
+template <int ENTRIES>
+struct WarpList {
+    uint32_t idx[ENTRIES + 4];
+};
+
+// a warp's private survivors of one 32-record batch (warp-per-tile kernels, raster_lite.cu)
 struct WarpBatch {
     float4 a[32];  // mx, my, -A/2, -B
     float4 b[32];  // -C/2, thr, opacity, bits: range position (fwd: 1-based, bwd: 0-based)
@@ -94,6 +108,13 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {  // relea
 }
 __device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t parity) {  // acquire.cta
     const uint32_t a = smem_u32(bar);
+    // A warp that waits (its pixels are saturated, it has no contributor left, or the producer is behind) must not
+    // take issue slots from the warps that work: profiles/r2b, r2c -- with a fixed 128 ns sleep, and likewise with
+    // try_wait's suspend-time hint (which the hardware caps far below a stage's duration), the polling loop was
+    // 16-18 % of all executed instructions while `not selected` was the top stall.  Exponential back-off: a short
+    // wait wakes within tens of ns, a long one (waiting for the other warps of the tile) polls every 2 us.  (Letting a
+    // warp with nothing left in its tile start at 2 us was slower: its late arrival on `empty` stalls the producer.)
+    uint32_t ns = 32;
     for (;;) {
         uint32_t ok;
         asm volatile(
@@ -104,9 +125,8 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* bar, uint32_t pari
             : "r"(a), "r"(parity)
             : "memory");
         if (ok) break;
-        // a warp that waits (its pixels are saturated, or the producer is behind) must not take issue
-        // slots from the warps that work (profiles/r1c: 13 % of all instructions were this loop)
-        __nanosleep(128);
+        __nanosleep(ns);
+        ns = min(ns * 2u, 2048u);
     }
 }
 
@@ -181,11 +201,21 @@ __device__ __forceinline__ PixelBox warp_pixel_box(bool active, int ipx, int ipy
 template <class RingT>
 __device__ __forceinline__ void ring_init(RingT& R) {
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kStages; ++s) {
+        for (int s = 0; s < RingT::kStages; ++s) {
             mbar_init(&R.full[s], 1u);
             mbar_init(&R.empty[s], (uint32_t)kConsumers);
         }
         for (int w = 0; w < kConsumers; ++w) R.done_seq[w] = 0u;
+        for (int s = 0; s < RingT::kStages; ++s) {  // the dummy record of every stage
+            auto& st = R.st[s];
+            constexpr int E = RingT::kEntries;
+            st.p0[E] = make_float4(0.f, 0.f, 0.f, 0.f);
+            st.p1[E] = make_float4(0.f, 0.f, 0.f, 0.f);
+            st.ct[E] = make_float2(0.f, 1.f);
+            st.bl[E] = 0.f;
+            st.id[E] = 0xffffffffu;
+            st.dz[RingT::kDepth ? E : 0] = 0.f;
+        }
     }
     __syncthreads();
 }
@@ -223,8 +253,8 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                 const uint32_t d = lane < kConsumers ? *(volatile uint32_t*)&R.done_seq[lane] : seq;
                 if (__all_sync(0xffffffffu, d >= seq)) break;
             }
-            const uint32_t s = gchunk % kStages;
-            mbar_wait(&R.empty[s], ((gchunk / kStages) & 1u) ^ 1u);
+            const uint32_t s = gchunk % RingT::kStages;
+            mbar_wait(&R.empty[s], ((gchunk / RingT::kStages) & 1u) ^ 1u);
             constexpr int kStageEntries = RingT::kEntries;
             const uint32_t cnt = min((uint32_t)kStageEntries, len - produced);
             auto& st = R.st[s];
@@ -253,9 +283,13 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                 for (int j = 0; j < 2; ++j) {
                     if (g[j] != 0xffffffffu) {
                         const int i = h * 64 + j * 32 + lane;
+                        const float nC = -0.5f * r1[j].x;
                         st.p0[i] = make_float4(r0[j].x, r0[j].y, -0.5f * r0[j].z, -r0[j].w);
-                        st.p1[i] = make_float4(-0.5f * r1[j].x, blend_threshold(r1[j].y), r1[j].y, r1[j].z);
-                        st.p2[i] = make_float4(r1[j].w, r2x[j].x, __uint_as_float(g[j]), r2x[j].y);
+                        st.p1[i] = make_float4(nC, r1[j].y, r1[j].z, r1[j].w);
+                        st.ct[i] = make_float2(nC, blend_threshold(r1[j].y));
+                        st.bl[i] = r2x[j].x;
+                        st.id[i] = g[j];
+                        if (RingT::kDepth) st.dz[i] = r2x[j].y;
                     }
                 }
             }
@@ -275,8 +309,8 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
         } while (produced < len);
     }
     // end of work
-    const uint32_t s = gchunk % kStages;
-    mbar_wait(&R.empty[s], ((gchunk / kStages) & 1u) ^ 1u);
+    const uint32_t s = gchunk % RingT::kStages;
+    mbar_wait(&R.empty[s], ((gchunk / RingT::kStages) & 1u) ^ 1u);
     if (lane == 0) {
         StageInfo inf;
         inf.cnt = 0; inf.hdr = kHdrEnd; inf.base = 0; inf.pad = 0;
