@@ -191,6 +191,7 @@ def workload_config(scene, args, P, k, n, cfg_index=None):
     return {"workload": f"BASELINE.json configs[{c}] ({scene.name})", "gaussians": scene.N,
             "sh_degree": scene.sh_degree, "image": [scene.cam.width, scene.cam.height],
             "tiles": scene.cam.num_tiles, "tile_pct": list(scene.tile_pct), "binning": "sampled tiles only (tile_select)",
+            "gradients": "sparse: touched mask + rows of the touched Gaussians (tgs_raster_bwd_sparse `touched`, the update mask of tgs_lm_solve)",
             "pixel_mode": "all" if scene.pixel_mode == 0 else "bernoulli_err", "pairs_P": None if P is None else int(P),
             "sampled_tiles_k": int(k), "sampled_pixels_n": int(n), "parallelism": f"replicas x{args.gpus}"}
 
@@ -239,8 +240,9 @@ class GpuWorkload:
                           sc.pix_rate, sc.sample_seed, err=D["err"])
 
     def full_step(self):
+        # gradients as (touched mask, rows of the touched Gaussians): what tgs_lm_solve consumes (tgs.h, sparse gradients)
         self.fwd()
-        self.step.backward(self.g_dev)
+        self.step.backward(self.g_dev, sparse=True)
 
     # ---- the step, launched call by call, CUDA events around each step, L2 flushed between steps ----
     def time_eager(self, steps, warmup, flush, rep, sampler=None):
@@ -316,7 +318,8 @@ class GpuWorkload:
                                  out=st.bwd)
             e_[5].record()
             tg.raster_bwd_sparse(cam, sc.sh_degree, st.pre.splats, st.binned, st.samp, st.fwd, self.g_dev, D["means3D"],
-                                 D["scales"], D["quats"], D["sh"], st.pre.radii, st.pre.clamped, project=True, out=st.bwd)
+                                 D["scales"], D["quats"], D["sh"], st.pre.radii, st.pre.clamped, project=True, out=st.bwd,
+                                 sparse=True)
             e_[6].record()
             torch.cuda.synchronize()
             d = [e_[i].elapsed_time(e_[i + 1]) for i in range(6)]

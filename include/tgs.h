@@ -172,7 +172,13 @@ int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const floa
  * inside the call).  Projection half: chains dL_dsplats through tgs_preprocess to
  * dL_dmeans3D[N,3] dL_dscales[N,3] dL_dquats[N,4] dL_dopacities[N] dL_dsh[N,K,3]; it is skipped when
  * dL_dmeans3D == NULL (then only dL_dsplats is produced).  Derivatives are those of the forward as
- * defined: zero through an active 0.99 alpha clamp, an active colour clamp and for culled Gaussians. */
+ * defined: zero through an active 0.99 alpha clamp, an active colour clamp and for culled Gaussians.
+ * touched[N] (int32, nullable): SPARSE GRADIENTS.  A Gaussian that is not listed in any sampled tile (or whose raster
+ * gradient record is all zero) has a zero gradient; with 5 % of the tiles sampled that is ~85 % of them.  NULL: their
+ * rows of the five outputs are written as zeros.  Given: touched[i] = 1 and rows written where the record is
+ * non-zero, touched[i] = 0 and the rows of i LEFT UNWRITTEN otherwise -- the mask is the `update` argument of
+ * tgs_lm_solve (sparse-Adam convention), and the step's cost then follows the sampled-tile fraction
+ * instead of N. */
 int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_degree,
                           const float* splats, const uint32_t* tile_offsets, const uint32_t* gid_sorted,
                           int k, const uint32_t* tiles, const uint32_t* tile_pix_offsets,
@@ -182,7 +188,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
                           const float* sh, const int32_t* radii, const uint8_t* clamped,
                           float* dL_dsplats,
                           float* dL_dmeans3D, float* dL_dscales, float* dL_dquats,
-                          float* dL_dopacities, float* dL_dsh, void* stream);
+                          float* dL_dopacities, float* dL_dsh, int32_t* touched, void* stream);
 
 /* ---- f1: sparse supervision (Sec. 3.7 Eq. 9-11, 472-481
  * Eq. 17-18).  Sits between the forward and the backward: from the forward's colours of the n sampled

@@ -106,7 +106,7 @@ def load_library() -> C.CDLL:
                                C.POINTER(C.c_int32), vp, C.c_size_t, vp]
     lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
-                                         [vp] + [vp] * 5 + [vp]
+                                         [vp] + [vp] * 5 + [vp, vp]
     f32 = C.c_float
     lib.tgs_loss_sparse.argtypes = [vp, cam, i32, vp, vp, vp, vp, f32, f32, f32, vp, vp, vp, vp, vp]
     lib.tgs_raster_stats_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp]
@@ -343,7 +343,10 @@ class TGS:
 
     # ---- a5 + a6 ----
     def raster_bwd_sparse(self, cam, sh_degree, splats, binned, samp, fwd, dL_dcolor, means3D=None, scales=None,
-                          quats=None, sh=None, radii=None, clamped=None, project=True, out=None, stream=None):
+                          quats=None, sh=None, radii=None, clamped=None, project=True, out=None, stream=None,
+                          sparse=False):
+        """sparse=True: out.touched[N] (int32) marks the Gaussians with a non-zero gradient; the rows of the others are
+        left unwritten (tgs.h: sparse gradients)."""
         cam = Camera.of(cam)
         N = splats.shape[0]
         if out is None:
@@ -355,10 +358,13 @@ class TGS:
                 out.dL_dquats = torch.empty((N, 4), dtype=torch.float32, device=self.device)
                 out.dL_dopacities = torch.empty(N, dtype=torch.float32, device=self.device)
                 out.dL_dsh = torch.empty((N, K, 3), dtype=torch.float32, device=self.device)
+        if sparse and getattr(out, "touched", None) is None:
+            out.touched = torch.empty(N, dtype=torch.int32, device=self.device)
         g = lambda name: _p(getattr(out, name)) if project else None
         self._check(self.lib.tgs_raster_bwd_sparse(
             self._h, C.byref(cam), N, sh_degree, _p(splats), _p(binned.tile_offsets), _p(binned.gid_sorted), samp.k,
             _p(samp.tiles), _p(samp.tile_pix_offsets), _p(samp.pix), _p(fwd.T), _p(fwd.n_contrib), _p(dL_dcolor),
             _p(means3D), _p(scales), _p(quats), _p(sh), _p(radii), _p(clamped), _p(out.dL_dsplats),
-            g("dL_dmeans3D"), g("dL_dscales"), g("dL_dquats"), g("dL_dopacities"), g("dL_dsh"), _stream(stream)))
+            g("dL_dmeans3D"), g("dL_dscales"), g("dL_dquats"), g("dL_dopacities"), g("dL_dsh"),
+            _p(out.touched) if (sparse and project) else None, _stream(stream)))
         return out

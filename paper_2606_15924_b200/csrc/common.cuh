@@ -128,7 +128,7 @@ cudaError_t launch_raster_stats_lite(const CamK& cam, const float* splats, const
 cudaError_t launch_project_bwd(const CamK& cam, int N, int D, const float* mu, const float* sc, const float* qt,
                                const float* sh, const int32_t* radii, const uint8_t* clamped, const float* splats,
                                const float* dL_dsplats, float* dmu, float* dsc, float* dqt, float* dop,
-                               float* dsh, cudaStream_t s);
+                               float* dsh, int32_t* touched, cudaStream_t s);
 
 cudaError_t launch_sample_paper(const CamK& cam, const uint16_t* E_half, const uint16_t* age, int n_pix, int n_hard,
                                 int n_stable, uint64_t seed, uint32_t* tiles, uint32_t* tpo, uint32_t* pix,

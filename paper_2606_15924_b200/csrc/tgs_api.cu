@@ -278,7 +278,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
                           const uint32_t* n_contrib, const float* dL_dcolor, const float* means3D,
                           const float* scales, const float* quats, const float* sh, const int32_t* radii,
                           const uint8_t* clamped, float* dL_dsplats, float* dL_dmeans3D, float* dL_dscales,
-                          float* dL_dquats, float* dL_dopacities, float* dL_dsh, void* stream) {
+                          float* dL_dquats, float* dL_dopacities, float* dL_dsh, int32_t* touched, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
     if (!on_device(ctx, "tgs_raster_bwd_sparse")) return TGS_ERR_CUDA;
     if (!cam_ok(cam)) return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: bad camera");
@@ -299,7 +299,7 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
         if (((uintptr_t)quats & 15) || ((uintptr_t)dL_dquats & 15) || ((uintptr_t)dL_dsplats & 15))
             return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: quats, dL_dquats, dL_dsplats must be 16-byte aligned");
         e = launch_project_bwd(ck, N, sh_degree, means3D, scales, quats, sh, radii, clamped, splats, dL_dsplats, dL_dmeans3D,
-                               dL_dscales, dL_dquats, dL_dopacities, dL_dsh, s);
+                               dL_dscales, dL_dquats, dL_dopacities, dL_dsh, touched, s);
         if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (projection)", e);
     }
     return TGS_OK;

@@ -35,7 +35,7 @@ class SparseRasterStep:
                                    n_blended=e(npx, i32) if want_walked else None)
         self.bwd = SimpleNamespace(dL_dsplats=e((N, SPLAT_WORDS), f32), dL_dmeans3D=e((N, 3), f32),
                                    dL_dscales=e((N, 3), f32), dL_dquats=e((N, 4), f32), dL_dopacities=e(N, f32),
-                                   dL_dsh=e((N, K, 3), f32))
+                                   dL_dsh=e((N, K, 3), f32), touched=e(N, i32))
         self.ws_sort = e(tgs.bin_sort_workspace_bytes(N, P_capacity, T), u8)
         self.ws_sample = e(tgs.sample_workspace_bytes(self.cam), u8)
         self._side = torch.cuda.Stream(device=dev)
@@ -69,11 +69,12 @@ class SparseRasterStep:
         self._inputs = (means3D, scales, quats, sh)
         return self.fwd
 
-    def backward(self, dL_dcolor, project=True, stream=None):
+    def backward(self, dL_dcolor, project=True, stream=None, sparse=False):
+        """sparse=True: gradients as (touched mask, rows of the touched Gaussians); see tgs.h."""
         means3D, scales, quats, sh = self._inputs
         self.tgs.raster_bwd_sparse(self.cam, self.D, self.pre.splats, self.binned, self.samp, self.fwd, dL_dcolor,
                                    means3D, scales, quats, sh, self.pre.radii, self.pre.clamped, project=project,
-                                   out=self.bwd, stream=stream)
+                                   out=self.bwd, stream=stream, sparse=sparse)
         return self.bwd
 
     def counts(self):

@@ -221,6 +221,48 @@ def test_raster_bwd_parity(name, orc32, orc64, tgs, torch):
     print(name, f"fragile pixels zeroed: {r.n_fragile}", rep)
 
 
+@pytest.mark.parametrize("name", ["small_rot", "small_d2", "cfg2", "clamp_vis"])
+def test_raster_bwd_sparse_gradients(name, orc32, orc64, tgs, torch):
+    """tgs_raster_bwd_sparse with `touched` (tgs.h, sparse gradients): the mask marks exactly the Gaussians with a
+    non-zero raster gradient record; their rows equal the dense call's bit for bit where the raster half is
+    deterministic... it is not (atomics), so they are held to the oracle with the same bars; the rows of all other
+    Gaussians are left unwritten (a canary survives) and are exactly zero in the oracle."""
+    r = oracle_run(name, orc32, orc64)
+    sc = r.sc
+    splats = dev(pack_splats(r.pre), torch)
+    b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
+    fwd = type("F", (), {})()
+    fwd.T = dev(r.fwd.T, torch)
+    fwd.n_contrib = dev(r.fwd.n_contrib.astype(np.int64), torch, torch.int32)
+    d = scene_dev(sc, torch)
+    N, K = sc.N, (sc.sh_degree + 1) ** 2
+    CANARY = 12345.5
+    f = dict(dtype=torch.float32, device="cuda")
+    out = SimpleNamespace(dL_dsplats=torch.empty((N, 12), **f), dL_dmeans3D=torch.full((N, 3), CANARY, **f),
+                          dL_dscales=torch.full((N, 3), CANARY, **f), dL_dquats=torch.full((N, 4), CANARY, **f),
+                          dL_dopacities=torch.full((N,), CANARY, **f), dL_dsh=torch.full((N, K, 3), CANARY, **f),
+                          touched=torch.full((N,), -7, dtype=torch.int32, device="cuda"))
+    tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, b, s, fwd, dev(r.g, torch), d.means3D, d.scales, d.quats, d.sh,
+                          dev(r.pre.radii, torch), dev(r.pre.clamped, torch), out=out, sparse=True)
+    torch.cuda.synchronize()
+    touched = out.touched.cpu().numpy()
+    assert set(np.unique(touched)) <= {0, 1}
+    rec = out.dL_dsplats.cpu().numpy()[:, :9]
+    assert np.array_equal(touched == 1, (rec != 0).any(axis=1) & (r.pre.radii > 0))
+    on = touched == 1
+    assert 0 < on.sum() < N
+    # untouched: nothing written, and the oracle's gradient there is exactly zero
+    for nm in ("dL_dmeans3D", "dL_dscales", "dL_dquats", "dL_dopacities", "dL_dsh"):
+        got = getattr(out, nm).cpu().numpy()
+        assert (got[~on] == CANARY).all(), nm + ": a row of an untouched Gaussian was written"
+        assert (got[on] != CANARY).all(), nm + ": a row of a touched Gaussian was not written"
+        ref = r.rbwd.dL_dopacity if nm == "dL_dopacities" else getattr(r.pbwd, nm)
+        assert not np.asarray(ref)[~on].any(), nm + ": the oracle has a gradient where the mask says none"
+        getattr(out, nm)[torch.from_numpy(~on).cuda()] = 0.0   # then the dense comparison applies to every row
+    rep = check_chain_grads(out, r.pbwd, r.rbwd, r.scale)
+    print(name, f"sparse gradients: {int(on.sum())} of {N} Gaussians touched", rep)
+
+
 @pytest.mark.parametrize("name", SCENES)
 def test_end_to_end_all_gpu(name, orc32, orc64, tgs, torch):
     """preprocess -> bin_sort -> sample -> fwd -> bwd entirely on the GPU, no oracle data in between."""
