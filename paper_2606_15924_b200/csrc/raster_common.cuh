@@ -56,7 +56,14 @@ struct Stage {
     float2 ct[ENTRIES + 4];
     float bl[ENTRIES + 4];
     uint32_t id[ENTRIES + 4];
-    float dz[DEPTH ? ENTRIES + 4 : 4];
+};
+// DEPTH = true (statistics forward, which copies its survivors into a private batch and needs the depth): three
+// float4 planes   p0 = mx, my, -A/2, -B      p1 = -C/2, thr, opacity, red      p2 = green, blue, bits: Gaussian id, depth
+template <int ENTRIES>
+struct Stage<ENTRIES, true> {
+    float4 p0[ENTRIES];
+    float4 p1[ENTRIES];
+    float4 p2[ENTRIES];
 };
 template <int ENTRIES, bool DEPTH = false, int STAGES = 4>
 struct Ring {
@@ -206,15 +213,16 @@ __device__ __forceinline__ void ring_init(RingT& R) {
             mbar_init(&R.empty[s], (uint32_t)kConsumers);
         }
         for (int w = 0; w < kConsumers; ++w) R.done_seq[w] = 0u;
-        for (int s = 0; s < RingT::kStages; ++s) {  // the dummy record of every stage
-            auto& st = R.st[s];
-            constexpr int E = RingT::kEntries;
-            st.p0[E] = make_float4(0.f, 0.f, 0.f, 0.f);
-            st.p1[E] = make_float4(0.f, 0.f, 0.f, 0.f);
-            st.ct[E] = make_float2(0.f, 1.f);
-            st.bl[E] = 0.f;
-            st.id[E] = 0xffffffffu;
-            st.dz[RingT::kDepth ? E : 0] = 0.f;
+        if constexpr (!RingT::kDepth) {
+            for (int s = 0; s < RingT::kStages; ++s) {  // the dummy record of every stage
+                auto& st = R.st[s];
+                constexpr int E = RingT::kEntries;
+                st.p0[E] = make_float4(0.f, 0.f, 0.f, 0.f);
+                st.p1[E] = make_float4(0.f, 0.f, 0.f, 0.f);
+                st.ct[E] = make_float2(0.f, 1.f);
+                st.bl[E] = 0.f;
+                st.id[E] = 0xffffffffu;
+            }
         }
     }
     __syncthreads();
@@ -285,11 +293,15 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                         const int i = h * 64 + j * 32 + lane;
                         const float nC = -0.5f * r1[j].x;
                         st.p0[i] = make_float4(r0[j].x, r0[j].y, -0.5f * r0[j].z, -r0[j].w);
-                        st.p1[i] = make_float4(nC, r1[j].y, r1[j].z, r1[j].w);
-                        st.ct[i] = make_float2(nC, blend_threshold(r1[j].y));
-                        st.bl[i] = r2x[j].x;
-                        st.id[i] = g[j];
-                        if (RingT::kDepth) st.dz[i] = r2x[j].y;
+                        if constexpr (RingT::kDepth) {
+                            st.p1[i] = make_float4(nC, blend_threshold(r1[j].y), r1[j].y, r1[j].z);
+                            st.p2[i] = make_float4(r1[j].w, r2x[j].x, __uint_as_float(g[j]), r2x[j].y);
+                        } else {
+                            st.p1[i] = make_float4(nC, r1[j].y, r1[j].z, r1[j].w);
+                            st.ct[i] = make_float2(nC, blend_threshold(r1[j].y));
+                            st.bl[i] = r2x[j].x;
+                            st.id[i] = g[j];
+                        }
                     }
                 }
             }

@@ -66,7 +66,6 @@ raster_fwd_lite_kernel(const CamK cam, const float4* __restrict__ splats, const 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpBatch& sb = batch[warp];
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const float kNaN = __int_as_float(0x7fc00000);
     for (;;) {
         const uint32_t it = lite_next(sched, lane);
         if (it >= (uint32_t)k) break;
@@ -83,7 +82,8 @@ raster_fwd_lite_kernel(const CamK cam, const float4* __restrict__ splats, const 
             ipy = (int)(id / (uint32_t)cam.W);
         }
         const PixelBox box = warp_pixel_box(active, ipx, ipy);
-        float px = active ? (float)ipx : kNaN;
+        const float px = (float)ipx;
+        bool alive = active;  // sampled and not yet terminated: gates the blend decision only (no loop-carried chain through px)
         const float py = (float)ipy;
         float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
         uint32_t last = 0, walked = len, blended = 0;
@@ -115,7 +115,7 @@ raster_fwd_lite_kernel(const CamK cam, const float4* __restrict__ splats, const 
                 const float dx = a.x - px, dy = a.y - py;
                 const float power = splat_power(a.z, a.w, b.x, dx, dy);
                 const float alpha = fminf(kAlphaMax, __fmul_rn(b.z, ex2_approx(power * kLog2e)));
-                const bool blend = (power <= 0.0f) && !(alpha < kAlphaMin);
+                const bool blend = alive && (power <= 0.0f) && !(alpha < kAlphaMin);
                 const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
                 const bool term = blend && (Tn < kTMin);
                 const bool upd = blend && !term;
@@ -127,9 +127,9 @@ raster_fwd_lite_kernel(const CamK cam, const float4* __restrict__ splats, const 
                     blended += upd ? 1u : 0u;
                     walked = term ? __float_as_uint(b.w) : walked;
                 }
-                px = term ? kNaN : px;
+                alive = alive && !term;
             }
-            if (__all_sync(0xffffffffu, px != px)) break;
+            if (!__any_sync(0xffffffffu, alive)) break;
             cur = nxt;
         }
         if (active) {
@@ -342,7 +342,6 @@ raster_stats_lite_kernel(const CamK cam, const float4* __restrict__ splats, cons
     WarpBatch& sb = sm.batch[warp];
     LiteStatXpose& sx = sm.xpose[warp];
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const float kNaN = __int_as_float(0x7fc00000);
     const int slot2 = lane & (kSlots - 1), half = lane >> 4;
     int m = 0;
 
@@ -388,7 +387,8 @@ raster_stats_lite_kernel(const CamK cam, const float4* __restrict__ splats, cons
             e_p = pix_err[slot];
         }
         const PixelBox box = warp_pixel_box(active, ipx, ipy);
-        float px = active ? (float)ipx : kNaN;
+        const float px = (float)ipx;
+        bool alive = active;  // sampled and not yet terminated: gates the blend decision only (no loop-carried chain through px)
         const float py = (float)ipy;
         float T = 1.0f, zacc = 0.f;
         __syncwarp();
@@ -424,14 +424,14 @@ raster_stats_lite_kernel(const CamK cam, const float4* __restrict__ splats, cons
                     const float dx = a.x - px, dy = a.y - py;
                     const float power = splat_power(a.z, a.w, b.x, dx, dy);
                     const float alpha = fminf(kAlphaMax, __fmul_rn(b.z, ex2_approx(power * kLog2e)));
-                    const bool blend = (power <= 0.0f) && !(alpha < kAlphaMin);
+                    const bool blend = alive && (power <= 0.0f) && !(alpha < kAlphaMin);
                     const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
                     const bool term = blend && (Tn < kTMin);
                     const bool upd = blend && !term;
                     const float w = upd ? alpha * T : 0.0f;
                     zacc = fmaf(w, sa[64 + ii].x, zacc);
                     T = upd ? Tn : T;
-                    px = term ? kNaN : px;
+                    alive = alive && !term;
                     vdst[ii * kTStride] = w;
                 }
                 if (lane < take) {
@@ -442,7 +442,7 @@ raster_stats_lite_kernel(const CamK cam, const float4* __restrict__ splats, cons
                 m += take;
                 if (m == kSlots) flush();
             }
-            if (__all_sync(0xffffffffu, px != px)) break;
+            if (!__any_sync(0xffffffffu, alive)) break;
             cur = nxt;
         }
         if (m > 0) flush();  // before the per-pixel array changes

@@ -36,7 +36,7 @@ using StatRing = Ring<kStatStageEntries, true>;  // with the depth plane
 
 struct StatShared {
     StatRing ring;
-    WarpList<kStatStageEntries> list[kConsumers];
+    WarpBatch batch[kConsumers];
     StatXpose xpose[kConsumers];
 };
 
@@ -55,15 +55,17 @@ raster_stats_kernel(const CamK cam, const float4* __restrict__ splats, const uin
         return;
     }
     StatRing& R = sm.ring;
-    uint32_t* const idx = sm.list[warp].idx;
+    WarpBatch& sb = sm.batch[warp];
     StatXpose& sx = sm.xpose[warp];
     const uint32_t lt_mask = (1u << lane) - 1u;
-    const float kNaN = __int_as_float(0x7fc00000);
     const int slot2 = lane & (kSlots - 1), half = lane >> 4;  // phase-2 role of this lane
 
     UnitInfo ui;
     ui.start = ui.end = ui.slot = 0; ui.active = false;
     PixelBox box = {0.f, 0.f, 0.f, 0.f};
+    const float kNaN = __int_as_float(0x7fc00000);
+    // (a finished or inactive lane carries px = NaN here: the alive flag of the forward kernel costs this kernel a
+    // register it does not have at 3 blocks / SM -- 90 bytes of spills in the inner loop, 0.87 instead of 0.74 ms)
     float px = kNaN, py = 0.f, T = 1.0f, zacc = 0.f;
     bool open = false;
     int m = 0;  // Gaussians pending in the transposed tile
@@ -90,7 +92,7 @@ raster_stats_kernel(const CamK cam, const float4* __restrict__ splats, const uin
         E += __shfl_xor_sync(0xffffffffu, E, 16);
         D += __shfl_xor_sync(0xffffffffu, D, 16);
         Wt += __shfl_xor_sync(0xffffffffu, Wt, 16);
-        if (slot2 < m && half == 0 && __float_as_uint(gb.y) != 0xffffffffu)  // (a padding slot holds the dummy record)
+        if (slot2 < m && half == 0)
             red_add_v4(reinterpret_cast<float4*>(stats) + __float_as_uint(gb.y), E, D, Wt, 0.f);
         m = 0;
         __syncwarp();
@@ -130,53 +132,63 @@ raster_stats_kernel(const CamK cam, const float4* __restrict__ splats, const uin
             }
         }
         if (open) {
+            // (survivors are copied into the warp's private batch, from three float4 planes, as in round 1: the
+            // in-place index list of the forward / backward kernels measured 0.83 instead of 0.74 ms in this kernel)
             const Stage<kStatStageEntries, true>& st = R.st[s];
-            // ---- cull the stage against the pixel box; survivors' indices in range order, padded to a multiple of four ----
-            uint32_t n = 0;
             for (uint32_t b0 = 0; b0 < inf.cnt; b0 += 32) {
+                // ---- cull this batch against the pixel box, compact survivors in range order ----
                 const uint32_t i = b0 + lane;
+                const bool have = i < inf.cnt;
                 const float4 q0 = st.p0[i];
-                const float2 c2 = st.ct[i];
-                const bool pass = i < inf.cnt && splat_may_touch(q0.x, q0.y, q0.z, q0.w, c2.x, c2.y, box);
+                const float4 q1 = st.p1[i];
+                const bool pass = have && splat_may_touch(q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, box);
                 const uint32_t ballot = __ballot_sync(0xffffffffu, pass);
-                if (pass) idx[n + __popc(ballot & lt_mask)] = i;
-                n += __popc(ballot);
-            }
-            if (lane < 3) idx[n + lane] = (uint32_t)kStatStageEntries;
-            n = (n + 3u) & ~3u;
-            __syncwarp();
-            for (uint32_t e = 0; e < n; e += 4) {
-                // ---- phase 1: walk four survivors in place, branch free ----
-                const uint4 j4 = *reinterpret_cast<const uint4*>(idx + e);
-                float* vdst = sx.v + m * kVStride + lane;
-#pragma unroll
-                for (int ii = 0; ii < 4; ++ii) {
-                    const uint32_t i = ii == 0 ? j4.x : (ii == 1 ? j4.y : (ii == 2 ? j4.z : j4.w));
-                    const float4 a = st.p0[i];
-                    const float2 b = *reinterpret_cast<const float2*>(&st.p1[i]);  // -C/2, opacity
-                    const float dx = a.x - px, dy = a.y - py;
-                    const float power = splat_power(a.z, a.w, b.x, dx, dy);
-                    const float alpha = fminf(kAlphaMax, __fmul_rn(b.y, ex2_approx(power * kLog2e)));
-                    const bool blend = (power <= 0.0f) && !(alpha < kAlphaMin);
-                    const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
-                    const bool term = blend && (Tn < kTMin);
-                    const bool upd = blend && !term;
-                    const float w = upd ? alpha * T : 0.0f;
-                    zacc = fmaf(w, st.dz[i], zacc);
-                    T = upd ? Tn : T;
-                    px = term ? kNaN : px;
-                    vdst[ii * kVStride] = w;
+                const int cnt = __popc(ballot);
+                __syncwarp();
+                if (pass) {
+                    const int slot = __popc(ballot & lt_mask);
+                    const float4 q2 = st.p2[i];
+                    sb.a[slot] = q0;
+                    sb.b[slot] = make_float4(q1.x, q1.y, q1.z, 0.f);  // -C/2, thr, opacity
+                    sb.c[slot] = make_float4(q2.w, q2.z, 0.f, 0.f);    // depth, bits: Gaussian id
                 }
-                if (lane < 4) {  // the Gaussians' parameters for phase 2: one parallel copy per group
-                    const uint32_t i = idx[e + lane];
-                    sx.ma[m + lane] = st.p0[i];
-                    sx.mb[m + lane] = make_float2(st.p1[i].x, __uint_as_float(st.id[i]));
+                __syncwarp();
+                int e = 0;
+                while (e < cnt) {
+                    // ---- phase 1: walk the next survivors (as many as fit in the transposed tile), branch free ----
+                    const int take = min(cnt - e, kSlots - m);
+                    const float4* sa = sb.a + e;
+                    float* vdst = sx.v + m * kVStride + lane;
+#pragma unroll 2
+                    for (int ii = 0; ii < take; ++ii) {
+                        const float4 a = sa[ii];
+                        const float4 b = sa[32 + ii];
+                        const float dx = a.x - px, dy = a.y - py;
+                        const float power = splat_power(a.z, a.w, b.x, dx, dy);
+                        const float alpha = fminf(kAlphaMax, __fmul_rn(b.z, ex2_approx(power * kLog2e)));
+                        const bool blend = (power <= 0.0f) && !(alpha < kAlphaMin);
+                        const float Tn = __fmul_rn(T, __fsub_rn(1.0f, alpha));
+                        const bool term = blend && (Tn < kTMin);
+                        const bool upd = blend && !term;
+                        const float w = upd ? alpha * T : 0.0f;
+                        zacc = fmaf(w, sa[64 + ii].x, zacc);
+                        T = upd ? Tn : T;
+                        px = term ? kNaN : px;
+                        vdst[ii * kVStride] = w;
+                    }
+                    if (lane < take) {  // the Gaussians' parameters for phase 2: one parallel copy per group
+                        sx.ma[m + lane] = sa[lane];
+                        sx.mb[m + lane] = make_float2(sa[32 + lane].x, sa[64 + lane].y);
+                    }
+                    e += take;
+                    m += take;
+                    if (m == kSlots) flush();
                 }
-                m += 4;
-                if (m == kSlots) flush();
+                if (__all_sync(0xffffffffu, px != px)) {
+                    finalize();
+                    break;
+                }
             }
-            __syncwarp();  // the list is rewritten at the next stage
-            if (__all_sync(0xffffffffu, px != px)) finalize();
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&R.empty[s]);
