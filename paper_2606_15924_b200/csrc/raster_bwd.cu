@@ -70,7 +70,6 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     float px = 0.f, py = 0.f, g0 = 0.f, g1 = 0.f, g2 = 0.f, bgdot = 0.f;
     float T = 0.f, Sg = 0.f;
     uint32_t last = 0, wmax = 0;
-    PixelBox box = {0.f, 0.f, 0.f, 0.f};
     int m = 0;  // Gaussians pending in the transposed tile
     uint32_t gchunk = 0;
 
@@ -139,7 +138,6 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
                     g0 = dL_dcolor[3 * (size_t)o]; g1 = dL_dcolor[3 * (size_t)o + 1]; g2 = dL_dcolor[3 * (size_t)o + 2];
                 }
                 wmax = __reduce_max_sync(0xffffffffu, last);
-                box = warp_pixel_box(ui.active, ipx, ipy);
                 px = (float)ipx; py = (float)ipy;
                 bgdot = (cam.bg[0] * g0 + cam.bg[1] * g1 + cam.bg[2] * g2) * Tf;
                 T = Tf; Sg = 0.f;
@@ -149,7 +147,11 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         }
         if (wmax > 0) {
             const Stage<kBwdStageEntries>& st = R.st[s];
-            // ---- cull the stage against the pixel box; survivors' indices in range order (descending position) ----
+            // the box of THIS stage: only the pixels whose deepest contributor lies in or in front of it (a record at
+            // position p can only contribute to pixels with n_contrib > p); it grows to the warp's full box towards the front
+            const uint32_t lowpos = inf.base - (inf.cnt - 1u);  // the front-most position staged here
+            const PixelBox box = warp_pixel_box(last > lowpos, (int)px, (int)py);
+            // ---- cull the stage against that box; survivors' indices in range order (descending position) ----
             uint32_t n = 0;
             for (uint32_t b0 = 0; b0 < inf.cnt; b0 += 32) {
                 // records of this batch sit at range positions base-b0 .. base-b0-31 (descending)

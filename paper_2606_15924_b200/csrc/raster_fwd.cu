@@ -105,6 +105,8 @@ raster_fwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
         }
         if (open) {
             const Stage<kFwdStageEntries>& st = R.st[s];
+            // the box shrinks with the pixels that are still alive: a Gaussian that only reaches terminated pixels is culled
+            if (inf.hdr == kHdrCont) box = warp_pixel_box(alive, (int)px, (int)py);
             // ---- cull the stage against the pixel box; survivors' indices in range order ----
             uint32_t n = 0;
             for (uint32_t b0 = 0; b0 < inf.cnt; b0 += 32) {
