@@ -501,6 +501,35 @@ def test_loss_sparse_modes_and_edge_tiles(mode, pct, rate, orc32, orc64, tgs, to
     assert lam_inside
 
 
+def test_loss_sparse_empty_tiles_in_the_list(orc32, orc64, tgs, torch):
+    """A list with EMPTY tiles (m = 0), which the library's samplers never produce but the ABI accepts: an empty tile
+    contributes nothing (tile_stats = 0, no NaN in loss), also as the last tile (no read past the list); the other
+    tiles are unaffected (the oracle skips empty tiles)."""
+    W, H = 96, 64
+    cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
+    rng = np.random.default_rng(33)
+    s = orc32.sample(cam, (100, 100), 1, (1, 2), 4, err=workloads.blob_error_map(rng, W, H, 4))
+    tpo = s.tile_pix_offsets.astype(np.int64)
+    # insert an empty tile after the second tile, and one at the end
+    tpo2 = np.concatenate([tpo[:3], [tpo[2]], tpo[3:], [tpo[-1]]]).astype(np.uint32)
+    s2 = SimpleNamespace(k=s.k + 2, n=s.n, tile_pix_offsets=tpo2, pix=s.pix)
+    target = rng.random((H, W, 3)).astype(np.float32)
+    color = rng.random((s.n, 3)).astype(np.float32)
+    ref = orc64.loss_sparse(cam, s, color, target)          # without the empty tiles
+    samp = SimpleNamespace(k=s2.k, n=s2.n, tile_pix_offsets=dev(tpo2.astype(np.int32), torch), pix=dev(s.pix.astype(np.int32), torch))
+    out = tgs.loss_sparse(cam, samp, dev(color, torch), dev(target, torch))
+    torch.cuda.synchronize()
+    ts = out.tile_stats.cpu().numpy()
+    assert not ts[2].any() and not ts[-1].any()
+    keep = np.ones(s2.k, bool)
+    keep[2] = keep[-1] = False
+    assert np.isfinite(out.loss.cpu().numpy()).all()
+    np.testing.assert_allclose(ts[keep], ref.tile_stats, rtol=2e-4, atol=1e-6)
+    np.testing.assert_allclose(out.loss.cpu().numpy(), ref.loss, rtol=1e-4, atol=1e-7)
+    g = out.dL_dcolor.cpu().numpy()[:s.n]
+    assert np.abs(g - ref.dL_dcolor).max() <= 1e-4 * np.abs(ref.dL_dcolor).max()
+
+
 def test_loss_feeds_the_backward(orc32, orc64, tgs, torch):
     """End of the chain: forward colours -> tgs_loss_sparse -> tgs_raster_bwd_sparse, all on the GPU.  The loss
     kernel's dL/dcolor is held to the loss test's bar against the oracle's O7; the backward is then compared with the

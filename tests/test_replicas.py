@@ -73,3 +73,25 @@ def test_single_process_is_the_identity():
         for k, v in env.items():
             if v is not None:
                 os.environ[k] = v
+
+
+def test_one_view_per_rank_orbits_the_scene():
+    """bench.py hands Replicas.view_seed(0) to workloads.orbit_view: rank 0 keeps the config's own camera, rank r > 0
+    sees the same Gaussians from another seeded direction at the same distance, through the oracle's projection."""
+    import numpy as np
+    import oracle
+    import workloads
+    sc = workloads.make(2)
+    assert workloads.orbit_view(sc, 0) is sc
+    o = oracle.Oracle("f32")
+    seen = []
+    for view in (0, 1, 2):
+        v = workloads.orbit_view(sc, view)
+        R = np.asarray(v.cam.R, np.float64)
+        assert np.allclose(R @ R.T, np.eye(3), atol=1e-6) and abs(np.linalg.det(R) - 1.0) < 1e-6    # a rotation
+        assert np.array_equal(v.cam.t, sc.cam.t) and v.means3D is sc.means3D                      # same distance, same scene
+        pre = o.preprocess(v.cam, v.sh_degree, v.means3D, v.scales, v.quats, v.opacities, v.sh)
+        vis = pre.radii > 0
+        assert vis.mean() > 0.3                                                                   # the cloud stays in view
+        seen.append(vis)
+    assert (seen[0] != seen[1]).any() and (seen[1] != seen[2]).any()                              # different views
