@@ -508,7 +508,7 @@ def test_loss_sparse_empty_tiles_in_the_list(orc32, orc64, tgs, torch):
     W, H = 96, 64
     cam = workloads.Camera(W, H, 100.0, 100.0, W / 2, H / 2, np.eye(3, dtype=np.float32), np.zeros(3, np.float32))
     rng = np.random.default_rng(33)
-    s = orc32.sample(cam, (100, 100), 1, (1, 2), 4, err=workloads.blob_error_map(rng, W, H, 4))
+    s = orc32.sample(cam, (50, 100), 1, (1, 2), 4, err=workloads.blob_error_map(rng, W, H, 4))   # 12 of 24 tiles: k + 2 <= T
     tpo = s.tile_pix_offsets.astype(np.int64)
     # insert an empty tile after the second tile, and one at the end
     tpo2 = np.concatenate([tpo[:3], [tpo[2]], tpo[3:], [tpo[-1]]]).astype(np.uint32)
