@@ -172,6 +172,7 @@ struct UnitInfo {
     uint32_t start, end;  // tile range in gid_sorted
     uint32_t slot;        // this lane's index in the sampled-pixel list (valid if active)
     bool active;
+    bool full;            // the tile lists all 256 pixels: the unit is an 8x4 block, lane j at (j & 7, j >> 3) from lane 0
 };
 
 // (sampled tile `it`, pixel group `gi`).  A full tile (256 pixels) is cut into 8x4-pixel blocks
@@ -184,6 +185,7 @@ __device__ __forceinline__ bool decode_unit(uint32_t it, uint32_t gi, int lane, 
     const uint32_t t = tiles[it];
     ui.start = tile_offsets[t];
     ui.end = tile_offsets[t + 1];
+    ui.full = m == 256u;
     if (m == 256u) {
         const uint32_t local = (((gi >> 1) * 4u + ((uint32_t)lane >> 3)) << 4) + (gi & 1u) * 8u + ((uint32_t)lane & 7u);
         ui.slot = p0 + local;
