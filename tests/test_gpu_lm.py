@@ -201,3 +201,32 @@ def test_lm_solve_follows_the_backward(tgs, torch):
         else:
             _close(got, d_ref[k], 1e-6, "delta " + k, atol=1e-30)
             _close(md[k].cpu().numpy(), m_ref[k], 1e-6, "m " + k, atol=1e-37)
+
+
+def test_lm_solve_full_size_sampled(tgs, torch):
+    """N = 1 M Gaussians, degree 3, V = 3 (the launch configuration bench.py times, a third of its N): the whole call on
+    the GPU, then the oracle on a seeded sample of 20 000 Gaussians (blocks and the SH sweep are per Gaussian, so a sample
+    is a full check of those rows) plus whole-array properties: masked rows untouched, everything finite."""
+    N, D, V, t = 1_000_000, 3, 3, 9
+    grads, m, v, upd = workloads.lm_state(99, N, D, views=V)
+    gd, md, vd = _dev(grads, torch), _dev(m, torch), _dev(v, torch)
+    dd = tgs.lm_solve(D, gd, md, vd, update=torch.from_numpy(upd).cuda(), beta1=B1, beta2=B2, eps=EPS, eta_sh=ETA, t=t)
+    torch.cuda.synchronize()
+    sel = np.sort(np.random.default_rng(5).choice(N, 20_000, replace=False))
+    sub = lambda ps, lead=False: {k: np.ascontiguousarray(a[:, sel] if lead else a[sel]) for k, a in ps.items()}
+    d_ref, m_ref, v_ref, _ = lm.lm_solve(sub(grads, True), sub(m), sub(v), upd[sel], B1, B2, EPS, ETA, t=t)
+    Em, Ev, Ed = _adam_bars(sub(grads, True), sub(m), sub(v), m_ref, v_ref, d_ref, V, t)
+    off = upd == 0
+    for k in KEYS:
+        got, gm, gv = dd[k].cpu().numpy(), md[k].cpu().numpy(), vd[k].cpu().numpy()
+        assert np.isfinite(got).all() and np.isfinite(gm).all() and np.isfinite(gv).all()
+        assert not got[off].any() and np.array_equal(gm[off], m[k][off]) and np.array_equal(gv[off], v[k][off])
+        if k == "sh":
+            _close(got[sel][:, 0], d_ref[k][:, 0], 1e-6, "delta DC", atol=1e-30)
+            _within(got[sel][:, 1:], d_ref[k][:, 1:], Ed, "delta sh (Adam)")
+            _within(gm[sel][:, 1:], m_ref[k][:, 1:], Em, "m sh (Adam)")
+            _within(gv[sel][:, 1:], v_ref[k][:, 1:], Ev, "v sh (Adam)")
+        else:
+            _close(got[sel], d_ref[k], 1e-6, "delta " + k, atol=1e-30)
+            _close(gm[sel], m_ref[k], 1e-6, "m " + k, atol=1e-37)
+            _close(gv[sel], v_ref[k], 1e-6, "v " + k, atol=1e-37)
