@@ -465,7 +465,8 @@ def run_tgs(args):
         for k_, v in H.items():
             D[k_].copy_(v, non_blocking=True)
         g_dev[:n].copy_(g_pin[:n], non_blocking=True)
-        w.full_step()
+        w.fwd()
+        step.backward(g_dev)   # dense gradients: every row is written, every row is copied back
         for k_, v in Hout.items():
             v.copy_(getattr(step.bwd, k_), non_blocking=True)
 
