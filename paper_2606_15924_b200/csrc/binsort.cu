@@ -27,7 +27,9 @@
 //   K6 giant_split    segments above the shared-memory capacity are split by depth: 1024 fine
 //                     buckets (monotone interpolation between the segment's min and max key) merged
 //                     into sub-segments of ~2k elements.
-//   K7 seg_sort       (three launches: <= 2048 / 4096 / 8192 elements) a block sorts a segment in
+//   K7 seg_sort       (three launches: <= 2048 / 4096 / 8192 elements with 256 / 1024 / 1024 threads; four elements
+//                     per thread in the middle class: a segment's latency, not throughput, sets the time when few
+//                     tiles are sampled -- 0.131 -> 0.122 ms at 5 % of config 5's tiles) a block sorts a segment in
 //                     shared memory in ONE distribution step: bucket = monotone interpolation of the
 //                     depth bits between the segment's min and max (about two buckets per element);
 //                     the slot inside a bucket comes from one write-then-check round on a 16-bit
@@ -778,7 +780,7 @@ seg_sort_kernel(const Seg* __restrict__ list, const uint32_t* n_work_ptr, uint32
 }
 
 constexpr int kSmallThreads = 256, kSmallCap = 2048, kSmallNb = 4096;
-constexpr int kMediumThreads = 512, kMediumCap = 4096, kMediumNb = 8192;
+constexpr int kMediumThreads = 1024, kMediumCap = 4096, kMediumNb = 8192;
 constexpr int kLargeThreads = 1024, kLargeCap = 8192, kLargeNb = 8192;
 constexpr size_t kSmallSmem = sizeof(SortSmem<kSmallCap, kSmallNb>);
 constexpr size_t kMediumSmem = sizeof(SortSmem<kMediumCap, kMediumNb>);
@@ -841,7 +843,7 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
     static SmemOptIn opt[3];  // per device
     e = opt[0].ensure((const void*)seg_sort_kernel<kSmallThreads, kSmallCap, kSmallNb, true, 4>, kSmallSmem);
     if (e != cudaSuccess) return e;
-    e = opt[1].ensure((const void*)seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2>, kMediumSmem);
+    e = opt[1].ensure((const void*)seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 1>, kMediumSmem);
     if (e != cudaSuccess) return e;
     e = opt[2].ensure((const void*)seg_sort_kernel<kLargeThreads, kLargeCap, kLargeNb, true, 1>, kLargeSmem);
     if (e != cudaSuccess) return e;
@@ -905,8 +907,8 @@ cudaError_t launch_bin_sort(const CamK& cam, int N, const float* splats_f, const
                 w.large_list, &w.ctr->n_large, &w.ctr->sched_large, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
             count_launches(1);
         }
-        int mb = num_sms * 2 < T ? num_sms * 2 : T;
-        seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 2><<<mb, kMediumThreads, kMediumSmem, a>>>(
+        int mb = num_sms < T ? num_sms : T;
+        seg_sort_kernel<kMediumThreads, kMediumCap, kMediumNb, true, 1><<<mb, kMediumThreads, kMediumSmem, a>>>(
             w.medium_list, &w.ctr->n_medium, &w.ctr->sched_medium, w.pairs, w.tmp, gid_sorted, keys_sorted, P_dev, gid_bits);
         count_launches(1);
         e = cudaEventRecord(side->join, a);
