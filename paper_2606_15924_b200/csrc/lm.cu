@@ -21,7 +21,6 @@ namespace tgs {
 namespace {
 
 constexpr int kLmThreads = 128;
-   // views whose gradients are loaded together
 
 // In-register Cholesky solve of (A + diag(sqrt(vb) + eps)) x = -mb for one SPD system of size D, A = J^T J given
 // as its lower triangle (row major, idx(i, j) = i (i + 1) / 2 + j).  Every loop has constant bounds and is fully
