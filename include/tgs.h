@@ -277,6 +277,10 @@ typedef struct tgs_params {
  *           correction); Eq. 19 right takes m_hat = m/(1-beta1^t), v_hat = v/(1-beta2^t), t >= 1.
  *   update  [N] int32, nullable: a Gaussian with update == 0 keeps its moments and gets Delta = 0 (it received no
  *           gradient; the sparse-Adam convention of Tab. 5).  NULL updates every Gaussian.
+ *   view_touched  [V,N] int32, nullable: the `touched` masks of the V calls of tgs_raster_bwd_sparse (sparse
+ *           gradients).  Where view_touched[v][n] == 0 the gradient of view v for Gaussian n is ZERO and its rows of
+ *           grads are NOT READ (they were left unwritten); a Gaussian touched in no view is treated like
+ *           update[n] == 0.  NULL: every row of grads is read.
  *   delta   nullable: receives Delta in the parameter layouts.
  *   params  nullable: Alg. 1 step 10, params <- params + Delta in place.  At least one of delta / params.
  * Arithmetic: fp32 storage.  For the two LM blocks the moment sums, J^T J and the Cholesky factorisation /
@@ -287,7 +291,7 @@ typedef struct tgs_params {
  * Two kernels (geometry arrays; sh + opacity arrays), no workspace, no synchronisation; V <= 64.  All sh pointers
  * 16-byte aligned. */
 int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update,
-                 float beta1, float beta2, float eps, float eta_sh, int t,
+                 const int32_t* view_touched, float beta1, float beta2, float eps, float eta_sh, int t,
                  const tgs_params* m, const tgs_params* v, const tgs_params* delta, const tgs_params* params,
                  void* stream);
 

@@ -26,6 +26,9 @@ Readings (R30-R35; the paper leaves these open):
   R34  `update` (nullable mask): a Gaussian with update == 0 received no gradient this iteration; its moments
        are left unchanged and its Delta is 0 (the sparse-Adam convention of Tab. 5).
   R35  Alg. 1 step 10 G <- G + Delta G is `apply`.
+  R36  `view_touched` (nullable [V, N] mask): view i's gradient of Gaussian n counts as ZERO where the mask is 0 (the
+       sparse raster backward left those rows unwritten, whatever they hold); a Gaussian touched in no view is
+       treated like update == 0.  Pure input handling: the arithmetic after it is unchanged.
 Layouts mirror the parameters: a "parameter set" is a dict with keys means3D [N,3], scales [N,3], quats [N,4],
 opacities [N], sh [N,K,3]; gradients carry a leading view axis [V, ...]; moments m / v are parameter sets, the
 moments of the RGB DC live in sh[:, 0, :].
@@ -107,7 +110,8 @@ def _unblock(out, x: np.ndarray, geometry: bool) -> None:
         out["opacities"][...] = x[:, 3]
 
 
-def lm_solve(grads, m, v, update=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=2.5e-3 / 20.0, t=1, params=None):
+def lm_solve(grads, m, v, update=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=2.5e-3 / 20.0, t=1, params=None,
+             view_touched=None):
     """One call of Alg. 1 step 9 (and step 10 when `params` is given).
 
     grads: parameter set with a leading view axis [V, N, ...]; m, v: parameter sets [N, ...] (not modified).
@@ -117,6 +121,13 @@ def lm_solve(grads, m, v, update=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=
     v0 = {k: np.asarray(v[k], np.float64) for k in KEYS}
     V, N = g["opacities"].shape
     upd = np.ones(N, bool) if update is None else (np.asarray(update) != 0)
+    if view_touched is not None:                            # R36
+        vt = np.asarray(view_touched) != 0
+        assert vt.shape == (V, N)
+        for k in KEYS:
+            mask = vt.reshape(vt.shape + (1,) * (g[k].ndim - 2))
+            g[k] = np.where(mask, g[k], 0.0)
+        upd = upd & vt.any(axis=0)
     m1 = {k: m0[k].copy() for k in KEYS}
     v1 = {k: v0[k].copy() for k in KEYS}
     delta = {k: np.zeros_like(m0[k]) for k in KEYS}

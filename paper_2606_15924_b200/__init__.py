@@ -5,7 +5,7 @@ this package is its thin Python binding.  There is no CPU fallback.
 """
 from .binding import (Camera, LIB_PATH, PIXELS_ALL, PIXELS_BERNOULLI_ERR, SPLAT_WORDS, SYMBOLS, TGS, TgsError,
                       load_library)
-from .pipeline import SparseRasterStep
+from .pipeline import SparseIteration, SparseRasterStep
 
 __all__ = ["Camera", "LIB_PATH", "PIXELS_ALL", "PIXELS_BERNOULLI_ERR", "SPLAT_WORDS", "SYMBOLS", "TGS", "TgsError",
-           "load_library", "SparseRasterStep"]
+           "load_library", "SparseIteration", "SparseRasterStep"]

@@ -114,7 +114,7 @@ def load_library() -> C.CDLL:
                                      C.c_size_t, vp]
     lib.tgs_maps_update.argtypes = [vp, cam, vp, vp, vp, vp, vp, f32, vp]
     ps = C.POINTER(Params)
-    lib.tgs_lm_solve.argtypes = [vp, i32, i32, i32, ps, vp, f32, f32, f32, f32, i32, ps, ps, ps, ps, vp]
+    lib.tgs_lm_solve.argtypes = [vp, i32, i32, i32, ps, vp, vp, f32, f32, f32, f32, i32, ps, ps, ps, ps, vp]
     return lib
 
 
@@ -326,9 +326,10 @@ class TGS:
         return out
 
     # ---- f4: moment-damped LM solve (Alg. 1 steps 9-10) ----
-    def lm_solve(self, sh_degree, grads, m, v, update=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, t=1,
+    def lm_solve(self, sh_degree, grads, m, v, update=None, view_touched=None, beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, t=1,
                  want_delta=True, delta=None, params=None, stream=None):
         """grads: parameter set with a leading view axis [V,N,...]; m, v (and params, if given) are updated in place.
+        view_touched: [V,N] int32, the `touched` masks of the V backward calls (rows of grads are read only where set).
         Returns the delta parameter set (allocated here unless given; None if want_delta is False)."""
         V, N = grads["opacities"].shape
         if delta is None and want_delta:
@@ -336,7 +337,7 @@ class TGS:
         pg, pm, pv = Params.of(grads), Params.of(m), Params.of(v)
         pd = Params.of(delta) if delta is not None else None
         pp = Params.of(params) if params is not None else None
-        self._check(self.lib.tgs_lm_solve(self._h, N, sh_degree, V, C.byref(pg), _p(update), beta1, beta2, eps, eta_sh, int(t),
+        self._check(self.lib.tgs_lm_solve(self._h, N, sh_degree, V, C.byref(pg), _p(update), _p(view_touched), beta1, beta2, eps, eta_sh, int(t),
                                           C.byref(pm), C.byref(pv), C.byref(pd) if pd is not None else None,
                                           C.byref(pp) if pp is not None else None, _stream(stream)))
         return delta

@@ -152,7 +152,8 @@ struct LmSet {
 
 struct LmArgs {
     LmSet g, m, v, d, p;   // g: [V, N, ...] read only; d / p nullable as a whole (d.mu == nullptr, p.mu == nullptr)
-    const int32_t* update; // nullable
+    const int32_t* update; // nullable [N]
+    const int32_t* vt;     // nullable [V, N]: per-view touched masks; a view's gradient rows are read only where set
     int N, K, V;
     double b1, b2, eps;    // Eq. 14
     double inv_bc1, inv_bc2;  // 1 / (1 - beta^t), Eq. 19 right
@@ -161,5 +162,16 @@ struct LmArgs {
 };
 
 cudaError_t launch_lm_solve(const LmArgs& a, cudaStream_t s);
+
+// Which views touch Gaussian n (bit v; all ones without per-view masks), 0 if the call does not update it at all:
+// update[n] == 0, or touched in no view.  All mask words are loaded before any gradient (one latency, not one per view).
+template <bool VT>
+__device__ __forceinline__ unsigned long long lm_views(const LmArgs& a, int n) {
+    if (a.update != nullptr && __ldg(a.update + n) == 0) return 0ull;
+    if (!VT) return ~0ull;
+    unsigned long long bits = 0ull;
+    for (int vw = 0; vw < a.V; ++vw) bits |= (unsigned long long)(__ldg(a.vt + (size_t)vw * a.N + n) != 0) << vw;
+    return bits;
+}
 
 }  // namespace tgs

@@ -64,8 +64,8 @@ __device__ __forceinline__ void chol_solve(double (&A)[D * (D + 1) / 2], const d
 
 // One LM block of one Gaussian.  off[c] / ptr selection is done by the caller through the small accessor below:
 // element c of the block lives at base(c)[n * stride(c) + sub(c)] of a parameter set.
-template <int D, int kViewBatch, class Acc>
-__device__ __forceinline__ void lm_block(const LmArgs& a, const Acc acc, int n) {
+template <int D, int kViewBatch, bool VT, class Acc>
+__device__ __forceinline__ void lm_block(const LmArgs& a, const Acc acc, int n, unsigned long long views) {
     double A[D * (D + 1) / 2];
     double gb[D];
 #pragma unroll
@@ -86,7 +86,8 @@ __device__ __forceinline__ void lm_block(const LmArgs& a, const Acc acc, int n) 
         for (int u = 0; u < kViewBatch; ++u)
 #pragma unroll
             for (int c = 0; c < D; ++c)
-                gf[u][c] = vw0 + u < a.V ? __ldg(acc.view(a.g, c, vw0 + u, a.N) + acc.off(c, n)) : 0.f;
+                gf[u][c] = (vw0 + u < a.V && (!VT || ((views >> (vw0 + u)) & 1ull)))
+                               ? __ldg(acc.view(a.g, c, vw0 + u, a.N) + acc.off(c, n)) : 0.f;
 #pragma unroll
         for (int u = 0; u < kViewBatch; ++u) {
             if (vw0 + u >= a.V) break;
@@ -153,7 +154,7 @@ __device__ __forceinline__ float comp(const float& q, int) { return q; }
 __device__ __forceinline__ float& comp(float4& q, int i) { return i == 0 ? q.x : (i == 1 ? q.y : (i == 2 ? q.z : q.w)); }
 __device__ __forceinline__ float& comp(float& q, int) { return q; }
 
-template <int VEC, int kViewBatch, int kSpanBatch, int MINB>
+template <int VEC, int kViewBatch, int kSpanBatch, int MINB, bool VT>
 __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArgs a) {
     using T = typename Vec<VEC>::T;
     const int n = blockIdx.x * kLmThreads + threadIdx.x;
@@ -167,6 +168,7 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArg
             size_t e[kSpanBatch];
             bool ok[kSpanBatch], on[kSpanBatch];
             int r[kSpanBatch];
+            unsigned long long views[kSpanBatch];
             T m4[kSpanBatch], v4[kSpanBatch];
             float gs[kSpanBatch][VEC];
 #pragma unroll
@@ -176,7 +178,8 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArg
                 ok[u] = j < per_block && e[u] < total;
                 const int gn = ok[u] ? (int)(e[u] / row) : 0;
                 r[u] = (int)(e[u] - (size_t)gn * row);   // first element's position inside the Gaussian's row
-                on[u] = ok[u] && (a.update == nullptr || __ldg(a.update + gn) != 0);
+                views[u] = ok[u] ? lm_views<VT>(a, gn) : 0ull;
+                on[u] = views[u] != 0ull;
                 if (VEC == 1 && r[u] < 3) on[u] = ok[u] = false;   // DC band: appearance block
 #pragma unroll
                 for (int i = 0; i < VEC; ++i) gs[u][i] = 0.f;
@@ -193,7 +196,10 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArg
                 for (int w = 0; w < kViewBatch; ++w)
 #pragma unroll
                     for (int u = 0; u < kSpanBatch; ++u)
-                        if (on[u] && vw0 + w < a.V) g4[w][u] = __ldg(reinterpret_cast<const T*>(a.g.sh + (size_t)(vw0 + w) * total + e[u]));
+                        if (on[u] && vw0 + w < a.V && (!VT || ((views[u] >> (vw0 + w)) & 1ull)))
+                            g4[w][u] = __ldg(reinterpret_cast<const T*>(a.g.sh + (size_t)(vw0 + w) * total + e[u]));
+                        else if (VT)
+                            g4[w][u] = T{};
 #pragma unroll
                 for (int w = 0; w < kViewBatch; ++w)
 #pragma unroll
@@ -238,7 +244,8 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArg
     }
     // ---- the appearance block of Gaussian n (Eq. 14): RGB DC + opacity ----
     if (n >= a.N) return;
-    if (a.update != nullptr && __ldg(a.update + n) == 0) {
+    const unsigned long long nviews = lm_views<VT>(a, n);
+    if (nviews == 0ull) {
         if (a.d.mu) {
             const AppAcc aa{a.K};
 #pragma unroll
@@ -246,16 +253,17 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_app_sh_kernel(const LmArg
         }
         return;
     }
-    lm_block<4, kViewBatch>(a, AppAcc{a.K}, n);
+    lm_block<4, kViewBatch, VT>(a, AppAcc{a.K}, n, nviews);
 }
 
 // The geometry block (position, scale, rotation) of Eq. 14: one thread per Gaussian, the 55 entries of the lower
 // triangle in fp64 registers.  Touches means3D / scales / quats only, so it runs beside lm_app_sh_kernel.
-template <int kViewBatch, int MINB>
+template <int kViewBatch, int MINB, bool VT>
 __global__ void __launch_bounds__(kLmThreads, MINB) lm_geo_kernel(const LmArgs a) {
     const int n = blockIdx.x * kLmThreads + threadIdx.x;
     if (n >= a.N) return;
-    if (a.update != nullptr && __ldg(a.update + n) == 0) {
+    const unsigned long long nviews = lm_views<VT>(a, n);
+    if (nviews == 0ull) {
         if (a.d.mu) {
             const GeoAcc ga;
 #pragma unroll
@@ -263,7 +271,7 @@ __global__ void __launch_bounds__(kLmThreads, MINB) lm_geo_kernel(const LmArgs a
         }
         return;
     }
-    lm_block<10, kViewBatch>(a, GeoAcc(), n);
+    lm_block<10, kViewBatch, VT>(a, GeoAcc(), n, nviews);
 }
 
 }  // namespace
@@ -273,9 +281,16 @@ cudaError_t launch_lm_solve(const LmArgs& a, cudaStream_t s) {
     const int blocks = (a.N + kLmThreads - 1) / kLmThreads;
     // batching measured on B200 at N = 3 M, V = 3 (profiles/r2_lm.md): geometry 4 views per batch at 2 blocks / SM
     // (248 registers), SH sweep 4 pieces of the span per thread, one view at a time (109 registers, 4 blocks / SM)
-    lm_geo_kernel<4, 2><<<blocks, kLmThreads, 0, s>>>(a);
-    if ((a.K * 3) % 4 == 0) lm_app_sh_kernel<4, 1, 4, 1><<<blocks, kLmThreads, 0, s>>>(a);
-    else lm_app_sh_kernel<1, 1, 4, 1><<<blocks, kLmThreads, 0, s>>>(a);
+    // (the per-view masks are a template flag: with them as a run-time test the unmasked call ran 40 % slower)
+    if (a.vt) {
+        lm_geo_kernel<4, 2, true><<<blocks, kLmThreads, 0, s>>>(a);
+        if ((a.K * 3) % 4 == 0) lm_app_sh_kernel<4, 1, 4, 1, true><<<blocks, kLmThreads, 0, s>>>(a);
+        else lm_app_sh_kernel<1, 1, 4, 1, true><<<blocks, kLmThreads, 0, s>>>(a);
+    } else {
+        lm_geo_kernel<4, 2, false><<<blocks, kLmThreads, 0, s>>>(a);
+        if ((a.K * 3) % 4 == 0) lm_app_sh_kernel<4, 1, 4, 1, false><<<blocks, kLmThreads, 0, s>>>(a);
+        else lm_app_sh_kernel<1, 1, 4, 1, false><<<blocks, kLmThreads, 0, s>>>(a);
+    }
     count_launches(2);
     return cudaGetLastError();
 }

@@ -380,7 +380,8 @@ int tgs_maps_update(tgs_ctx* ctx, const tgs_camera* cam, uint16_t* E_half, uint1
     return TGS_OK;
 }
 
-int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update, float beta1,
+int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* grads, const int32_t* update,
+                 const int32_t* view_touched, float beta1,
                  float beta2, float eps, float eta_sh, int t, const tgs_params* m, const tgs_params* v,
                  const tgs_params* delta, const tgs_params* params, void* stream) {
     if (!ctx) return TGS_ERR_INVALID_ARG;
@@ -404,6 +405,7 @@ int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* gr
         *dst[i] = LmSet{q->means3D, q->scales, q->quats, q->opacities, q->sh};
     }
     a.update = update;
+    a.vt = view_touched;
     a.N = N; a.K = (sh_degree + 1) * (sh_degree + 1); a.V = V;
     a.b1 = (double)beta1; a.b2 = (double)beta2; a.eps = (double)eps;
     // bias corrections of Eq. 19 (right) are scalars of the call, formed in double on the host

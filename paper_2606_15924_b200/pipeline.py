@@ -42,10 +42,15 @@ class SparseRasterStep:
         self._ev_fork, self._ev_join = torch.cuda.Event(), torch.cuda.Event()
 
     def forward(self, means3D, scales, quats, opacities, sh, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0,
-                err=None, render=None, target=None, stream=None, restrict=True):
+                err=None, render=None, target=None, stream=None, restrict=True, cam=None):
         """restrict=True: sample first and bin only the selected tiles (tgs_bin_sort's tile_select;
-        DESIGN.md R14).  restrict=False: bin every tile, then sample (the call order of north_star)."""
+        DESIGN.md R14).  restrict=False: bin every tile, then sample (the call order of north_star).
+        cam: another view of the same image size (the buffers are sized by the image, not by the pose)."""
         t = self.tgs
+        if cam is not None:
+            cam = Camera.of(cam)
+            assert (cam.width, cam.height) == (self.cam.width, self.cam.height), "a step's views share the image size"
+            self.cam = cam
         if restrict:
             # projection and sampling do not depend on each other: the sampler runs on a side stream (fork / join by
             # events, also under graph capture) while the projection runs on the caller's stream
@@ -69,13 +74,15 @@ class SparseRasterStep:
         self._inputs = (means3D, scales, quats, sh)
         return self.fwd
 
-    def backward(self, dL_dcolor, project=True, stream=None, sparse=False):
-        """sparse=True: gradients as (touched mask, rows of the touched Gaussians); see tgs.h."""
+    def backward(self, dL_dcolor, project=True, stream=None, sparse=False, out=None):
+        """sparse=True: gradients as (touched mask, rows of the touched Gaussians); see tgs.h.
+        out: where the gradients go (default: the step's own buffers), e.g. one view's slices of [V, N, ...] buffers."""
         means3D, scales, quats, sh = self._inputs
+        out = out if out is not None else self.bwd
         self.tgs.raster_bwd_sparse(self.cam, self.D, self.pre.splats, self.binned, self.samp, self.fwd, dL_dcolor,
                                    means3D, scales, quats, sh, self.pre.radii, self.pre.clamped, project=project,
-                                   out=self.bwd, stream=stream, sparse=sparse)
-        return self.bwd
+                                   out=out, stream=stream, sparse=sparse)
+        return out
 
     def counts(self):
         """(P, k, n) -- synchronises."""
@@ -85,3 +92,43 @@ class SparseRasterStep:
             raise RuntimeError(f"P = {P} exceeds P_capacity = {self.P_capacity}")
         self.binned.P, self.samp.k, self.samp.n = P, k, n
         return P, k, n
+
+
+class SparseIteration:
+    """Alg. 1 steps 3-10 for the V views of one iteration, all on the device: per view the five-call
+    step, the fused sparse loss and the sparse backward -- its gradients written view-major into [V, N, ...] buffers
+    with one `touched` mask per view -- then ONE tgs_lm_solve over the V views that updates the moments and the
+    parameters in place.  Host logic only: buffer ownership and call order; nothing synchronises."""
+
+    def __init__(self, tgs: TGS, cams, N: int, sh_degree: int, P_capacity: int):
+        self.tgs, self.cams, self.N, self.D = tgs, [Camera.of(c) for c in cams], int(N), int(sh_degree)
+        V, K, dev = len(self.cams), (sh_degree + 1) ** 2, tgs.device
+        self.step = SparseRasterStep(tgs, self.cams[0], N, sh_degree, P_capacity)
+        f = dict(dtype=torch.float32, device=dev)
+        self.grads = {"means3D": torch.empty((V, N, 3), **f), "scales": torch.empty((V, N, 3), **f),
+                      "quats": torch.empty((V, N, 4), **f), "opacities": torch.empty((V, N), **f),
+                      "sh": torch.empty((V, N, K, 3), **f)}
+        self.touched = torch.empty((V, N), dtype=torch.int32, device=dev)
+        g = self.grads
+        self.views = [SimpleNamespace(dL_dsplats=self.step.bwd.dL_dsplats, dL_dmeans3D=g["means3D"][i],
+                                      dL_dscales=g["scales"][i], dL_dquats=g["quats"][i], dL_dopacities=g["opacities"][i],
+                                      dL_dsh=g["sh"][i], touched=self.touched[i]) for i in range(V)]
+        self.losses = [None] * V
+
+    def run(self, params, targets, errs, m, v, t, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, beta1=0.9, beta2=0.999,
+            eps=1e-8, eta_sh=1.25e-4, stream=None):
+        """params, m, v: parameter sets (dicts of device tensors), updated in place; targets[i]: [H, W, 3] image of view
+        i; errs[i]: [H, W] error map that drives view i's sampling.  Returns the per-view loss namespaces."""
+        st, tg = self.step, self.tgs
+        for i, cam in enumerate(self.cams):
+            fw = st.forward(params["means3D"], params["scales"], params["quats"], params["opacities"], params["sh"],
+                            tile_pct, pixel_mode, pix_rate, seed + i, err=errs[i], stream=stream, cam=cam)
+            samp = SimpleNamespace(k=tg.sample_num_tiles(cam, tile_pct[0], tile_pct[1]), n=None,
+                                   tile_pix_offsets=st.samp.tile_pix_offsets, pix=st.samp.pix)
+            lo = tg.loss_sparse(cam, samp, fw.color, targets[i], out=self.losses[i], stream=stream)
+            self.losses[i] = lo
+            st.samp.k = samp.k
+            st.backward(lo.dL_dcolor, sparse=True, out=self.views[i], stream=stream)
+        tg.lm_solve(self.D, self.grads, m, v, view_touched=self.touched, beta1=beta1, beta2=beta2, eps=eps, eta_sh=eta_sh,
+                    t=t, want_delta=False, params=params, stream=stream)
+        return self.losses

@@ -10,6 +10,8 @@ and Delta = -eta m_hat / (sqrt(v_hat) + eps) carries those two errors to first o
 (IEEE fp32 sqrt and division, the two bias-correction factors rounded to fp32).
 Masked Gaussians: exactly zero / exactly unchanged.
 """
+from types import SimpleNamespace
+
 import numpy as np
 import pytest
 
@@ -230,3 +232,94 @@ def test_lm_solve_full_size_sampled(tgs, torch):
             _close(got[sel], d_ref[k], 1e-6, "delta " + k, atol=1e-30)
             _close(gm[sel], m_ref[k], 1e-6, "m " + k, atol=1e-37)
             _close(gv[sel], v_ref[k], 1e-6, "v " + k, atol=1e-37)
+
+
+@pytest.mark.parametrize("D,V", [(3, 3), (2, 5), (0, 2)])
+def test_lm_solve_per_view_masks(tgs, torch, D, V):
+    """view_touched [V, N] (tgs.h): rows of a view's gradient are read only where its mask is set -- NaN sits in every
+    masked row here, and a Gaussian touched in no view keeps its moments (oracle R36)."""
+    n = 2000 + 13 * D
+    grads, m, v, _ = workloads.lm_state(80 + D, n, D, views=V, p_update=1.0)
+    rng = np.random.default_rng(81)
+    vt = (rng.random((V, n)) < 0.5).astype(np.int32)
+    vt[:, :7] = 0
+    garbage = {k: np.where(vt.reshape(vt.shape + (1,) * (a.ndim - 2)) != 0, a, np.nan).astype(np.float32) for k, a in grads.items()}
+    d_ref, m_ref, v_ref, _ = lm.lm_solve(garbage, m, v, None, B1, B2, EPS, ETA, t=6, view_touched=vt)
+    zeroed = {k: np.nan_to_num(a, nan=0.0) for k, a in garbage.items()}
+    gd, md, vd = _dev(garbage, torch), _dev(m, torch), _dev(v, torch)
+    dd = tgs.lm_solve(D, gd, md, vd, view_touched=torch.from_numpy(vt).cuda(), beta1=B1, beta2=B2, eps=EPS, eta_sh=ETA, t=6)
+    torch.cuda.synchronize()
+    off = ~(vt.any(0))
+    assert off[:7].all()
+    for k in KEYS:
+        got, gm, gv = dd[k].cpu().numpy(), md[k].cpu().numpy(), vd[k].cpu().numpy()
+        assert np.isfinite(got).all() and np.isfinite(gm).all() and np.isfinite(gv).all(), k + ": a masked row was read"
+        assert not got[off].any() and np.array_equal(gm[off], m[k][off]) and np.array_equal(gv[off], v[k][off])
+        if k == "sh":
+            _close(got[:, 0], d_ref[k][:, 0], 1e-6, "delta DC", atol=1e-30)
+            if got.shape[1] > 1:
+                Em, Ev, Ed = _adam_bars(zeroed, m, v, m_ref, v_ref, d_ref, V, 6)
+                _within(got[:, 1:], d_ref[k][:, 1:], Ed, "delta sh (Adam)")
+                _within(gm[:, 1:], m_ref[k][:, 1:], Em, "m sh (Adam)")
+        else:
+            _close(got, d_ref[k], 1e-6, "delta " + k, atol=1e-30)
+            _close(gm, m_ref[k], 1e-6, "m " + k, atol=1e-37)
+            _close(gv, v_ref[k], 1e-6, "v " + k, atol=1e-37)
+
+
+def test_sparse_iteration_equals_its_calls(tgs, torch):
+    """pipeline.SparseIteration (Alg. 1 steps 3-10 for V views: step, loss, sparse backward into view-major slices, one
+    tgs_lm_solve with the per-view touched masks) against the same calls made one by one with DENSE gradients and an
+    explicit update mask.  Every call has its own oracle parity test; this one holds the plumbing: camera per view,
+    slices, masks, in-place parameter update.  (Atomics reorder the gradient sums from run to run: 1e-4.)"""
+    import paper_2606_15924_b200 as pk
+    from helpers import dev, scene_dev
+    V, D = 3, 3
+    sc = workloads.small_random_scene(7, 3000, 200, 136, sh_degree=D, bg=(0.1, 0.3, 0.2), spread=1.3, log_scale=(-2.8, 0.6))
+    cams = [workloads.orbit_view(sc, i).cam for i in range(V)]
+    N, W, H = sc.N, sc.cam.width, sc.cam.height
+    rng = np.random.default_rng(17)
+    targets = [dev(rng.random((H, W, 3)).astype(np.float32), torch) for _ in range(V)]
+    errs = [dev(workloads.blob_error_map(rng, W, H, 6), torch) for _ in range(V)]
+    _, m_np, v_np, _ = workloads.lm_state(71, N, D, views=1)
+    d = scene_dev(sc, torch)
+    base = {"means3D": d.means3D, "scales": d.scales, "quats": d.quats, "opacities": d.opacities, "sh": d.sh}
+    clone = lambda ps: {k: a.clone() for k, a in ps.items()}
+    P_cap = 200_000
+
+    it = pk.SparseIteration(tgs, cams, N, D, P_cap)
+    p1, m1, v1 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
+    it.run(p1, targets, errs, m1, v1, t=3, tile_pct=(50, 100), pixel_mode=pk.PIXELS_ALL, seed=5)
+    torch.cuda.synchronize()
+    touched = it.touched.cpu().numpy()
+    assert set(np.unique(touched)) <= {0, 1} and 0 < touched.sum() < touched.size
+
+    # the same iteration, call by call, dense gradients
+    step = pk.SparseRasterStep(tgs, cams[0], N, D, P_cap)
+    K = (D + 1) ** 2
+    G = {"means3D": torch.zeros((V, N, 3), device="cuda"), "scales": torch.zeros((V, N, 3), device="cuda"),
+         "quats": torch.zeros((V, N, 4), device="cuda"), "opacities": torch.zeros((V, N), device="cuda"),
+         "sh": torch.zeros((V, N, K, 3), device="cuda")}
+    for i, cam in enumerate(cams):
+        fw = step.forward(base["means3D"], base["scales"], base["quats"], base["opacities"], base["sh"], (50, 100),
+                          pk.PIXELS_ALL, (1, 1), 5 + i, err=errs[i], cam=cam)
+        samp = SimpleNamespace(k=step.samp.k, n=None, tile_pix_offsets=step.samp.tile_pix_offsets, pix=step.samp.pix)
+        lo = tgs.loss_sparse(cam, samp, fw.color, targets[i])
+        bw = step.backward(lo.dL_dcolor)
+        G["means3D"][i], G["scales"][i], G["quats"][i] = bw.dL_dmeans3D, bw.dL_dscales, bw.dL_dquats
+        G["opacities"][i], G["sh"][i] = bw.dL_dopacities, bw.dL_dsh
+        rec = bw.dL_dsplats.cpu().numpy()[:, :9]
+        assert np.array_equal(touched[i] == 1, (rec != 0).any(axis=1)), "touched mask of view %d" % i
+    p2, m2, v2 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
+    upd = torch.from_numpy(touched.any(0).astype(np.int32)).cuda()
+    tgs.lm_solve(D, G, m2, v2, update=upd, t=3, want_delta=False, params=p2)
+    torch.cuda.synchronize()
+    moved = 0
+    for k in KEYS:
+        a, b, b0 = p1[k].cpu().numpy().astype(np.float64), p2[k].cpu().numpy().astype(np.float64), base[k].cpu().numpy()
+        step_size = np.abs(b - b0)
+        assert np.abs(a - b).max() <= 1e-4 * step_size.max() + 1e-7, (k, np.abs(a - b).max(), step_size.max())
+        assert np.array_equal(a[upd.cpu().numpy() == 0], b0[upd.cpu().numpy() == 0])     # untouched Gaussians do not move
+        np.testing.assert_allclose(m1[k].cpu().numpy(), m2[k].cpu().numpy(), rtol=1e-3, atol=1e-9)
+        moved += int((step_size > 0).sum())
+    assert moved > 1000

@@ -208,3 +208,19 @@ def test_sh_degree_0_has_no_adam_branch():
     grads, m, v, upd = workloads.lm_state(4, 8, 0, views=2)
     d, m1, v1, _ = lm.lm_solve(grads, m, v, None, B1, B2, EPS, ETA, t=1)
     assert d["sh"].shape == (8, 1, 3) and np.all(np.isfinite(d["sh"]))
+
+
+def test_view_touched_is_zeroed_rows():
+    """R36: per-view masks are the same as zero gradient rows (whatever the masked rows hold) and a Gaussian touched in no
+    view keeps its moments."""
+    grads, m, v, upd = workloads.lm_state(7, 50, 2, views=3, p_update=1.0)
+    rng = np.random.default_rng(8)
+    vt = (rng.random((3, 50)) < 0.6).astype(np.int32)
+    vt[:, 0] = 0                                            # touched in no view
+    zeroed = {k: np.where(vt.reshape(vt.shape + (1,) * (a.ndim - 2)) != 0, a, 0.0).astype(np.float32) for k, a in grads.items()}
+    garbage = {k: np.where(vt.reshape(vt.shape + (1,) * (a.ndim - 2)) != 0, a, np.nan).astype(np.float32) for k, a in grads.items()}
+    d0, m0, v0, _ = lm.lm_solve(zeroed, m, v, vt.any(0).astype(np.int32), B1, B2, EPS, ETA, t=2)
+    d1, m1, v1, _ = lm.lm_solve(garbage, m, v, None, B1, B2, EPS, ETA, t=2, view_touched=vt)
+    for k in lm.KEYS:
+        assert np.array_equal(d0[k], d1[k]) and np.array_equal(m0[k], m1[k]) and np.array_equal(v0[k], v1[k])
+        assert not d1[k][0].any() and np.array_equal(m1[k][0], np.asarray(m[k], np.float64)[0])
