@@ -296,8 +296,10 @@ int tgs_raster_bwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, int sh_deg
     if (dL_dmeans3D) {
         if (!dL_dscales || !dL_dquats || !dL_dopacities || !dL_dsh || !means3D || !scales || !quats || !sh || !radii || !clamped)
             return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: null pointer (projection half)");
-        if (((uintptr_t)quats & 15) || ((uintptr_t)dL_dquats & 15) || ((uintptr_t)dL_dsplats & 15))
-            return fail(ctx, TGS_ERR_INVALID_ARG, "tgs_raster_bwd_sparse: quats, dL_dquats, dL_dsplats must be 16-byte aligned");
+        if (((uintptr_t)quats & 15) || ((uintptr_t)dL_dquats & 15) || ((uintptr_t)dL_dsplats & 15) || ((uintptr_t)sh & 15) ||
+            ((uintptr_t)dL_dsh & 15))
+            return fail(ctx, TGS_ERR_INVALID_ARG,
+                        "tgs_raster_bwd_sparse: quats, sh, dL_dquats, dL_dsh, dL_dsplats must be 16-byte aligned");
         e = launch_project_bwd(ck, N, sh_degree, means3D, scales, quats, sh, radii, clamped, splats, dL_dsplats, dL_dmeans3D,
                                dL_dscales, dL_dquats, dL_dopacities, dL_dsh, touched, s);
         if (e != cudaSuccess) return cuda_fail(ctx, "tgs_raster_bwd_sparse (projection)", e);
