@@ -263,6 +263,27 @@ def test_raster_bwd_sparse_gradients(name, orc32, orc64, tgs, torch):
     print(name, f"sparse gradients: {int(on.sum())} of {N} Gaussians touched", rep)
 
 
+def test_raster_bwd_rejects_a_misaligned_sh_gradient(orc32, orc64, tgs, torch):
+    """dL_dsh (and sh) are moved with 16-byte accesses: a misaligned slice is an error, not a fault."""
+    import paper_2606_15924_b200 as pk
+    r = oracle_run("small_d2", orc32, orc64)
+    sc = r.sc
+    splats = dev(pack_splats(r.pre), torch)
+    b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
+    fwd = SimpleNamespace(T=dev(r.fwd.T, torch), n_contrib=dev(r.fwd.n_contrib.astype(np.int64), torch, torch.int32))
+    d = scene_dev(sc, torch)
+    N, K = sc.N, 9
+    f = dict(dtype=torch.float32, device="cuda")
+    raw = torch.empty(N * K * 3 + 1, **f)
+    out = SimpleNamespace(dL_dsplats=torch.empty((N, 12), **f), dL_dmeans3D=torch.empty((N, 3), **f),
+                          dL_dscales=torch.empty((N, 3), **f), dL_dquats=torch.empty((N, 4), **f),
+                          dL_dopacities=torch.empty((N,), **f), dL_dsh=raw[1:].view(N, K, 3))
+    with pytest.raises(pk.TgsError) as e:
+        tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, b, s, fwd, dev(r.g, torch), d.means3D, d.scales, d.quats, d.sh,
+                              dev(r.pre.radii, torch), dev(r.pre.clamped, torch), out=out)
+    assert e.value.code == 1 and "aligned" in str(e.value)
+
+
 @pytest.mark.parametrize("name", SCENES)
 def test_end_to_end_all_gpu(name, orc32, orc64, tgs, torch):
     """preprocess -> bin_sort -> sample -> fwd -> bwd entirely on the GPU, no oracle data in between."""
