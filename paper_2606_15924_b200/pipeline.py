@@ -114,9 +114,20 @@ class SparseIteration:
                                       dL_dscales=g["scales"][i], dL_dquats=g["quats"][i], dL_dopacities=g["opacities"][i],
                                       dL_dsh=g["sh"][i], touched=self.touched[i]) for i in range(V)]
         self.losses = [None] * V
+        self.delta = None
+
+    def _solve(self, params, m, v, t, beta1, beta2, eps, eta_sh, apply, stream):
+        """Alg. 1 steps 9-10.  apply=False: the update goes to self.delta instead of the parameters (Eq. 14 prints no step
+        size: with small gradients it degenerates to a unit-rate Adam step, R37 -- a caller that wants a trust
+        region scales Delta itself)."""
+        if not apply and self.delta is None:
+            self.delta = {k: torch.empty_like(a) for k, a in params.items()}
+        self.tgs.lm_solve(self.D, self.grads, m, v, view_touched=self.touched, beta1=beta1, beta2=beta2, eps=eps,
+                          eta_sh=eta_sh, t=t, want_delta=not apply, delta=None if apply else self.delta,
+                          params=params if apply else None, stream=stream)
 
     def run(self, params, targets, errs, m, v, t, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, beta1=0.9, beta2=0.999,
-            eps=1e-8, eta_sh=1.25e-4, stream=None):
+            eps=1e-8, eta_sh=1.25e-4, stream=None, apply=True):
         """params, m, v: parameter sets (dicts of device tensors), updated in place; targets[i]: [H, W, 3] image of view
         i; errs[i]: [H, W] error map that drives view i's sampling.  Returns the per-view loss namespaces."""
         st, tg = self.step, self.tgs
@@ -129,6 +140,29 @@ class SparseIteration:
             self.losses[i] = lo
             st.samp.k = samp.k
             st.backward(lo.dL_dcolor, sparse=True, out=self.views[i], stream=stream)
-        tg.lm_solve(self.D, self.grads, m, v, view_touched=self.touched, beta1=beta1, beta2=beta2, eps=eps, eta_sh=eta_sh,
-                    t=t, want_delta=False, params=params, stream=stream)
+        self._solve(params, m, v, t, beta1, beta2, eps, eta_sh, apply, stream)
+        return self.losses
+
+    def run_paper(self, params, targets, E_maps, ages, m, v, t, n_pix=25, n_hard=10, n_stable=8, beta=0.4, seed=0,
+                  beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, stream=None, apply=True):
+        """The same iteration with the paper's own sampler: per view, n_pix pixels in EVERY tile from the
+        view's persistent maps -- E_maps[i] (fp16 bits, [H, W]) and ages[i] (uint16 bits) --, all tiles binned, sparse
+        forward, fused loss, map update with the loss kernel's per-pixel error (Eq. 3-4), sparse backward; then the LM
+        solve.  params, m, v and the maps are updated in place."""
+        st, tg, D = self.step, self.tgs, self.D
+        p = params
+        for i, cam in enumerate(self.cams):
+            st.cam = cam
+            tg.preprocess(cam, D, p["means3D"], p["scales"], p["quats"], p["opacities"], p["sh"], out=st.pre, stream=stream)
+            sp = tg.sample_paper(cam, E_maps[i], ages[i], n_pix, n_hard, n_stable, seed=seed + i, out=st.samp,
+                                 workspace=st.ws_sample, sync=False, stream=stream)
+            tg.bin_sort(cam, st.pre.splats, st.P_capacity, out=st.binned, workspace=st.ws_sort, sync=False, stream=stream)
+            fw = tg.raster_fwd_sparse(cam, st.pre.splats, st.binned, sp, out=st.fwd, stream=stream)
+            lo = tg.loss_sparse(cam, sp, fw.color, targets[i], out=self.losses[i], stream=stream)
+            self.losses[i] = lo
+            tg.maps_update(cam, E_maps[i], ages[i], sp, lo.pix_err, beta, stream=stream)
+            tg.raster_bwd_sparse(cam, D, st.pre.splats, st.binned, sp, st.fwd, lo.dL_dcolor, p["means3D"], p["scales"],
+                                 p["quats"], p["sh"], st.pre.radii, st.pre.clamped, out=self.views[i], stream=stream,
+                                 sparse=True)
+        self._solve(params, m, v, t, beta1, beta2, eps, eta_sh, apply, stream)
         return self.losses

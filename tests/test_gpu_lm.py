@@ -323,3 +323,89 @@ def test_sparse_iteration_equals_its_calls(tgs, torch):
         np.testing.assert_allclose(m1[k].cpu().numpy(), m2[k].cpu().numpy(), rtol=1e-3, atol=1e-9)
         moved += int((step_size > 0).sum())
     assert moved > 1000
+
+
+def test_paper_iteration_equals_its_calls_and_replays_in_a_graph(tgs, torch):
+    """SparseIteration.run_paper (the paper's sampler from persistent maps, all tiles binned, loss, map update, sparse
+    backward, LM solve) against the same calls made one by one with dense gradients; the maps are integer work and must
+    agree bit for bit.  Then the whole iteration captured in ONE CUDA graph and replayed: nothing in it synchronises."""
+    import paper_2606_15924_b200 as pk
+    from helpers import dev, scene_dev
+    V, D = 2, 3
+    sc = workloads.small_random_scene(7, 3000, 200, 136, sh_degree=D, bg=(0.1, 0.3, 0.2), spread=1.3, log_scale=(-2.8, 0.6))
+    cams = [workloads.orbit_view(sc, i).cam for i in range(V)]
+    N, W, H = sc.N, sc.cam.width, sc.cam.height
+    rng = np.random.default_rng(23)
+    targets = [dev(rng.random((H, W, 3)).astype(np.float32), torch) for _ in range(V)]
+    E0 = [(4.0 * rng.random((H, W)) ** 3).astype(np.float16).view(np.int16) for _ in range(V)]
+    A0 = [rng.integers(0, 40, (H, W)).astype(np.int16) for _ in range(V)]
+    _, m_np, v_np, _ = workloads.lm_state(72, N, D, views=1)
+    d = scene_dev(sc, torch)
+    base = {"means3D": d.means3D, "scales": d.scales, "quats": d.quats, "opacities": d.opacities, "sh": d.sh}
+    clone = lambda ps: {k: a.clone() for k, a in ps.items()}
+    P_cap = 400_000
+    kw = dict(n_pix=25, n_hard=10, n_stable=8, beta=0.4, seed=9)
+
+    it = pk.SparseIteration(tgs, cams, N, D, P_cap)
+    p1, m1, v1 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
+    E1, A1 = [dev(e, torch) for e in E0], [dev(a, torch) for a in A0]
+    it.run_paper(p1, targets, E1, A1, m1, v1, t=2, **kw)
+    torch.cuda.synchronize()
+    P = int(it.step.binned.P_dev.cpu()[0])
+    assert 0 < P <= P_cap and int(it.step.binned.P_dev.cpu()[1]) == 0
+
+    # call by call, dense gradients
+    step = pk.SparseRasterStep(tgs, cams[0], N, D, P_cap)
+    K = (D + 1) ** 2
+    G = {"means3D": torch.zeros((V, N, 3), device="cuda"), "scales": torch.zeros((V, N, 3), device="cuda"),
+         "quats": torch.zeros((V, N, 4), device="cuda"), "opacities": torch.zeros((V, N), device="cuda"),
+         "sh": torch.zeros((V, N, K, 3), device="cuda")}
+    E2, A2 = [dev(e, torch) for e in E0], [dev(a, torch) for a in A0]
+    touched = np.zeros((V, N), bool)
+    for i, cam in enumerate(cams):
+        pre = tgs.preprocess(cam, D, base["means3D"], base["scales"], base["quats"], base["opacities"], base["sh"])
+        sp = tgs.sample_paper(cam, E2[i], A2[i], 25, 10, 8, seed=9 + i)
+        b = tgs.bin_sort(cam, pre.splats, P_cap)
+        fw = tgs.raster_fwd_sparse(cam, pre.splats, b, sp)
+        lo = tgs.loss_sparse(cam, sp, fw.color, targets[i])
+        tgs.maps_update(cam, E2[i], A2[i], sp, lo.pix_err, 0.4)
+        bw = tgs.raster_bwd_sparse(cam, D, pre.splats, b, sp, fw, lo.dL_dcolor, base["means3D"], base["scales"],
+                                   base["quats"], base["sh"], pre.radii, pre.clamped)
+        G["means3D"][i], G["scales"][i], G["quats"][i] = bw.dL_dmeans3D, bw.dL_dscales, bw.dL_dquats
+        G["opacities"][i], G["sh"][i] = bw.dL_dopacities, bw.dL_dsh
+        touched[i] = (bw.dL_dsplats.cpu().numpy()[:, :9] != 0).any(axis=1)
+        # the maps: integer / fixed-rounding work, deterministic given the same pix_err... which is (forward + loss are)
+        assert torch.equal(E1[i], E2[i]) and torch.equal(A1[i], A2[i]), "maps of view %d" % i
+    assert np.array_equal(it.touched.cpu().numpy() == 1, touched)
+    p2, m2, v2 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
+    upd = torch.from_numpy(touched.any(0).astype(np.int32)).cuda()
+    tgs.lm_solve(D, G, m2, v2, update=upd, t=2, want_delta=False, params=p2)
+    torch.cuda.synchronize()
+    for k in KEYS:
+        a, b_, b0 = p1[k].cpu().numpy().astype(np.float64), p2[k].cpu().numpy().astype(np.float64), base[k].cpu().numpy()
+        assert np.abs(a - b_).max() <= 1e-4 * np.abs(b_ - b0).max() + 1e-7, k
+    assert np.abs(p2["means3D"].cpu().numpy() - base["means3D"].cpu().numpy()).max() > 0
+
+    # one CUDA graph for the whole iteration, replayed on fresh state: same result as the eager run above
+    p3, m3, v3 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
+    E3, A3 = [dev(e, torch) for e in E0], [dev(a, torch) for a in A0]
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        it.run_paper(p3, targets, E3, A3, m3, v3, t=2, **kw)      # warm-up on the capture stream
+        s.synchronize()
+        for dst, src in ((p3, base), (m3, _dev(m_np, torch)), (v3, _dev(v_np, torch))):
+            for k in KEYS:
+                dst[k].copy_(src[k])
+        for i in range(V):
+            E3[i].copy_(dev(E0[i], torch)); A3[i].copy_(dev(A0[i], torch))
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            it.run_paper(p3, targets, E3, A3, m3, v3, t=2, **kw)
+    g.replay()
+    torch.cuda.synchronize()
+    for i in range(V):
+        assert torch.equal(E3[i], E1[i]) and torch.equal(A3[i], A1[i])
+    for k in KEYS:
+        a, b_, b0 = p3[k].cpu().numpy().astype(np.float64), p1[k].cpu().numpy().astype(np.float64), base[k].cpu().numpy()
+        assert np.abs(a - b_).max() <= 1e-4 * np.abs(b_ - b0).max() + 1e-7, k
