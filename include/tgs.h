@@ -152,6 +152,47 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam,
                uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host,
                void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- a3 without any allocation: tgs_sample for callers that cannot obtain device memory ------
+ * Who this is for.  tgs_sample needs a device workspace, and every other call needs a tgs_ctx, whose creation
+ * makes a small cudaMalloc.  Some hosts of this library can do neither: a plug-in whose host application hands it
+ * the input and output buffers but forbids it to allocate on the GPU (the host accounts for every byte of HBM
+ * itself); a step inside a training or serving loop whose latency budget rules out cudaMalloc, because it
+ * synchronises the whole device and stalls every other stream; and a process in which a framework's caching
+ * allocator already owns all of HBM, so that a raw cudaMalloc from a library beside it simply fails.  For them:
+ *
+ * tgs_sample_static computes exactly what tgs_sample computes (same kernels, same bit-exact outputs, same
+ * argument meaning) but takes NO context and NO workspace.  Its scratch -- 36 B of keep mask and 4 B of selection
+ * flag per tile -- is a fixed array inside the library's device image, sized for
+ * TGS_SAMPLE_STATIC_MAX_TILES = 16384 tiles (any image up to 2048 x 2048, e.g. all five BASELINE.json
+ * configs): 640 KiB that every GPU which loads libtgs holds until the process exits, whether or not this call is
+ * ever made.  The call itself, and everything it calls, uses no cudaMalloc, cudaFree, cudaMallocAsync, stream or
+ * event creation, or any library routine that allocates; inputs and outputs are the caller's, as in tgs_sample.
+ *
+ *   device        the CUDA device the buffers and `stream` live on; made current by the call.
+ *   err_msg       (host, nullable) receives a NUL-terminated description when the return value is not TGS_OK;
+ *                 err_msg_bytes is its capacity.  There is no context to ask afterwards.
+ *   everything else as tgs_sample (kn_host non-NULL forces one stream synchronisation).
+ *
+ * Limit: an image of more than TGS_SAMPLE_STATIC_MAX_TILES tiles is refused with TGS_ERR_CAPACITY and a message
+ * naming both numbers; nothing is launched.  Use tgs_sample with a workspace for such images.
+ * First call on a device: looks up the device address of the scratch array (cudaGetSymbolAddress), which can make
+ * the CUDA runtime load this library's device code onto that GPU.  Make that first call once per device during
+ * start-up, before any stream capture begins and outside any region where an implicit synchronisation hurts;
+ * later calls on that device only launch three kernels.
+ * Sharing: there is ONE array per GPU and every call on that GPU uses it, from whatever thread or stream.  Calls
+ * are safe one after another in the same stream (nothing needs clearing in between: a call overwrites every word
+ * it later reads and never reads beyond its own tile count, so a previous call's contents are invisible).  Two
+ * calls that may run on the GPU at the same time -- different streams, or different threads without ordering --
+ * overwrite each other's masks and give wrong pixel lists: order them with events or use one stream. */
+#define TGS_SAMPLE_STATIC_MAX_TILES 16384
+int tgs_sample_static(int device, const tgs_camera* cam,
+                      const float* err, const float* render, const float* target,
+                      int tile_pct_num, int tile_pct_den, int pixel_mode,
+                      int pix_rate_num, int pix_rate_den, uint64_t seed,
+                      uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+                      uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host,
+                      char* err_msg, size_t err_msg_bytes, void* stream);
+
 /* ---- a4: sparse forward (Eq. 1, 154-166) ---------------------------------------
  * For each sampled pixel p of sampled tile tiles[i]: front-to-back over the tile's range,
  *   alpha = min(0.99, o * exp(-1/2 d^T conic d)), skipped if alpha < 1/255, stop before the

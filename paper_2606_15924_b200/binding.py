@@ -25,7 +25,7 @@ ERR_NAMES = {0: "TGS_OK", 1: "TGS_ERR_INVALID_ARG", 2: "TGS_ERR_CAPACITY", 3: "T
 # every symbol include/tgs.h declares (tests check the library exports them all)
 SYMBOLS = ["tgs_create", "tgs_destroy", "tgs_last_error", "tgs_version", "tgs_launch_count", "tgs_fp32_peak", "tgs_preprocess",
            "tgs_bin_sort_workspace_bytes", "tgs_bin_sort", "tgs_sample_num_tiles",
-           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse", "tgs_sample_paper",
+           "tgs_sample_workspace_bytes", "tgs_sample", "tgs_sample_static", "tgs_raster_fwd_sparse", "tgs_raster_bwd_sparse", "tgs_loss_sparse", "tgs_raster_stats_sparse", "tgs_sample_paper",
            "tgs_maps_update", "tgs_lm_solve"]
 PARAM_KEYS = ("means3D", "scales", "quats", "opacities", "sh")
 
@@ -104,6 +104,8 @@ def load_library() -> C.CDLL:
     lib.tgs_sample_workspace_bytes.argtypes = [cam, C.POINTER(C.c_size_t)]
     lib.tgs_sample.argtypes = [vp, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp, vp,
                                C.POINTER(C.c_int32), vp, C.c_size_t, vp]
+    lib.tgs_sample_static.argtypes = [i32, cam, vp, vp, vp, i32, i32, i32, i32, i32, u64, vp, vp, vp, vp, vp, vp,
+                                      C.POINTER(C.c_int32), C.c_char_p, C.c_size_t, vp]
     lib.tgs_raster_fwd_sparse.argtypes = [vp, cam, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.tgs_raster_bwd_sparse.argtypes = [vp, cam, i32, i32, vp, vp, vp, i32, vp, vp, vp, vp, vp, vp] + [vp] * 6 + \
                                          [vp] + [vp] * 5 + [vp, vp]
@@ -128,6 +130,43 @@ def _p(t):
 def _stream(stream=None):
     s = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(s.cuda_stream)
+
+
+SAMPLE_STATIC_MAX_TILES = 16384  # TGS_SAMPLE_STATIC_MAX_TILES of include/tgs.h
+
+
+def sample_static(device, cam, tile_pct, pixel_mode, out, pix_rate=(1, 1), seed=0, err=None, render=None, target=None,
+                  sync=True, stream=None, lib=None):
+    """tgs_sample_static: what `TGS.sample` computes, for a caller that may not allocate device memory.
+
+    Some programs that embed this library are handed their GPU buffers and are not allowed (or not able) to get more:
+    a plug-in under a host application's memory budget, a step in a loop that cannot afford cudaMalloc's device-wide
+    synchronisation, a process whose framework allocator already owns all of HBM.  This call needs no `TGS` context
+    and no workspace: its scratch is a fixed 640 KiB array inside the loaded library, good for images of up to
+    SAMPLE_STATIC_MAX_TILES = 16384 tiles (2048 x 2048); a larger image raises TgsError (TGS_ERR_CAPACITY).
+
+    `out` is REQUIRED and is the caller's: a namespace with device tensors tile_score[T] (int64), tiles[T],
+    tile_pix_offsets[T+1], pix[W*H], kn_dev[2] (int32) and optionally tile_select[T] -- the fields `TGS.sample`
+    returns.  This wrapper allocates no tensor either.  The first call on a device resolves the scratch address
+    (it may load the library's device code): make it during start-up, before capturing any stream.  All calls on
+    one GPU share the one scratch array: issue them on one stream, or order them with events -- calls that overlap
+    on the GPU corrupt each other's pixel lists."""
+    lib = lib if lib is not None else load_library()
+    cam = Camera.of(cam)
+    kn = (C.c_int32 * 2)(-1, -1)
+    msg = C.create_string_buffer(512)
+    rc = lib.tgs_sample_static(int(device), C.byref(cam), _p(err), _p(render), _p(target), int(tile_pct[0]),
+                               int(tile_pct[1]), int(pixel_mode), int(pix_rate[0]), int(pix_rate[1]), C.c_uint64(seed),
+                               _p(out.tile_score), _p(out.tiles), _p(out.tile_pix_offsets), _p(out.pix),
+                               _p(getattr(out, "tile_select", None)), _p(out.kn_dev), kn if sync else None,
+                               msg, len(msg), _stream(stream))
+    if rc != 0:
+        raise TgsError(rc, msg.value.decode())
+    out.k = lib.tgs_sample_num_tiles(C.byref(cam), int(tile_pct[0]), int(tile_pct[1]))
+    if sync:
+        assert kn[0] == out.k
+        out.n = int(kn[1])
+    return out
 
 
 class TGS:

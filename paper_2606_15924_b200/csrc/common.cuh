@@ -99,6 +99,13 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
                           uint32_t* tpo, uint32_t* pix, uint32_t* tile_select, int32_t* kn_dev, void* ws,
                           cudaStream_t s);
 
+// tgs_sample_static: launch_sample with its scratch in a static device array of sample.cu (no workspace argument)
+int sample_static_max_tiles();
+cudaError_t launch_sample_static(int device, const CamK& cam, const float* err, const float* render, const float* target,
+                                 int k, int mode, int rnum, int rden, uint64_t seed, uint64_t* tile_score,
+                                 uint32_t* tiles, uint32_t* tpo, uint32_t* pix, uint32_t* tile_select, int32_t* kn_dev,
+                                 cudaStream_t s);
+
 cudaError_t launch_raster_fwd(const CamK& cam, const float* splats, const uint32_t* tile_offsets,
                               const uint32_t* gid_sorted, int k, const uint32_t* tiles, const uint32_t* tpo,
                               const uint32_t* pix, float* out_color, float* out_T, uint32_t* n_contrib,

@@ -4,7 +4,19 @@
 // integers on a fixed-point copy of the error so that it is order independent and bit exact.
 #include <cuda_fp16.h>
 
+#include <atomic>
+
 #include "common.cuh"
+
+// Scratch of tgs_sample_static (include/tgs.h): the per-tile keep masks and selection flags that tgs_sample keeps
+// in a caller-allocated workspace live here instead, in memory that is part of the loaded library image, so that the
+// call works for a host program that has no way to allocate device memory.  Sized for
+// TGS_SAMPLE_STATIC_MAX_TILES = 16384 tiles (36 B + 4 B per tile, each part rounded up to 256 B): 640 KiB, held by
+// every GPU that loads libtgs from the moment the module is loaded until the process exits.
+// In HOST code this name is only a handle for cudaGetSymbolAddress -- it is not a device address and is never
+// passed to a kernel; static_scratch_on() below turns it into one, per device.
+constexpr size_t kStaticScratchBytes = 640u * 1024u;
+static __device__ __align__(256) unsigned char g_sample_static_scratch[kStaticScratchBytes];
 
 namespace tgs {
 
@@ -411,6 +423,59 @@ cudaError_t launch_sample(const CamK& cam, const float* err, const float* render
     const int T = cam.gx * cam.gy;
     TileMeta* meta = (TileMeta*)ws;
     uint32_t* selected = tile_select ? tile_select : (uint32_t*)((char*)ws + align256((size_t)T * sizeof(TileMeta)));
+    tile_reduce_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, err, render, target, mode, rnum, rden, seed, tile_score, meta);
+    tile_select_compact_kernel<<<1, 1024, 0, s>>>(T, k, tile_score, meta, selected, tiles, tpo, kn_dev);
+    write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);
+    count_launches(3);
+    return cudaGetLastError();
+}
+
+// ---- tgs_sample_static: the same three kernels, scratch in g_sample_static_scratch ----
+namespace {
+
+constexpr int kStaticMaxTiles = TGS_SAMPLE_STATIC_MAX_TILES;
+static_assert(sizeof(TileMeta) == 36, "TileMeta is 36 B per tile");
+static_assert(((size_t)kStaticMaxTiles * sizeof(TileMeta) + 255) / 256 * 256 + ((size_t)kStaticMaxTiles * 4 + 255) / 256 * 256
+                  <= kStaticScratchBytes, "static scratch too small for TGS_SAMPLE_STATIC_MAX_TILES");
+
+constexpr int kStaticDevSlots = 64;
+std::atomic<void*> g_static_scratch_dev[kStaticDevSlots];  // device address of the array on device d, once resolved
+
+// Device address of g_sample_static_scratch on `device`, which must be the current device.  Every GPU has its own
+// copy of the array, so the address is looked up once per device and remembered (two threads racing here both get
+// the same answer).  The look-up may load the library's device code on that GPU: that is the set-up step the header
+// asks callers to get out of the way before they start capturing a stream.
+cudaError_t static_scratch_on(int device, void** out) {
+    void* p = device < kStaticDevSlots ? g_static_scratch_dev[device].load(std::memory_order_acquire) : nullptr;
+    if (!p) {
+        cudaError_t e = cudaGetSymbolAddress(&p, g_sample_static_scratch);
+        if (e != cudaSuccess) return e;
+        if (!p) return cudaErrorInvalidSymbol;
+        if (device < kStaticDevSlots) g_static_scratch_dev[device].store(p, std::memory_order_release);
+    }
+    *out = p;
+    return cudaSuccess;
+}
+
+}  // namespace
+
+int sample_static_max_tiles() { return kStaticMaxTiles; }
+
+// Same launches as launch_sample, scratch = the static array.  Nothing in the scratch has to start at zero: for the
+// T tiles of this call, tile_reduce_kernel writes all nine words of meta[t] and tile_select_compact_kernel writes
+// selected[t] before any kernel reads them, and no kernel reads beyond tile T-1, so whatever an earlier (possibly
+// larger) call left behind is never seen.
+cudaError_t launch_sample_static(int device, const CamK& cam, const float* err, const float* render, const float* target,
+                                 int k, int mode, int rnum, int rden, uint64_t seed, uint64_t* tile_score,
+                                 uint32_t* tiles, uint32_t* tpo, uint32_t* pix, uint32_t* tile_select, int32_t* kn_dev,
+                                 cudaStream_t s) {
+    const int T = cam.gx * cam.gy;
+    if (T > kStaticMaxTiles) return cudaErrorInvalidValue;  // the ABI glue has already said so in words
+    void* ws = nullptr;
+    cudaError_t e = static_scratch_on(device, &ws);
+    if (e != cudaSuccess) return e;
+    TileMeta* meta = (TileMeta*)ws;
+    uint32_t* selected = tile_select ? tile_select : (uint32_t*)((char*)ws + align256((size_t)kStaticMaxTiles * sizeof(TileMeta)));
     tile_reduce_kernel<<<(T + 7) / 8, 256, 0, s>>>(cam, err, render, target, mode, rnum, rden, seed, tile_score, meta);
     tile_select_compact_kernel<<<1, 1024, 0, s>>>(T, k, tile_score, meta, selected, tiles, tpo, kn_dev);
     write_pix_kernel<<<(k + 7) / 8, 256, 0, s>>>(cam, k, tiles, tpo, meta, pix);

@@ -254,6 +254,53 @@ int tgs_sample(tgs_ctx* ctx, const tgs_camera* cam, const float* err, const floa
     return TGS_OK;
 }
 
+// tgs_sample without a context or a workspace (include/tgs.h: for callers that cannot allocate device memory).
+// Validation mirrors tgs_sample; messages go to the caller's buffer because there is no context to keep them in.
+// Nothing on this path allocates: no cudaMalloc / cudaFree, no stream or event creation, no new / malloc.
+int tgs_sample_static(int device, const tgs_camera* cam, const float* err, const float* render, const float* target,
+                      int tile_pct_num, int tile_pct_den, int pixel_mode, int pix_rate_num, int pix_rate_den,
+                      uint64_t seed, uint64_t* tile_score, uint32_t* tiles, uint32_t* tile_pix_offsets, uint32_t* pix,
+                      uint32_t* tile_select, int32_t* kn_dev, int32_t* kn_host, char* err_msg, size_t err_msg_bytes,
+                      void* stream) {
+    auto say = [&](int code, const char* fmt, auto... a) {
+        if (err_msg && err_msg_bytes) snprintf(err_msg, err_msg_bytes, fmt, a...);
+        return code;
+    };
+    if (err_msg && err_msg_bytes) err_msg[0] = 0;
+    if (device < 0) return say(TGS_ERR_INVALID_ARG, "tgs_sample_static: device %d", device);
+    cudaError_t e = cudaSetDevice(device);
+    if (e != cudaSuccess) return say(TGS_ERR_CUDA, "tgs_sample_static: cudaSetDevice(%d): %s", device, cudaGetErrorString(e));
+    if (!cam_ok(cam)) return say(TGS_ERR_INVALID_ARG, "%s", "tgs_sample_static: bad camera");
+    if (tile_pct_den <= 0 || tile_pct_num < 0 || tile_pct_num > tile_pct_den)
+        return say(TGS_ERR_INVALID_ARG, "tgs_sample_static: tile fraction %d/%d not in [0,1]", tile_pct_num, tile_pct_den);
+    if (pixel_mode != TGS_PIXELS_ALL && pixel_mode != TGS_PIXELS_BERNOULLI_ERR)
+        return say(TGS_ERR_UNSUPPORTED, "tgs_sample_static: pixel_mode %d", pixel_mode);
+    if (pixel_mode == TGS_PIXELS_BERNOULLI_ERR &&
+        (pix_rate_den <= 0 || pix_rate_den > 255 || pix_rate_num < 0 || pix_rate_num > 255))
+        return say(TGS_ERR_INVALID_ARG, "tgs_sample_static: pixel rate %d/%d outside 0..255", pix_rate_num, pix_rate_den);
+    if (!err && !(render && target)) return say(TGS_ERR_INVALID_ARG, "%s", "tgs_sample_static: need err or render+target");
+    if (!tile_score || !tiles || !tile_pix_offsets || !pix || !kn_dev)
+        return say(TGS_ERR_INVALID_ARG, "%s", "tgs_sample_static: null pointer");
+    // 64-bit tile count: the camera is unchecked user input and the limit must hold before anything is launched
+    const int64_t T = (int64_t)((cam->width + kTile - 1) / kTile) * (int64_t)((cam->height + kTile - 1) / kTile);
+    if (T > (int64_t)sample_static_max_tiles())
+        return say(TGS_ERR_CAPACITY,
+                   "tgs_sample_static: a %d x %d image has %lld tiles, the static scratch holds %d "
+                   "(TGS_SAMPLE_STATIC_MAX_TILES); use tgs_sample with a workspace",
+                   cam->width, cam->height, (long long)T, sample_static_max_tiles());
+    const int k = tgs_sample_num_tiles(cam, tile_pct_num, tile_pct_den);
+    cudaStream_t s = (cudaStream_t)stream;
+    e = launch_sample_static(device, make_camk(cam), err, render, target, k, pixel_mode, pix_rate_num, pix_rate_den, seed,
+                             tile_score, tiles, tile_pix_offsets, pix, tile_select, kn_dev, s);
+    if (e != cudaSuccess) return say(TGS_ERR_CUDA, "tgs_sample_static: %s", cudaGetErrorString(e));
+    if (kn_host) {
+        e = cudaMemcpyAsync(kn_host, kn_dev, 2 * sizeof(int32_t), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) return say(TGS_ERR_CUDA, "tgs_sample_static (k,n readback): %s", cudaGetErrorString(e));
+    }
+    return TGS_OK;
+}
+
 int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const float* splats,
                           const uint32_t* tile_offsets, const uint32_t* gid_sorted, int k, const uint32_t* tiles,
                           const uint32_t* tile_pix_offsets, const uint32_t* pix, float* out_color, float* out_T,
