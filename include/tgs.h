@@ -326,6 +326,12 @@ typedef struct tgs_params {
  *           update[n] == 0.  NULL: every row of grads is read.
  *   delta   nullable: receives Delta in the parameter layouts.
  *   params  nullable: Alg. 1 step 10, params <- params + Delta in place.  At least one of delta / params.
+ *           Eq. 14 prints no step size: with small gradients Delta degenerates to -m/(sqrt(v)+eps), an Adam direction
+ *           at unit rate, and a few such steps diverge (R37).  Pass `delta` and apply a scaled step yourself
+ *           unless you want the step exactly as printed; the Python pipeline does so by default (apply=False).
+ *   t       HOST scalar (t >= 1): 1 - beta^t is formed on the host (pow) and travels in the launch arguments, as do
+ *           the seeds of tgs_sample / tgs_sample_paper.  A CUDA graph that captured these calls therefore replays with
+ *           the t and seeds of the capture; re-capture, or update the kernel-node parameters, when they must change.
  * Arithmetic: fp32 storage.  For the two LM blocks the moment sums, J^T J and the Cholesky factorisation /
  * substitutions run in fp64 registers (the systems mix parameter groups whose gradients differ by orders of
  * magnitude: condition numbers of 1e4-1e8 would otherwise leave 1e-3-level errors in Delta); the Adam branch is

@@ -1,5 +1,6 @@
 // C-ABI entry points of libtgs (include/tgs.h): argument validation, error reporting and launch
 // order.  No arithmetic of the method lives here.
+#include <math.h>
 #include <stdarg.h>
 #include <string.h>
 
@@ -457,9 +458,8 @@ int tgs_lm_solve(tgs_ctx* ctx, int N, int sh_degree, int V, const tgs_params* gr
     a.vt = view_touched;
     a.N = N; a.K = (sh_degree + 1) * (sh_degree + 1); a.V = V;
     a.b1 = (double)beta1; a.b2 = (double)beta2; a.eps = (double)eps;
-    // bias corrections of Eq. 19 (right) are scalars of the call, formed in double on the host
-    double p1 = 1.0, p2 = 1.0;
-    for (int i = 0; i < t && (p1 > 0.0 || p2 > 0.0); ++i) { p1 *= a.b1; p2 *= a.b2; }
+    // bias corrections of Eq. 19 (right) are scalars of the call, formed in double on the host (pow: O(1) in t)
+    const double p1 = pow(a.b1, (double)t), p2 = pow(a.b2, (double)t);
     a.inv_bc1 = 1.0 / (1.0 - p1); a.inv_bc2 = 1.0 / (1.0 - p2);
     a.eta = eta_sh; a.epsf = eps;
     a.b1f = beta1; a.b2f = beta2; a.omb1f = (float)(1.0 - a.b1); a.omb2f = (float)(1.0 - a.b2);

@@ -103,6 +103,13 @@ class SparseIteration:
     def __init__(self, tgs: TGS, cams, N: int, sh_degree: int, P_capacity: int):
         self.tgs, self.cams, self.N, self.D = tgs, [Camera.of(c) for c in cams], int(N), int(sh_degree)
         V, K, dev = len(self.cams), (sh_degree + 1) ** 2, tgs.device
+        # view i's SH gradients are the slice grads["sh"][i] of one [V, N, K, 3] buffer, and the kernels read and write SH
+        # rows as float4: the per-view stride N*K*3 floats must be a multiple of 4 (only sh_degree 2, K = 9, with N % 4 != 0
+        # breaks it).  Refused here, at construction, rather than by tgs_raster_bwd_sparse in the middle of an iteration.
+        if V > 1 and (self.N * K * 3) % 4 != 0:
+            raise ValueError(f"SparseIteration: with sh_degree = {sh_degree} the per-view SH gradient slice is "
+                             f"{self.N * K * 3} floats, not a multiple of 4 (16-byte alignment of every view's slice): "
+                             f"make N = {self.N} a multiple of 4")
         self.step = SparseRasterStep(tgs, self.cams[0], N, sh_degree, P_capacity)
         f = dict(dtype=torch.float32, device=dev)
         self.grads = {"means3D": torch.empty((V, N, 3), **f), "scales": torch.empty((V, N, 3), **f),
@@ -117,9 +124,10 @@ class SparseIteration:
         self.delta = None
 
     def _solve(self, params, m, v, t, beta1, beta2, eps, eta_sh, apply, stream):
-        """Alg. 1 steps 9-10.  apply=False: the update goes to self.delta instead of the parameters (Eq. 14 prints no step
-        size: with small gradients it degenerates to a unit-rate Adam step, R37 -- a caller that wants a trust
-        region scales Delta itself)."""
+        """Alg. 1 steps 9-10.  apply=False (the default of run / run_paper): the update goes to self.delta and the
+        parameters are left alone.  Eq. 14 prints no step size: with small gradients it degenerates to a unit-rate Adam
+        step, and three such steps blow the scales up on configs[3] (R37) -- so the step as printed is only
+        applied when the caller asks for it with apply=True; a caller that wants a trust region scales Delta itself."""
         if not apply and self.delta is None:
             self.delta = {k: torch.empty_like(a) for k, a in params.items()}
         self.tgs.lm_solve(self.D, self.grads, m, v, view_touched=self.touched, beta1=beta1, beta2=beta2, eps=eps,
@@ -127,9 +135,14 @@ class SparseIteration:
                           params=params if apply else None, stream=stream)
 
     def run(self, params, targets, errs, m, v, t, tile_pct, pixel_mode, pix_rate=(1, 1), seed=0, beta1=0.9, beta2=0.999,
-            eps=1e-8, eta_sh=1.25e-4, stream=None, apply=True):
-        """params, m, v: parameter sets (dicts of device tensors), updated in place; targets[i]: [H, W, 3] image of view
-        i; errs[i]: [H, W] error map that drives view i's sampling.  Returns the per-view loss namespaces."""
+            eps=1e-8, eta_sh=1.25e-4, stream=None, apply=False):
+        """params, m, v: parameter sets (dicts of device tensors); m and v are updated in place, params only with
+        apply=True (Alg. 1 step 10 as printed, no step size: DESIGN.md R37), otherwise Delta is left in self.delta;
+        targets[i]: [H, W, 3] image of view i; errs[i]: [H, W] error map that drives view i's sampling.  Returns the
+        per-view loss namespaces.
+        CUDA graphs: t (the bias correction of Eq. 19) and the per-view sampler seeds seed + i are HOST scalars that go
+        into the launch arguments, so a captured iteration replays with the t and the seeds it was captured with:
+        re-capture (or update the kernel-node parameters) every iteration that needs new ones."""
         st, tg = self.step, self.tgs
         for i, cam in enumerate(self.cams):
             fw = st.forward(params["means3D"], params["scales"], params["quats"], params["opacities"], params["sh"],
@@ -144,11 +157,12 @@ class SparseIteration:
         return self.losses
 
     def run_paper(self, params, targets, E_maps, ages, m, v, t, n_pix=25, n_hard=10, n_stable=8, beta=0.4, seed=0,
-                  beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, stream=None, apply=True):
+                  beta1=0.9, beta2=0.999, eps=1e-8, eta_sh=1.25e-4, stream=None, apply=False):
         """The same iteration with the paper's own sampler: per view, n_pix pixels in EVERY tile from the
         view's persistent maps -- E_maps[i] (fp16 bits, [H, W]) and ages[i] (uint16 bits) --, all tiles binned, sparse
         forward, fused loss, map update with the loss kernel's per-pixel error (Eq. 3-4), sparse backward; then the LM
-        solve.  params, m, v and the maps are updated in place."""
+        solve.  m, v and the maps are updated in place; params only with apply=True (see run), else Delta is in
+        self.delta.  A captured graph of this call replays with the t and seeds of the capture (see run)."""
         st, tg, D = self.step, self.tgs, self.D
         p = params
         for i, cam in enumerate(self.cams):

@@ -289,7 +289,7 @@ def test_sparse_iteration_equals_its_calls(tgs, torch):
 
     it = pk.SparseIteration(tgs, cams, N, D, P_cap)
     p1, m1, v1 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
-    it.run(p1, targets, errs, m1, v1, t=3, tile_pct=(50, 100), pixel_mode=pk.PIXELS_ALL, seed=5)
+    it.run(p1, targets, errs, m1, v1, t=3, tile_pct=(50, 100), pixel_mode=pk.PIXELS_ALL, seed=5, apply=True)
     torch.cuda.synchronize()
     touched = it.touched.cpu().numpy()
     assert set(np.unique(touched)) <= {0, 1} and 0 < touched.sum() < touched.size
@@ -344,7 +344,7 @@ def test_paper_iteration_equals_its_calls_and_replays_in_a_graph(tgs, torch):
     base = {"means3D": d.means3D, "scales": d.scales, "quats": d.quats, "opacities": d.opacities, "sh": d.sh}
     clone = lambda ps: {k: a.clone() for k, a in ps.items()}
     P_cap = 400_000
-    kw = dict(n_pix=25, n_hard=10, n_stable=8, beta=0.4, seed=9)
+    kw = dict(n_pix=25, n_hard=10, n_stable=8, beta=0.4, seed=9, apply=True)
 
     it = pk.SparseIteration(tgs, cams, N, D, P_cap)
     p1, m1, v1 = clone(base), _dev(m_np, torch), _dev(v_np, torch)
@@ -409,3 +409,24 @@ def test_paper_iteration_equals_its_calls_and_replays_in_a_graph(tgs, torch):
     for k in KEYS:
         a, b_, b0 = p3[k].cpu().numpy().astype(np.float64), p1[k].cpu().numpy().astype(np.float64), base[k].cpu().numpy()
         assert np.abs(a - b_).max() <= 1e-4 * np.abs(b_ - b0).max() + 1e-7, k
+
+    # a SECOND replay: t and the sampler seeds are host scalars baked into the captured launches (tgs.h, tgs_lm_solve),
+    # so the replay is the eager call with the SAME t = 2 and seed = 9 on the state the first iteration left -- not an
+    # iteration with t = 3.  Both start from identical state (the eager run's), in the buffers the graph points at.
+    for dst, src in ((p3, p1), (m3, m1), (v3, v1)):
+        for k in KEYS:
+            dst[k].copy_(src[k])
+    for i in range(V):
+        E3[i].copy_(E1[i]); A3[i].copy_(A1[i])
+    before = {k: p1[k].clone() for k in KEYS}
+    it.run_paper(p1, targets, E1, A1, m1, v1, t=2, **kw)
+    torch.cuda.synchronize()
+    g.replay()
+    torch.cuda.synchronize()
+    for i in range(V):
+        assert torch.equal(E3[i], E1[i]) and torch.equal(A3[i], A1[i]), "maps of view %d after the second replay" % i
+    for k in KEYS:
+        a, b_, b0 = p3[k].cpu().numpy().astype(np.float64), p1[k].cpu().numpy().astype(np.float64), before[k].cpu().numpy()
+        assert np.abs(a - b_).max() <= 1e-4 * np.abs(b_ - b0).max() + 1e-7, k
+        np.testing.assert_allclose(m3[k].cpu().numpy(), m1[k].cpu().numpy(), rtol=1e-3, atol=1e-9)
+    assert np.abs(p1["means3D"].cpu().numpy() - before["means3D"].cpu().numpy()).max() > 0
