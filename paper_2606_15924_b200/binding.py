@@ -371,6 +371,22 @@ class TGS:
         view_touched: [V,N] int32, the `touched` masks of the V backward calls (rows of grads are read only where set).
         Returns the delta parameter set (allocated here unless given; None if want_delta is False)."""
         V, N = grads["opacities"].shape
+        K = (sh_degree + 1) ** 2
+        if not 1 <= V <= 64:
+            raise ValueError(f"lm_solve: V = {V} views, the kernels take 1..64")
+        # the kernels index raw pointers with these extents: a wrong dtype or shape is misread silently (a bool mask
+        # even out of bounds), so it is refused here
+        shapes = {"means3D": (N, 3), "scales": (N, 3), "quats": (N, 4), "opacities": (N,), "sh": (N, K, 3)}
+        for name, ps, lead in (("grads", grads, (V,)), ("m", m, ()), ("v", v, ()), ("delta", delta, ()), ("params", params, ())):
+            if ps is None:
+                continue
+            for k in PARAM_KEYS:
+                if tuple(ps[k].shape) != lead + shapes[k]:
+                    raise ValueError(f"lm_solve: {name}[{k!r}] has shape {tuple(ps[k].shape)}, expected {lead + shapes[k]}")
+        for name, mask, shape in (("update", update, (N,)), ("view_touched", view_touched, (V, N))):
+            if mask is not None and (mask.dtype != torch.int32 or tuple(mask.shape) != shape):
+                raise ValueError(f"lm_solve: {name} must be an int32 tensor of shape {shape}, got {mask.dtype} "
+                                 f"{tuple(mask.shape)}")
         if delta is None and want_delta:
             delta = {k: torch.empty_like(m[k]) for k in PARAM_KEYS}
         pg, pm, pv = Params.of(grads), Params.of(m), Params.of(v)
