@@ -215,7 +215,10 @@ int tgs_raster_fwd_sparse(tgs_ctx* ctx, const tgs_camera* cam, int N, const floa
  * dL_dmeans3D == NULL (then only dL_dsplats is produced).  Derivatives are those of the forward as
  * defined: zero through an active 0.99 alpha clamp, an active colour clamp and for culled Gaussians.
  * quats, sh, dL_dquats, dL_dsh and dL_dsplats must be 16-byte aligned (a view's slice of a [V,N,K,3] buffer is, unless
- * sh_degree == 2 and N is not a multiple of 4).
+ * sh_degree is 0 or 2 and N is not a multiple of 4).
+ * Pixel order: the pixels of one tile may be listed in any order (in all three raster calls; the lists need not come
+ * from tgs_sample).  A 256-pixel tile listed row-major, as tgs_sample writes it, takes a faster accumulation path in the
+ * backward; the kernel checks the order per 32-pixel unit and any other order takes the general path, same results.
  * touched[N] (int32, nullable): SPARSE GRADIENTS.  A Gaussian that is not listed in any sampled tile (or whose raster
  * gradient record is all zero) has a zero gradient; with 5 % of the tiles sampled that is ~85 % of them.  NULL: their
  * rows of the five outputs are written as zeros.  Given: touched[i] = 1 and rows written where the record is

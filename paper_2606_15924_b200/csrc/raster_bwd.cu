@@ -35,7 +35,7 @@ struct WarpXpose {
     float4 mb[kSlots];            // -C/2, opacity, bits: Gaussian id, unused
     float4 pa[32];                // per pixel: px, py, g0, g1
     float pb[32];                 // per pixel: g2
-    float4 org;                   // x, y of lane 0's pixel; z != 0: the unit is a full 8x4 block (separable phase 2)
+    float4 org;                   // x, y of lane 0's pixel; z != 0: the unit is an 8x4 block of a row-major full tile (separable phase 2)
 };
 
 constexpr int kBwdStageEntries = 128;
@@ -58,7 +58,8 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     ring_init(sm.ring);
     if (warp == kConsumers) {
-        producer_loop<true>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, n_contrib, sched, lane, kLitePixels);
+        producer_loop<true>(sm.ring, splats, tile_offsets, gid_sorted, (uint32_t)k, tiles, tpo, n_contrib, sched, lane, kLitePixels,
+                            pix, (uint32_t)cam.W);
         return;
     }
     BwdRing& R = sm.ring;
@@ -170,7 +171,7 @@ raster_bwd_kernel(const CamK cam, const float4* __restrict__ splats, const uint3
                 T = Tf; Sg = 0.f;
                 sx.pa[lane] = make_float4(px, py, g0, g1);
                 sx.pb[lane] = g2;
-                if (lane == 0) sx.org = make_float4(px, py, ui.full ? 1.f : 0.f, 0.f);
+                if (lane == 0) sx.org = make_float4(px, py, inf.rowmajor ? 1.f : 0.f, 0.f);  // 256 pixels, verified row-major
             }
         }
         if (wmax > 0) {

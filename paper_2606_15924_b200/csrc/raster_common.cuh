@@ -47,7 +47,7 @@ struct StageInfo {
     uint32_t cnt;   // valid records in this stage
     uint32_t hdr;   // index into tiles[] of the sampled tile this stage STARTS, kHdrCont, or kHdrEnd
     uint32_t base;  // range position (0-based) of record 0; forward ascending, backward descending
-    uint32_t pad;
+    uint32_t rowmajor;  // backward, on a tile's first stage: 1 = the tile lists 256 pixels in row-major order (else 0)
 };
 template <int ENTRIES, bool DEPTH = false>
 struct Stage {
@@ -172,7 +172,8 @@ struct UnitInfo {
     uint32_t start, end;  // tile range in gid_sorted
     uint32_t slot;        // this lane's index in the sampled-pixel list (valid if active)
     bool active;
-    bool full;            // the tile lists all 256 pixels: the unit is an 8x4 block, lane j at (j & 7, j >> 3) from lane 0
+    bool full;            // the tile lists all 256 pixels: the unit is slots of an 8x4 block -- lane j at (j & 7, j >> 3) from
+                          // lane 0 IF the list is row-major (StageInfo::rowmajor)
 };
 
 // (sampled tile `it`, pixel group `gi`).  A full tile (256 pixels) is cut into 8x4-pixel blocks
@@ -238,7 +239,8 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                                               const uint32_t* __restrict__ gid_sorted, uint32_t k,
                                               const uint32_t* __restrict__ tiles, const uint32_t* __restrict__ tpo,
                                               const uint32_t* __restrict__ n_contrib, uint32_t* __restrict__ sched,
-                                              int lane, uint32_t lite_max = 0u) {
+                                              int lane, uint32_t lite_max = 0u,
+                                              const uint32_t* __restrict__ pix = nullptr, uint32_t W = 0u) {
     uint32_t gchunk = 0, seq = 0;
     for (;;) {
         uint32_t it = 0;
@@ -250,11 +252,24 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
         const uint32_t t = tiles[it];
         const uint32_t start = tile_offsets[t];
         uint32_t len = tile_offsets[t + 1] - start;
+        uint32_t rowmajor = 0u;
         if (BWD) {
             const uint32_t p0 = tpo[it], m = tpo[it + 1] - p0;
             uint32_t mx = 0;
             for (uint32_t i = lane; i < m; i += 32) mx = max(mx, n_contrib[p0 + i]);
             len = __reduce_max_sync(0xffffffffu, mx);
+            // The backward's separable phase 2 takes a unit's pixels from lane 0's pixel plus a fixed 8x4 offset, which
+            // holds when the tile's 256 pixels are listed row-major (as tgs_sample writes them).  A caller's own list may
+            // be in any order, so the producer -- which has registers to spare and walks the tile's slots anyway --
+            // verifies it once per tile; any other order takes the general phase 2, which reads px, py per pixel.
+            if (m == 256u && pix != nullptr) {
+                const uint32_t id0 = pix[p0];
+                bool ok = id0 % W + 15u < W;  // no wrap into the next image row
+#pragma unroll
+                for (uint32_t i = lane; i < 256u; i += 32)
+                    ok = ok && pix[p0 + i] == id0 + (i >> 4) * W + (i & 15u);
+                rowmajor = __all_sync(0xffffffffu, ok) ? 1u : 0u;
+            }
         }
         uint32_t produced = 0;
         bool first = true;
@@ -312,7 +327,7 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
                 inf.cnt = cnt;
                 inf.hdr = first ? it : kHdrCont;
                 inf.base = BWD ? (len - 1u - produced) : produced;
-                inf.pad = 0;
+                inf.rowmajor = rowmajor;
                 R.info[s] = inf;
             }
             __syncwarp();
@@ -327,7 +342,7 @@ __device__ __forceinline__ void producer_loop(RingT& R, const float4* __restrict
     mbar_wait(&R.empty[s], ((gchunk / RingT::kStages) & 1u) ^ 1u);
     if (lane == 0) {
         StageInfo inf;
-        inf.cnt = 0; inf.hdr = kHdrEnd; inf.base = 0; inf.pad = 0;
+        inf.cnt = 0; inf.hdr = kHdrEnd; inf.base = 0; inf.rowmajor = 0;
         R.info[s] = inf;
         mbar_arrive(&R.full[s]);
         // the last producer to leave re-arms the scheduler counters for the next launch

@@ -221,6 +221,37 @@ def test_raster_bwd_parity(name, orc32, orc64, tgs, torch):
     print(name, f"fragile pixels zeroed: {r.n_fragile}", rep)
 
 
+@pytest.mark.parametrize("name", ["cfg1_full", "small_rot"])
+def test_raster_bwd_takes_a_full_tile_listed_in_any_order(name, orc32, orc64, tgs, torch):
+    """A caller's own pixel list may give a tile's 256 pixels in any order (tgs.h fixes the order of the TILES, not of
+    the pixels inside one).  Per-Gaussian gradients are sums over pixels, so the oracle's result does not change; the
+    backward's fast path for full tiles assumes the row-major order tgs_sample writes and must notice when it is absent."""
+    r = oracle_run(name, orc32, orc64)
+    sc = r.sc
+    tpo = r.samp.tile_pix_offsets.astype(np.int64)
+    rng = np.random.default_rng(3)
+    perm = np.arange(r.samp.n)
+    full = 0
+    for i in range(r.samp.k):
+        if tpo[i + 1] - tpo[i] == 256:
+            # reversed, row-swapped and random orders in turn
+            sl = perm[tpo[i]:tpo[i + 1]]
+            perm[tpo[i]:tpo[i + 1]] = (sl[::-1], sl.reshape(16, 16).T.reshape(-1), rng.permutation(sl))[full % 3]
+            full += 1
+    assert full >= 3
+    splats = dev(pack_splats(r.pre), torch)
+    b, s = binned_dev(r.binned, torch, sc.cam.num_tiles), samp_dev(r.samp, torch)
+    s.pix = dev(r.samp.pix[perm].astype(np.int64), torch, torch.int32)
+    fwd = SimpleNamespace(T=dev(r.fwd.T[perm], torch), n_contrib=dev(r.fwd.n_contrib[perm].astype(np.int64), torch, torch.int32))
+    d = scene_dev(sc, torch)
+    out = tgs.raster_bwd_sparse(sc.cam, sc.sh_degree, splats, b, s, fwd, dev(np.ascontiguousarray(r.g[perm]), torch),
+                                d.means3D, d.scales, d.quats, d.sh, dev(r.pre.radii, torch), dev(r.pre.clamped, torch))
+    torch.cuda.synchronize()
+    rep = check_raster_grads(out.dL_dsplats.cpu().numpy(), r.rbwd)
+    rep.update(check_chain_grads(out, r.pbwd, r.rbwd, r.scale))
+    print(name, f"{full} full tiles listed out of order", rep)
+
+
 @pytest.mark.parametrize("name", ["small_rot", "small_d2", "cfg2", "clamp_vis"])
 def test_raster_bwd_sparse_gradients(name, orc32, orc64, tgs, torch):
     """tgs_raster_bwd_sparse with `touched` (tgs.h, sparse gradients): the mask marks exactly the Gaussians with a
