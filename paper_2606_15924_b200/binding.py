@@ -378,7 +378,7 @@ class TGS:
         # even out of bounds), so it is refused here
         shapes = {"means3D": (N, 3), "scales": (N, 3), "quats": (N, 4), "opacities": (N,), "sh": (N, K, 3)}
         for name, ps, lead in (("grads", grads, (V,)), ("m", m, ()), ("v", v, ()), ("delta", delta, ()), ("params", params, ())):
-            if ps is None:
+            if ps is None or not 0 <= sh_degree <= 3:   # an unsupported degree is the library's to refuse (TGS_ERR_UNSUPPORTED)
                 continue
             for k in PARAM_KEYS:
                 if tuple(ps[k].shape) != lead + shapes[k]:

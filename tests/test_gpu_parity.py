@@ -366,6 +366,36 @@ def test_end_to_end_all_gpu(name, orc32, orc64, tgs, torch):
     print(name, rep)
 
 
+@pytest.mark.parametrize("name", ["small_rot", "cfg2", "clamp_vis"])
+def test_end_to_end_in_north_star_call_order(name, orc32, orc64, tgs, torch):
+    """SparseRasterStep.forward(restrict=False): preprocess, bin EVERY tile, then sample, forward, backward -- the call
+    order BASELINE.json's north_star gives (the default step samples first and bins only the selected tiles).  All on
+    the GPU, no oracle data in between; the full binning is held bit for bit against the oracle's unrestricted lists."""
+    import paper_2606_15924_b200 as pk
+    r = oracle_run(name, orc32, orc64)
+    sc = r.sc
+    d = scene_dev(sc, torch)
+    step = pk.SparseRasterStep(tgs, sc.cam, sc.N, sc.sh_degree, r.binned.P + 1000, want_walked=True)
+    step.forward(d.means3D, d.scales, d.quats, d.opacities, d.sh, sc.tile_pct, sc.pixel_mode, sc.pix_rate,
+                 sc.sample_seed, err=dev(sc.err, torch), restrict=False)
+    P, k, n = step.counts()
+    assert (P, k, n) == (r.binned.P, r.samp.k, r.samp.n)
+    assert np.array_equal(u32(step.binned.tile_offsets), r.binned.tile_offsets)
+    assert np.array_equal(u32(step.binned.gid_sorted)[:P], r.binned.gid_sorted)
+    assert np.array_equal(u32(step.samp.tiles)[:k], r.samp.tiles)
+    assert np.array_equal(u32(step.samp.tile_pix_offsets)[:k + 1], r.samp.tile_pix_offsets)
+    assert np.array_equal(u32(step.samp.pix)[:n], r.samp.pix)
+    rep = check_forward(step.fwd.color[:n].cpu().numpy(), step.fwd.T[:n].cpu().numpy(),
+                        u32(step.fwd.n_contrib)[:n], r.fwd, r.cmax)
+    g = torch.zeros((sc.cam.height * sc.cam.width, 3), device="cuda")
+    g[:n] = dev(r.g, torch)
+    bw = step.backward(g)
+    torch.cuda.synchronize()
+    rep.update(check_raster_grads(bw.dL_dsplats.cpu().numpy(), r.rbwd))
+    rep.update(check_chain_grads(bw, r.pbwd, r.rbwd, r.scale))
+    print(name, "restrict=False", rep)
+
+
 def test_full_mask_equals_dense_and_empty_gradients(orc32, tgs, torch):
     """north_star: a full mask reproduces dense rendering; zero upstream gradient gives zero gradients."""
     sc = workloads.small_random_scene(21, 4000, 250, 130, sh_degree=3, bg=(0.2, 0.1, 0.4), spread=1.4)
