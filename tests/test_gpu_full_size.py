@@ -152,5 +152,25 @@ def test_full_size_config(cfg, pct, orc32, orc64, tgs, torch):
     torch.cuda.synchronize()
     W = st.stats[:, 2].double().sum().item()
     assert np.isclose(W, (1.0 - Tf.astype(np.float64)).sum(), rtol=2e-4)
+    # ---- a property of the whole image, backward: Eq. 1 is linear in the splat colours, so for ANY upstream gradient g
+    #   sum_p g_p . color_p  =  sum_i rgb_i . dL/drgb_i  +  sum_p T_p (bg . g_p)          (per colour channel)
+    # with the GPU's own forward and backward.  g is positive on EVERY sampled pixel of EVERY sampled tile (nothing cancels),
+    # so a tile the backward skipped, replayed short, or credited to the wrong splats shows as a deficit of that tile's
+    # share of the sum (~1/k, 1e-4 at config 4) against rounding of ~1e-7: the bar is 1e-5 of the sum.  (Last: it reuses
+    # the step's gradient buffers.)
+    gall = torch.from_numpy(np.random.default_rng(1000 + cfg).uniform(0.05, 1.0, (n, 3)).astype(np.float32)).cuda()
+    gd.zero_()
+    gd[:n] = gall
+    bw2 = step.backward(gd)
+    torch.cuda.synchronize()
+    rgb, drgb = step.pre.splats[:, 6:9].double(), bw2.dL_dsplats[:, 6:9].double()
+    lhs = (gall.double() * fw.color[:n].double()).sum(0)
+    rhs = (rgb * drgb).sum(0) + torch.tensor(list(cam.bg), dtype=torch.float64, device="cuda") * (fw.T[:n].double()[:, None] * gall.double()).sum(0)
+    lin = ((lhs - rhs).abs() / lhs).max().item()
+    assert lhs.min().item() > 0.01 * n and lin <= 1e-5, (lhs.tolist(), rhs.tolist())
+    n_col = int((drgb != 0).any(1).sum())
+    assert n_col > 1000   # occluded, sub-threshold and between-pixel splats get none (most of the listed ones, as measured)
+    print(f"cfg{cfg} pct={pct}: whole-image colour linearity of the backward (all {k} tiles, {n} pixels, {n_col} of "
+          f"{int(listed.sum())} listed Gaussians with a colour gradient): rel. defect {lin:.2e}")
     print(f"cfg{cfg} pct={pct}: P={P} k={k} n={n} forward {rep}; backward on {sub.k} tiles / {sub.n} pixels "
           f"({n_frag} fragile zeroed, {len(touched)} Gaussians): {rep_b}")
