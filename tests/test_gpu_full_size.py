@@ -174,3 +174,52 @@ def test_full_size_config(cfg, pct, orc32, orc64, tgs, torch):
           f"{int(listed.sum())} listed Gaussians with a colour gradient): rel. defect {lin:.2e}")
     print(f"cfg{cfg} pct={pct}: P={P} k={k} n={n} forward {rep}; backward on {sub.k} tiles / {sub.n} pixels "
           f"({n_frag} fragile zeroed, {len(touched)} Gaussians): {rep_b}")
+
+
+def test_full_size_paper_regime(orc32, tgs, torch):
+    """The paper's own operating point at full size (Sec. 3.5; Tab. 6 at :522-525): 25 pixels in EVERY
+    one of config 4's 8 487 tiles, all tiles binned, 3 M Gaussians -- the regime the warp-per-tile kernels of
+    raster_lite.cu exist for and bench.py's iteration_paper_regime times.  The sampler's lists and the full binning are
+    held bit for bit; the forward is compared on every sampled pixel and the raster backward on every row of every
+    Gaussian, with a non-zero upstream gradient in every tile of the image (fragile pixels zeroed on both sides)."""
+    sc, pre = _scene_and_projection(4, None, orc32)
+    cam = sc.cam
+    W, H = cam.width, cam.height
+    rng = np.random.default_rng(2606)
+    e = (rng.random((H, W)) ** 3 * 4).astype(np.float32)
+    e[rng.random((H, W)) < 0.2] = 0
+    E, A = e.astype(np.float16).view(np.uint16), rng.integers(0, 40, (H, W)).astype(np.uint16)
+    n_pix, n_hard, n_stable = 25, 10, 8
+    samp = orc32.sample_paper(cam, E, A, n_pix, n_hard, n_stable, seed=31)
+    assert samp.k == cam.num_tiles and samp.n > 24 * samp.k
+    binned = orc32.bin_sort(cam, pre)
+    # ---- GPU: projection, the paper's sampler, every tile binned, sparse forward ----
+    d = scene_dev(sc, torch)
+    gpre = tgs.preprocess(cam, sc.sh_degree, d.means3D, d.scales, d.quats, d.opacities, d.sh)
+    sd = tgs.sample_paper(cam, dev(E.view(np.int16), torch), dev(A.view(np.int16), torch), n_pix, n_hard, n_stable, seed=31)
+    assert (sd.k, sd.n) == (samp.k, samp.n)
+    assert np.array_equal(u32(sd.tiles)[:samp.k], samp.tiles)
+    assert np.array_equal(u32(sd.tile_pix_offsets)[:samp.k + 1], samp.tile_pix_offsets)
+    assert np.array_equal(u32(sd.pix)[:samp.n], samp.pix)
+    bd = tgs.bin_sort(cam, gpre.splats, binned.P + 1024)
+    assert bd.P == binned.P
+    assert np.array_equal(u32(bd.tile_offsets), binned.tile_offsets)
+    assert np.array_equal(u32(bd.gid_sorted)[:bd.P], binned.gid_sorted)
+    fw = tgs.raster_fwd_sparse(cam, gpre.splats, bd, sd)
+    torch.cuda.synchronize()
+    n = samp.n
+    ofw = orc32.raster_fwd(cam, binned, pre, samp)
+    rep = check_forward(fw.color[:n].cpu().numpy(), fw.T[:n].cpu().numpy(), u32(fw.n_contrib)[:n], ofw, colour_max(pre, cam))
+    assert (ofw.n_contrib > 0).mean() > 0.3
+    # ---- backward: every tile carries gradient ----
+    g, n_frag = zero_fragile(workloads.dl_dcolor(4, n), ofw)
+    per_tile = np.add.reduceat(np.abs(g).sum(1), samp.tile_pix_offsets[:-1].astype(np.int64))
+    assert (per_tile > 0).all()
+    bw = tgs.raster_bwd_sparse(cam, sc.sh_degree, gpre.splats, bd, sd, fw, dev(g, torch), project=False)
+    torch.cuda.synchronize()
+    orb = orc32.raster_bwd(cam, binned, pre, samp, ofw, g, want_abs=True)
+    rep_b = check_raster_grads(bw.dL_dsplats.cpu().numpy(), orb)
+    reached = int(orb.sum_abs.any(axis=1).sum())
+    assert reached > 100_000
+    print(f"cfg4 paper regime: P={bd.P} k={samp.k} n={n} forward {rep}; backward over all tiles ({n_frag} fragile zeroed, "
+          f"{reached} Gaussians reached): {rep_b}")
