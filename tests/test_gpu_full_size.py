@@ -8,7 +8,10 @@ oracle pass); configs 3 and 5 on a spread of sampled tiles that includes the lon
 pixel lists.  Backward: the upstream gradient is non-zero only on such a spread of tiles (every other pixel then
 contributes exactly zero, so the oracle's backward over the spread is the whole gradient) and EVERY element of every
 gradient array is held to the bar of tests/helpers.py.  Properties that hold at any size cover the rest: sum over the
-image of (1 - T_final) against the statistics forward, exact zeros for Gaussians no sampled tile lists.
+image of (1 - T_final) against the statistics forward, exact zeros for Gaussians no sampled tile lists, and -- for the
+backward over the WHOLE image -- colour linearity of Eq. 1 with a positive upstream gradient on every sampled pixel.
+test_full_size_paper_regime adds the paper's own operating point on config 4's scene (25 pixels in every tile, all tiles
+binned): there the oracle's backward is cheap enough to cover every tile, so every row of all 3 M Gaussians is compared.
 """
 from types import SimpleNamespace
 
